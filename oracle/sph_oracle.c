@@ -1,0 +1,474 @@
+/*
+ * sph_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU statement of what the SPH hot path computes (density sum with
+ * smoothing-length iteration, then the symmetric hydro-force pair sum).  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build,
+ * load or call it.  It shares no code, header, table or helper with the CUDA path in
+ * paper_2003_10850_b200/csrc and neither includes the other.
+ *
+ * Authority.  The paper states the problem only: "computes particle densities by
+ * multiple iterations and the second one computes hydrodynamic forces" (§1), for
+ * a list of active particles "find all neighbouring particles within a given distance"
+ * (§1); the SPH formulation is delegated to its refs [2] and [6] (§1).
+ * Every formula below is therefore a READING, restated from that published lineage and listed
+ * in DESIGN.md §"Readings" (R1..R16, following SURVEY.md §8(c)); the section tags in the
+ * comments name the reading.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): kernel normalisation integral = 1 and
+ * central values 8/pi, 1365/(64 pi); finite-difference derivative identities; equal-mass
+ * identity N_w = (4 pi/3) H^3 rho/m; perfect-lattice values; two-particle hand computation;
+ * brute force == cell list; momentum and energy conservation; viscous heating >= 0; static gas
+ * v_sig = 2 sqrt(gamma (gamma-1) u); permutation / translation / axis-swap / scaling symmetries.
+ * PARITY UNPINNED: the trajectory of the h iteration (which H inside the tolerance band is
+ * returned) is fixed only by the rule R7 written here, not by the paper; its fixed point is
+ * pinned (perfect lattice root, final neighbour number inside the band).
+ *
+ * Summation order: ascending j inside a cell, cells in ascending index order; brute force in
+ * ascending j.  No blocking, fusion or reordering beyond the definitions.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+typedef struct {
+    int kernel;      /* 0 cubic spline, 1 Wendland C6 (R1) */
+    double box;      /* periodic cube edge L */
+    double gamma;    /* adiabatic index */
+    double alpha;    /* artificial viscosity alpha (R9) */
+    int count_mode;  /* 0: kernel-weighted number N_w drives the iteration, 1: integer count (R2) */
+    int max_iter;    /* iteration cap (R7) */
+} orc_params;
+
+/* flags returned per particle by orc_density */
+#define ORC_F_CONVERGED 1
+#define ORC_F_BRACKET 2   /* bracket collapsed */
+#define ORC_F_NOTCONV 4   /* max_iter reached */
+#define ORC_F_STALLED 8   /* update could not move H (cap at 0.49999 L) */
+/* edge-class bits: the fp32 path may legitimately take the other branch */
+#define ORC_E_RADIUS 1    /* some neighbour with |r/H - 1| < 1e-6 at some evaluation */
+#define ORC_E_BAND 2      /* | |N-N_t| - tol | < 1e-4 N_t at some evaluation */
+#define ORC_E_BRANCH 4    /* clamp / bisection / slope guard within 1e-6 of switching */
+
+/* ---------------------------------------------------------------- kernels (R1, R3, R4) */
+/* W(r,H) = sigma H^-3 w(q), q = r/H, H = support radius (W = 0 for q >= 1). */
+static double k_sigma(int k) { return k == 0 ? 8.0 / M_PI : 1365.0 / (64.0 * M_PI); }
+
+static double k_w(int k, double q)
+{
+    if (q >= 1.0) return 0.0;
+    if (k == 0) {
+        if (q <= 0.5) return 1.0 - 6.0 * q * q + 6.0 * q * q * q;
+        double t = 1.0 - q;
+        return 2.0 * t * t * t;
+    } else {
+        double t = 1.0 - q;
+        double t2 = t * t, t4 = t2 * t2, t8 = t4 * t4;
+        return t8 * (1.0 + 8.0 * q + 25.0 * q * q + 32.0 * q * q * q);
+    }
+}
+
+static double k_dw(int k, double q) /* w'(q) */
+{
+    if (q >= 1.0) return 0.0;
+    if (k == 0) {
+        if (q <= 0.5) return -12.0 * q + 18.0 * q * q;
+        double t = 1.0 - q;
+        return -6.0 * t * t;
+    } else {
+        double t = 1.0 - q;
+        double t2 = t * t, t4 = t2 * t2, t7 = t4 * t2 * t;
+        return -22.0 * q * t7 * (1.0 + 7.0 * q + 16.0 * q * q);
+    }
+}
+
+/* exported so the pins can integrate / differentiate them */
+double orc_kernel_w(int k, double q) { return k_w(k, q); }
+double orc_kernel_dw(int k, double q) { return k_dw(k, q); }
+double orc_kernel_sigma(int k) { return k_sigma(k); }
+double orc_W(int k, double r, double H) { return k_sigma(k) / (H * H * H) * k_w(k, r / H); }
+double orc_dWdr(int k, double r, double H) { return k_sigma(k) / (H * H * H * H) * k_dw(k, r / H); }
+double orc_dWdH(int k, double r, double H)
+{
+    double q = r / H;
+    return -k_sigma(k) / (H * H * H * H) * (3.0 * k_w(k, q) + q * k_dw(k, q));
+}
+
+/* ---------------------------------------------------------------- geometry (R11: static periodic box) */
+static inline double min_image(double d, double L)
+{
+    if (d >= 0.5 * L) d -= L;
+    else if (d < -0.5 * L) d += L;
+    return d;
+}
+
+/* uniform periodic grid; used only to skip cells that cannot hold a neighbour */
+typedef struct {
+    int G;
+    double L;
+    int64_t *start; /* G^3 + 1 */
+    int32_t *idx;   /* particle ids, ascending inside a cell */
+    double *hmax;   /* per-cell max support radius (force pass), may be NULL */
+} orc_grid;
+
+static inline int cell_of(const orc_grid *g, double x)
+{
+    int c = (int)floor(x / g->L * g->G);
+    if (c < 0) c = 0;
+    if (c >= g->G) c = g->G - 1;
+    return c;
+}
+
+static orc_grid *grid_build(int64_t n, const float *pos, double L, double cell_hint, const float *h)
+{
+    orc_grid *g = (orc_grid *)calloc(1, sizeof(orc_grid));
+    int G = (int)floor(L / (cell_hint > 0 ? cell_hint : L));
+    if (G < 1) G = 1;
+    if (G > 160) G = 160;
+    g->G = G;
+    g->L = L;
+    int64_t nc = (int64_t)G * G * G;
+    g->start = (int64_t *)calloc(nc + 1, sizeof(int64_t));
+    g->idx = (int32_t *)malloc(sizeof(int32_t) * (n > 0 ? n : 1));
+    g->hmax = h ? (double *)calloc(nc, sizeof(double)) : NULL;
+    int64_t *cnt = (int64_t *)calloc(nc, sizeof(int64_t));
+    for (int64_t i = 0; i < n; i++) {
+        int64_t c = ((int64_t)cell_of(g, pos[3 * i + 2]) * G + cell_of(g, pos[3 * i + 1])) * G + cell_of(g, pos[3 * i]);
+        cnt[c]++;
+        if (h && (double)h[i] > g->hmax[c]) g->hmax[c] = (double)h[i];
+    }
+    for (int64_t c = 0; c < nc; c++) g->start[c + 1] = g->start[c] + cnt[c];
+    memset(cnt, 0, sizeof(int64_t) * nc);
+    for (int64_t i = 0; i < n; i++) {
+        int64_t c = ((int64_t)cell_of(g, pos[3 * i + 2]) * G + cell_of(g, pos[3 * i + 1])) * G + cell_of(g, pos[3 * i]);
+        g->idx[g->start[c] + cnt[c]++] = (int32_t)i;
+    }
+    free(cnt);
+    return g;
+}
+
+static void grid_free(orc_grid *g)
+{
+    if (!g) return;
+    free(g->start);
+    free(g->idx);
+    free(g->hmax);
+    free(g);
+}
+
+/* cells of one axis that can hold a point within R of x: [lo, lo+cnt) modulo G, each at most once */
+static void axis_range(const orc_grid *g, double x, double R, int *lo, int *cnt)
+{
+    double cs = g->L / g->G;
+    int a = (int)floor((x - R) / cs) - 1; /* one cell of slack: pruning only, never correctness */
+    int b = (int)floor((x + R) / cs) + 1;
+    int c = b - a + 1;
+    if (c >= g->G) { *lo = 0; *cnt = g->G; }
+    else { *lo = a; *cnt = c; }
+}
+
+/* minimum distance^2 from point to a cell (periodic), lower bound used for pruning */
+static double cell_mindist2(const orc_grid *g, const double *x, int cx, int cy, int cz)
+{
+    double cs = g->L / g->G, s = 0.0;
+    int c[3] = {cx, cy, cz};
+    for (int a = 0; a < 3; a++) {
+        double centre = (c[a] + 0.5) * cs;
+        double d = fabs(min_image(x[a] - centre, g->L)) - 0.5 * cs;
+        if (d > 0) s += d * d;
+    }
+    return s;
+}
+
+/* ---------------------------------------------------------------- density (R1-R6, R13) */
+typedef struct {
+    double S;      /* sum_j W(r_ij, H)                       */
+    double Dp;     /* sum_j dW/dH(r_ij, H)                   */
+    double rho;    /* sum_j m_j W                            */
+    double drho;   /* sum_j m_j dW/dH                        */
+    double Nw;     /* (4 pi/3) H^3 S                         */
+    int32_t Nint;  /* #{j : r_ij < H}, self included, strict */
+    int edge;      /* some j with |r/H - 1| < 1e-6           */
+} dens_eval;
+
+typedef struct {
+    const orc_params *p;
+    int64_t n;
+    const float *pos;
+    const float *mass; /* NULL -> mass_scalar */
+    double mass_scalar;
+    const orc_grid *grid; /* NULL -> brute force over all j */
+} dens_ctx;
+
+static inline void dens_pair(const dens_ctx *c, const double *xi, double H, int64_t j, dens_eval *e)
+{
+    double L = c->p->box;
+    double dx = min_image(xi[0] - (double)c->pos[3 * j], L);
+    double dy = min_image(xi[1] - (double)c->pos[3 * j + 1], L);
+    double dz = min_image(xi[2] - (double)c->pos[3 * j + 2], L);
+    double r2 = dx * dx + dy * dy + dz * dz;
+    double r = sqrt(r2);
+    if (fabs(r / H - 1.0) < 1e-6) e->edge = 1;
+    if (!(r2 < H * H)) return; /* strict (R4) */
+    double q = r / H;
+    double mj = c->mass ? (double)c->mass[j] : c->mass_scalar;
+    double sg = k_sigma(c->p->kernel);
+    double W = sg / (H * H * H) * k_w(c->p->kernel, q);
+    double dWdH = -sg / (H * H * H * H) * (3.0 * k_w(c->p->kernel, q) + q * k_dw(c->p->kernel, q));
+    e->S += W;
+    e->Dp += dWdH;
+    e->rho += mj * W;
+    e->drho += mj * dWdH;
+    e->Nint += 1;
+}
+
+static void dens_at(const dens_ctx *c, int64_t i, double H, dens_eval *e)
+{
+    memset(e, 0, sizeof(*e));
+    double xi[3] = {(double)c->pos[3 * i], (double)c->pos[3 * i + 1], (double)c->pos[3 * i + 2]};
+    if (!c->grid) {
+        for (int64_t j = 0; j < c->n; j++) dens_pair(c, xi, H, j, e); /* self term j = i included (R5) */
+    } else {
+        const orc_grid *g = c->grid;
+        int lo[3], cnt[3];
+        for (int a = 0; a < 3; a++) axis_range(g, xi[a], H * (1.0 + 2e-6), &lo[a], &cnt[a]);
+        for (int kz = 0; kz < cnt[2]; kz++)
+            for (int ky = 0; ky < cnt[1]; ky++)
+                for (int kx = 0; kx < cnt[0]; kx++) {
+                    int cx = ((lo[0] + kx) % g->G + g->G) % g->G;
+                    int cy = ((lo[1] + ky) % g->G + g->G) % g->G;
+                    int cz = ((lo[2] + kz) % g->G + g->G) % g->G;
+                    int64_t cc = ((int64_t)cz * g->G + cy) * g->G + cx;
+                    for (int64_t s = g->start[cc]; s < g->start[cc + 1]; s++) dens_pair(c, xi, H, g->idx[s], e);
+                }
+    }
+    e->Nw = 4.0 * M_PI / 3.0 * H * H * H * e->S;
+}
+
+/* One evaluation at the given support radii (h[i], fp32 input promoted) for the listed particles. */
+int orc_density_eval(const orc_params *p, int64_t n, const float *pos, const float *mass, double mass_scalar,
+                     const float *h, const int32_t *active, int64_t n_active, int brute, double cell_hint,
+                     double *S, double *Dp, double *rho, double *drho, double *Nw, int32_t *Nint, uint8_t *edge)
+{
+    orc_grid *g = brute ? NULL : grid_build(n, pos, p->box, cell_hint, NULL);
+    dens_ctx c = {p, n, pos, mass, mass_scalar, g};
+    int64_t na = active ? n_active : n;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        dens_eval e;
+        dens_at(&c, i, (double)h[i], &e);
+        S[a] = e.S; Dp[a] = e.Dp; rho[a] = e.rho; drho[a] = e.drho; Nw[a] = e.Nw; Nint[a] = e.Nint;
+        if (edge) edge[a] = (uint8_t)(e.edge ? ORC_E_RADIUS : 0);
+    }
+    grid_free(g);
+    return 0;
+}
+
+/*
+ * The h iteration (R7; "computes particle densities by multiple iterations", §1).
+ * Per active particle, independently: safeguarded Newton iteration on
+ *   G(H) = (4 pi/3) H^3 S(H) - N_t,   G' = (3 N_w / H) (1 + H S'/(3 S)),
+ * so H - G/G' = H [1 - (N_w - N_t)/(3 N_w) g],  g = 1/(1 + H D'/(3 S)).
+ * With count_mode 1 the integer count N_int replaces N_w in the same expressions.
+ */
+int orc_density(const orc_params *p, int64_t n, const float *pos, const float *mass, double mass_scalar,
+                const float *h_guess, const int32_t *active, int64_t n_active, double n_target, double n_tol,
+                int brute, double cell_hint,
+                double *H_out, double *rho, double *omega, double *Nw_out, int32_t *Nint, int32_t *iters,
+                int32_t *flags, uint8_t *edge, int64_t *n_evals_total)
+{
+    orc_grid *g = brute ? NULL : grid_build(n, pos, p->box, cell_hint, NULL);
+    dens_ctx c = {p, n, pos, mass, mass_scalar, g};
+    int64_t na = active ? n_active : n;
+    const double smin = pow(2.0, -1.0 / 3.0), smax = pow(2.0, 1.0 / 3.0);
+    const double Hcap = 0.49999 * p->box;
+    int64_t evals = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : evals)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        double H = (double)h_guess[i], lo = 0.0, hi = INFINITY;
+        int it = 0, flag = 0, eb = 0;
+        dens_eval e;
+        for (;;) {
+            dens_at(&c, i, H, &e);
+            it++;
+            evals++;
+            if (e.edge) eb |= ORC_E_RADIUS;
+            double N = p->count_mode ? (double)e.Nint : e.Nw;
+            double dev = fabs(N - n_target);
+            if (isfinite(n_tol) && fabs(dev - n_tol) < 1e-4 * n_target) eb |= ORC_E_BAND;
+            if (dev <= n_tol) { flag = ORC_F_CONVERGED; break; } /* inclusive */
+            if (it >= p->max_iter) { flag = ORC_F_NOTCONV; break; }
+            if (N < n_target) { if (H > lo) lo = H; } else { if (H < hi) hi = H; }
+            if (isfinite(hi) && lo > 0.0) {
+                if (fabs((hi - lo) - 1e-6 * lo) < 1e-9 * lo) eb |= ORC_E_BRANCH;
+                if (hi - lo <= 1e-6 * lo) { flag = ORC_F_BRACKET; break; }
+            }
+            double gsl = 1.0 / (1.0 + H * e.Dp / (3.0 * e.S));
+            if (fabs(gsl) < 1e-6 || fabs(gsl - 4.0) < 1e-6) eb |= ORC_E_BRANCH;
+            if (!(gsl > 0.0 && gsl < 4.0) || N == 0.0) gsl = 1.0;
+            double s = (N == 0.0) ? smax : 1.0 - (N - n_target) / (3.0 * N) * gsl;
+            if (fabs(s - smin) < 1e-6 || fabs(s - smax) < 1e-6) eb |= ORC_E_BRANCH;
+            if (s < smin) s = smin;
+            if (s > smax) s = smax;
+            double Hn = H * s;
+            if (isfinite(hi) && lo > 0.0) {
+                if (fabs(Hn - lo) < 1e-6 * lo || fabs(Hn - hi) < 1e-6 * hi) eb |= ORC_E_BRANCH;
+                if (!(lo < Hn && Hn < hi)) Hn = cbrt(0.5 * (lo * lo * lo + hi * hi * hi)); /* volume bisection */
+            }
+            if (Hn > Hcap) Hn = Hcap;
+            if (Hn == H) { flag = ORC_F_STALLED; break; }
+            H = Hn;
+        }
+        H_out[a] = H;
+        rho[a] = e.rho;
+        omega[a] = 1.0 + H / (3.0 * e.rho) * e.drho; /* grad-h factor Omega (R1) */
+        Nw_out[a] = e.Nw;
+        Nint[a] = e.Nint;
+        iters[a] = it;
+        flags[a] = flag;
+        if (edge) edge[a] = (uint8_t)eb;
+    }
+    if (n_evals_total) *n_evals_total = evals;
+    grid_free(g);
+    return 0;
+}
+
+/* ---------------------------------------------------------------- hydro force (R8-R12) */
+/*
+ * For every active i, over all j != i with r_ij < max(H_i, H_j):
+ *   F_ij(H) = dW/dr(r_ij, H) (0 for r >= H), rhat = d_ij / r, v_ij = v_i - v_j,
+ *   mu = min(0, v_ij.rhat), v_sig,ij = c_i + c_j - 3 mu, Pi = -(alpha/2) v_sig mu / rhobar,
+ *   Fbar = (F_ij(H_i) + F_ij(H_j))/2,  A_k = P_k / (Omega_k rho_k^2), P = (gamma-1) rho u,
+ *   a_i     = - sum_j m_j [A_i F_ij(H_i) + A_j F_ij(H_j) + Pi Fbar] rhat
+ *   du_i/dt =   sum_j m_j [A_i F_ij(H_i) + Pi Fbar / 2] (v_ij.rhat)
+ *   vsig_i  =   max_j v_sig,ij   (0 if the set is empty)
+ * Coincident pairs (r = 0, j != i) give nothing to a, du/dt and c_i + c_j to vsig.
+ * Inactive neighbours enter with their current (h, rho, Omega, u, v) (R12).
+ */
+typedef struct {
+    double a[3], du, vsig;
+    double asum, dusum; /* sums of |pair term| for the parity tolerance floor (R15) */
+    double duvisc;      /* viscous part of du/dt (pin: >= 0) */
+    int64_t npair;
+    int edge;
+} force_acc;
+
+typedef struct {
+    const orc_params *p;
+    int64_t n;
+    const float *pos, *vel, *u, *mass, *h, *rho, *omega;
+    double mass_scalar;
+} force_ctx;
+
+static inline void force_pair(const force_ctx *c, int64_t i, int64_t j, force_acc *f)
+{
+    if (j == i) return;
+    const orc_params *p = c->p;
+    double L = p->box;
+    double d[3];
+    for (int a = 0; a < 3; a++) d[a] = min_image((double)c->pos[3 * i + a] - (double)c->pos[3 * j + a], L);
+    double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    double Hi = (double)c->h[i], Hj = (double)c->h[j];
+    double Hm = Hi > Hj ? Hi : Hj;
+    double r = sqrt(r2);
+    if (fabs(r / Hm - 1.0) < 1e-6) f->edge = 1;
+    if (!(r2 < Hm * Hm)) return;
+    double gm1 = p->gamma - 1.0;
+    double ci = sqrt(p->gamma * gm1 * (double)c->u[i]), cj = sqrt(p->gamma * gm1 * (double)c->u[j]);
+    f->npair++;
+    if (r == 0.0) {
+        if (ci + cj > f->vsig) f->vsig = ci + cj;
+        return;
+    }
+    double rhoi = (double)c->rho[i], rhoj = (double)c->rho[j];
+    double Ai = gm1 * (double)c->u[i] / ((double)c->omega[i] * rhoi);
+    double Aj = gm1 * (double)c->u[j] / ((double)c->omega[j] * rhoj);
+    double mj = c->mass ? (double)c->mass[j] : c->mass_scalar;
+    double sg = k_sigma(p->kernel);
+    double Fi = r < Hi ? sg / (Hi * Hi * Hi * Hi) * k_dw(p->kernel, r / Hi) : 0.0;
+    double Fj = r < Hj ? sg / (Hj * Hj * Hj * Hj) * k_dw(p->kernel, r / Hj) : 0.0;
+    double rh[3] = {d[0] / r, d[1] / r, d[2] / r};
+    double vr = 0.0;
+    for (int a = 0; a < 3; a++) vr += ((double)c->vel[3 * i + a] - (double)c->vel[3 * j + a]) * rh[a];
+    double mu = vr < 0.0 ? vr : 0.0;
+    double vs = ci + cj - 3.0 * mu;
+    double Pi = -0.5 * p->alpha * vs * mu / (0.5 * (rhoi + rhoj));
+    double Fbar = 0.5 * (Fi + Fj);
+    double t = mj * (Ai * Fi + Aj * Fj + Pi * Fbar);
+    for (int a = 0; a < 3; a++) f->a[a] -= t * rh[a];
+    f->asum += fabs(t);
+    double e = mj * (Ai * Fi + 0.5 * Pi * Fbar) * vr;
+    f->du += e;
+    f->dusum += fabs(e);
+    f->duvisc += mj * 0.5 * Pi * Fbar * vr;
+    if (vs > f->vsig) f->vsig = vs;
+}
+
+int orc_hydro_force(const orc_params *p, int64_t n, const float *pos, const float *vel, const float *u,
+                    const float *mass, double mass_scalar, const float *h, const float *rho, const float *omega,
+                    const int32_t *active, int64_t n_active, int brute, double cell_hint,
+                    double *acc, double *dudt, double *vsig, double *asum, double *dusum, double *duvisc,
+                    int64_t *npair, uint8_t *edge)
+{
+    orc_grid *g = brute ? NULL : grid_build(n, pos, p->box, cell_hint, h);
+    force_ctx c = {p, n, pos, vel, u, mass, h, rho, omega, mass_scalar};
+    double hglob = 0.0;
+    for (int64_t i = 0; i < n; i++)
+        if ((double)h[i] > hglob) hglob = (double)h[i];
+    int64_t na = active ? n_active : n;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        force_acc f;
+        memset(&f, 0, sizeof(f));
+        if (!g) {
+            for (int64_t j = 0; j < n; j++) force_pair(&c, i, j, &f);
+        } else {
+            double xi[3] = {(double)pos[3 * i], (double)pos[3 * i + 1], (double)pos[3 * i + 2]};
+            double Hi = (double)h[i];
+            int lo[3], cnt[3];
+            for (int ax = 0; ax < 3; ax++) axis_range(g, xi[ax], hglob * (1.0 + 2e-6), &lo[ax], &cnt[ax]);
+            for (int kz = 0; kz < cnt[2]; kz++)
+                for (int ky = 0; ky < cnt[1]; ky++)
+                    for (int kx = 0; kx < cnt[0]; kx++) {
+                        int cx = ((lo[0] + kx) % g->G + g->G) % g->G;
+                        int cy = ((lo[1] + ky) % g->G + g->G) % g->G;
+                        int cz = ((lo[2] + kz) % g->G + g->G) % g->G;
+                        int64_t cc = ((int64_t)cz * g->G + cy) * g->G + cx;
+                        if (g->start[cc] == g->start[cc + 1]) continue;
+                        double reach = (Hi > g->hmax[cc] ? Hi : g->hmax[cc]) * (1.0 + 2e-6);
+                        if (cell_mindist2(g, xi, cx, cy, cz) > reach * reach) continue; /* pruning only */
+                        for (int64_t s = g->start[cc]; s < g->start[cc + 1]; s++) force_pair(&c, i, g->idx[s], &f);
+                    }
+        }
+        acc[3 * a] = f.a[0]; acc[3 * a + 1] = f.a[1]; acc[3 * a + 2] = f.a[2];
+        dudt[a] = f.du; vsig[a] = f.vsig;
+        if (asum) asum[a] = f.asum;
+        if (dusum) dusum[a] = f.dusum;
+        if (duvisc) duvisc[a] = f.duvisc;
+        if (npair) npair[a] = f.npair;
+        if (edge) edge[a] = (uint8_t)(f.edge ? ORC_E_RADIUS : 0);
+    }
+    grid_free(g);
+    return 0;
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
