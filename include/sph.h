@@ -1,0 +1,162 @@
+/*
+ * sph.h -- C ABI of libsph.so: the data-parallel hot path of Gadget3's SPH modules on one B200.
+ *
+ * The paper states the problem, not an API: every module "compute[s] the force acting on a list of
+ * active particles by performing a tree walk over groups of one or more active particles and find[s]
+ * all neighbouring particles within a given distance" (§1); SPH is two such modules,
+ * "the first one computes particle densities by multiple iterations and the second one computes
+ * hydrodynamic forces" (§1).  The three calls below are that statement:
+ * sph_build_index (the structure the neighbour search walks), sph_density (active list, neighbour
+ * number target, tolerance) and sph_hydro_force (active list).  The SPH formulas themselves are the
+ * readings R1..R16 of DESIGN.md (the paper prints none).
+ *
+ * Conventions
+ *  - All array arguments are DEVICE pointers (caller-owned, e.g. torch tensors) unless the name ends
+ *    in _host.  The library never frees or reallocates caller arrays; it writes only the entries of
+ *    ACTIVE particles, indexed by the caller's particle id.  Sorted copies, the octree and scratch
+ *    are private to the context.
+ *  - Work is enqueued on the CUDA stream given to sph_create.  sph_build_index synchronises once
+ *    (it reads back the octree size); sph_density synchronises once (to return n_unconverged);
+ *    sph_hydro_force is fully asynchronous.  The *_host entry points synchronise before returning.
+ *  - Geometry: periodic cube [0, box)^3, minimum-image distances, support radius H < box/2.
+ *    H is the radius at which the kernel reaches zero (W = 0 for r >= H).
+ *  - Errors are return codes (sph_status); no exceptions, no abort, no printing.  A sticky CUDA error
+ *    is reported by every later call; sph_last_error describes the most recent failure.
+ *  - There is no CPU fallback and no other backend: without a CUDA device every call that needs one
+ *    returns SPH_E_CUDA.
+ */
+#ifndef SPH_H_
+#define SPH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sph_ctx sph_ctx; /* opaque; owns index + scratch only */
+
+typedef enum {
+    SPH_OK = 0,
+    SPH_E_ARG = 1,      /* bad argument (NULL pointer, n < 0, unknown kernel, ...) */
+    SPH_E_CUDA = 2,     /* CUDA runtime error (see sph_last_error) */
+    SPH_E_NOINDEX = 3,  /* sph_density / sph_hydro_force before sph_build_index */
+    SPH_E_OOM = 4,      /* device allocation failed */
+    SPH_E_INTERNAL = 5, /* an internal capacity was exceeded (reported, never silent) */
+    SPH_W_NOCONV = 16   /* warning: some active particles stopped without |N - N_t| <= tol */
+} sph_status;
+
+enum { SPH_KERNEL_CUBIC = 0, SPH_KERNEL_WC6 = 1 };
+
+/* per-particle status word written by sph_density: low 8 bits = evaluations used, then flags */
+enum {
+    SPH_ST_CONVERGED = 1 << 8, /* |N - N_t| <= tol at the returned H */
+    SPH_ST_BRACKET = 1 << 9,   /* bracket [lo,hi] collapsed to 1e-6 relative (count jumps over the band) */
+    SPH_ST_NOTCONV = 1 << 10,  /* max_iter evaluations used */
+    SPH_ST_STALLED = 1 << 11   /* H pinned at the cap 0.49999 box */
+};
+
+typedef struct {
+    int kernel;        /* SPH_KERNEL_CUBIC or SPH_KERNEL_WC6 (R1) */
+    float box;         /* periodic cube edge L > 0 */
+    float gamma;       /* adiabatic index (5/3) */
+    float alpha_visc;  /* artificial viscosity alpha (1.0), R9 */
+    int count_mode;    /* 0: kernel-weighted neighbour number drives the h iteration, 1: integer count (R2) */
+    int max_iter;      /* cap on evaluations per particle (64); 1..255 */
+    int leaf_cap;      /* octree leaf capacity = max active particles per group; 0 = default (32); <= 32 */
+} sph_params;
+
+typedef struct {
+    int64_t n;                 /* particles in the index */
+    int64_t n_nodes;           /* octree nodes */
+    int64_t n_groups;          /* groups (leaf chunks) of the all-active case */
+    int64_t launches;          /* kernels launched by this context so far (ours + CUB passes) */
+    /* counters of the most recent sph_density call */
+    int64_t dens_evals;        /* particle evaluations (sum over particles of iterations used) */
+    int64_t dens_candidates;   /* distance tests */
+    int64_t dens_pairs;        /* true pairs (r < H), self included */
+    /* counters of the most recent sph_hydro_force call */
+    int64_t force_candidates;
+    int64_t force_pairs;       /* true pairs r < max(H_i,H_j), self excluded */
+} sph_stats;
+
+/* Create a context. `cuda_stream` is a cudaStream_t (NULL = legacy default stream). */
+int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream);
+int sph_destroy(sph_ctx *ctx);
+
+/*
+ * Build the spatial index over n particles (steps a1-a5 of DESIGN.md): 48-bit Morton keys
+ * (16 bits per axis), radix sort of (key, id), sorted float4 copy (x,y,z,m), inverse permutation,
+ * an octree over the sorted order whose leaves hold <= leaf_cap particles, and the leaf-chunk group
+ * list.  Replaces the paper's Hilbert keys + domain decomposition + tree build (§1,
+ * :194-196 §4).
+ *   pos   [n*3] device, x,y,z per particle, 0 <= x < box (values outside are clamped into the
+ *         boundary cells for the search and otherwise used as given);
+ *   mass  [n] device or NULL; if NULL every particle has mass_scalar.
+ * n = 0 is valid (later calls do nothing).  Synchronises the stream once.
+ */
+int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar);
+
+/*
+ * SPH density with the smoothing-length iteration (steps a5-a9; R1-R7):
+ * for every active particle, starting from h[id], iterate the safeguarded Newton rule of R7 on the
+ * support radius until the neighbour number N (kernel-weighted, or integer with count_mode 1)
+ * satisfies |N - n_ngb_target| <= n_ngb_tol, then write
+ *   h[id]         converged support radius,
+ *   rho[id]       sum_j m_j W(r_ij, H_i)  (self term included),
+ *   omega[id]     1 + (H_i / 3 rho_i) d rho_i / d H_i,
+ *   ngb_count[id] integer count #{j : r_ij < H_i} at the returned H (self included),
+ *   status[id]    evaluations used | SPH_ST_* flags (status may be NULL).
+ *   active        [n_active] device int32 particle ids (unique, in range) or NULL = all particles
+ *                 (then n_active is ignored);
+ *   n_ngb_tol     +inf means "evaluate once at the given h";
+ *   n_unconverged_host  HOST pointer (may be NULL): number of active particles that stopped
+ *                 without SPH_ST_CONVERGED.
+ * Returns SPH_OK, or SPH_W_NOCONV if *n_unconverged_host would be > 0.  Synchronises once.
+ */
+int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol,
+                float *h, float *rho, float *omega, int32_t *ngb_count, int32_t *status,
+                int64_t *n_unconverged_host);
+
+/*
+ * Symmetric SPH hydro-force pair sum (steps a5, a6, a10, a11; R8-R12): for every active
+ * particle i, over all j != i with r_ij < max(H_i, H_j),
+ *   acc[id*3..]  = - sum_j m_j [A_i F_ij(H_i) + A_j F_ij(H_j) + Pi_ij Fbar_ij] rhat_ij
+ *   dudt[id]     =   sum_j m_j [A_i F_ij(H_i) + Pi_ij Fbar_ij / 2] (v_ij . rhat_ij)
+ *   vsig_max[id] =   max_j (c_i + c_j - 3 min(0, v_ij . rhat_ij))     (0 if no neighbour)
+ * with A = (gamma-1) u / (omega rho), F_ij(H) = dW/dr(r_ij, H), Pi_ij the signal-velocity viscosity.
+ *   vel [n*3], u [n], h [n], rho [n], omega [n]: device, valid for ALL n particles (inactive
+ *   neighbours contribute with their current values, R12); acc [n*3], dudt [n], vsig_max [n]: device,
+ *   written for active particles only.  Asynchronous.
+ */
+int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
+                    const float *h, const float *rho, const float *omega, float *acc, float *dudt,
+                    float *vsig_max);
+
+/*
+ * One whole pass of the hot path with HOST buffers (used for the end-to-end measurement): copies
+ * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
+ * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries
+ * of inactive particles of the outputs rho..vsig_max are unspecified unless the caller pre-filled the
+ * device state through an earlier call), and synchronises.  All pointers are HOST pointers (pinned
+ * memory makes the copies asynchronous); `active_host` may be NULL (all active).
+ */
+int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *vel_host, const float *u_host,
+                  float mass_scalar, const int32_t *active_host, int64_t n_active, float n_ngb_target,
+                  float n_ngb_tol, float *h_host /* in: guess, out */, float *rho_host, float *omega_host,
+                  int32_t *ngb_count_host, float *acc_host, float *dudt_host, float *vsig_host,
+                  int64_t *n_unconverged_host);
+
+/* Counters of the last calls (host struct filled; synchronises the stream). */
+int sph_get_stats(sph_ctx *ctx, sph_stats *out_host);
+
+/* Text of the most recent error of this context ("" if none). Never NULL; valid until the next call. */
+const char *sph_last_error(const sph_ctx *ctx);
+
+/* Library version string and the compute capability it was built for ("sm_100a"). */
+const char *sph_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_H_ */

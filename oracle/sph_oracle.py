@@ -111,6 +111,9 @@ def density_eval(pos, h, *, kernel, box=1.0, mass=None, mass_scalar=1.0, active=
     lib().orc_density_eval(C.byref(prm), C.c_int64(n), ppos, pm, C.c_double(mass_scalar), ph, pact,
                            C.c_int64(na), C.c_int(int(brute)), C.c_double(cell_hint),
                            *[out[k].ctypes.data_as(C.c_void_p) for k in ("S", "Dp", "rho", "drho", "Nw", "Nint", "edge")])
+    H = h_.astype(np.float64) if act_ is None else h_.astype(np.float64)[act_]
+    out["H"] = H
+    out["omega"] = 1.0 + H / (3.0 * out["rho"]) * out["drho"]  # grad-h factor (R1), as in orc_density
     return out
 
 

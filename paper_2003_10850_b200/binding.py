@@ -1,0 +1,177 @@
+"""Thin ctypes binding of libsph.so (include/sph.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for device
+memory and streams.  There is no CPU fallback: if libsph.so is missing or no CUDA device is
+present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsph.so")
+
+SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL, SPH_W_NOCONV = 0, 1, 2, 3, 4, 5, 16
+ST_CONVERGED, ST_BRACKET, ST_NOTCONV, ST_STALLED = 1 << 8, 1 << 9, 1 << 10, 1 << 11
+KERNEL_CUBIC, KERNEL_WC6 = 0, 1
+
+EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
+           "sph_get_stats", "sph_last_error", "sph_version"]
+
+
+class SphParams(C.Structure):
+    _fields_ = [("kernel", C.c_int), ("box", C.c_float), ("gamma", C.c_float), ("alpha_visc", C.c_float),
+                ("count_mode", C.c_int), ("max_iter", C.c_int), ("leaf_cap", C.c_int)]
+
+
+class SphStats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("n", "n_nodes", "n_groups", "launches", "dens_evals", "dens_candidates",
+                                         "dens_pairs", "force_candidates", "force_pairs")]
+
+
+class SphError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libsph status {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Load libsph.so (built in-tree by paper_2003_10850_b200/build.py). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built: run `python -m paper_2003_10850_b200.build` "
+                                    "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.sph_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(SphParams), C.c_void_p]
+        lib.sph_destroy.argtypes = [C.c_void_p]
+        lib.sph_build_index.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_float]
+        lib.sph_density.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float] + [C.c_void_p] * 5 + \
+                                   [C.POINTER(C.c_int64)]
+        lib.sph_hydro_force.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 8
+        lib.sph_step_host.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
+                                      C.c_int64, C.c_float, C.c_float] + [C.c_void_p] * 7 + [C.POINTER(C.c_int64)]
+        lib.sph_get_stats.argtypes = [C.c_void_p, C.POINTER(SphStats)]
+        lib.sph_last_error.argtypes = [C.c_void_p]
+        lib.sph_last_error.restype = C.c_char_p
+        lib.sph_version.restype = C.c_char_p
+        for name in EXPORTS[:7]:
+            getattr(lib, name).restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+def _dev(t, dtype, name, numel=None):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host(t, dtype, name, numel):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CPU tensor of dtype {dtype}")
+    if t.numel() != numel:
+        raise ValueError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Sph:
+    """One libsph context (sph_create ... sph_destroy) bound to a torch CUDA stream."""
+
+    def __init__(self, kernel=KERNEL_CUBIC, box=1.0, gamma=5.0 / 3.0, alpha_visc=1.0, count_mode=0, max_iter=64,
+                 leaf_cap=0, stream: "torch.cuda.Stream | None" = None):
+        self._lib = load()
+        self._h = C.c_void_p()
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        p = SphParams(kernel, box, gamma, alpha_visc, count_mode, max_iter, leaf_cap)
+        rc = self._lib.sph_create(C.byref(self._h), C.byref(p), C.c_void_p(self.stream.cuda_stream))
+        if rc != SPH_OK:
+            self._h = C.c_void_p()
+            raise SphError(rc, "sph_create failed (no CUDA device? there is no CPU fallback)")
+        self.n = 0
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self._lib.sph_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, allow=(SPH_OK,)):
+        if rc not in allow:
+            raise SphError(rc, self._lib.sph_last_error(self._h).decode())
+        return rc
+
+    # -- the three calls of the paper's statement of the problem -------------------------------
+    def sph_build_index(self, pos, mass=None, mass_scalar=1.0):
+        n = pos.shape[0]
+        self._check(self._lib.sph_build_index(self._h, n, _dev(pos, torch.float32, "pos", 3 * n),
+                                              _dev(mass, torch.float32, "mass", n), float(mass_scalar)))
+        self.n = n
+
+    def sph_density(self, h, rho, omega, ngb_count, n_ngb_target, n_ngb_tol, active=None, status=None):
+        """Returns the number of active particles that stopped without convergence."""
+        n = self.n
+        na = 0 if active is None else active.numel()
+        unconv = C.c_int64(0)
+        self._check(self._lib.sph_density(self._h, _dev(active, torch.int32, "active"), na, float(n_ngb_target),
+                                          float(n_ngb_tol), _dev(h, torch.float32, "h", n),
+                                          _dev(rho, torch.float32, "rho", n), _dev(omega, torch.float32, "omega", n),
+                                          _dev(ngb_count, torch.int32, "ngb_count", n),
+                                          _dev(status, torch.int32, "status", n), C.byref(unconv)),
+                    allow=(SPH_OK, SPH_W_NOCONV))
+        return int(unconv.value)
+
+    def sph_hydro_force(self, vel, u, h, rho, omega, acc, dudt, vsig_max, active=None):
+        n = self.n
+        na = 0 if active is None else active.numel()
+        self._check(self._lib.sph_hydro_force(self._h, _dev(active, torch.int32, "active"), na,
+                                              _dev(vel, torch.float32, "vel", 3 * n), _dev(u, torch.float32, "u", n),
+                                              _dev(h, torch.float32, "h", n), _dev(rho, torch.float32, "rho", n),
+                                              _dev(omega, torch.float32, "omega", n),
+                                              _dev(acc, torch.float32, "acc", 3 * n),
+                                              _dev(dudt, torch.float32, "dudt", n),
+                                              _dev(vsig_max, torch.float32, "vsig_max", n)))
+
+    def sph_step_host(self, pos, vel, u, mass_scalar, h, rho, omega, ngb_count, acc, dudt, vsig, n_ngb_target,
+                      n_ngb_tol, active=None):
+        """Whole pass with HOST (ideally pinned) tensors; returns the unconverged count."""
+        n = pos.shape[0]
+        na = 0 if active is None else active.numel()
+        unconv = C.c_int64(0)
+        f32, i32 = torch.float32, torch.int32
+        self._check(self._lib.sph_step_host(self._h, n, _host(pos, f32, "pos", 3 * n), _host(vel, f32, "vel", 3 * n),
+                                            _host(u, f32, "u", n), float(mass_scalar),
+                                            _host(active, i32, "active", na), na, float(n_ngb_target), float(n_ngb_tol),
+                                            _host(h, f32, "h", n), _host(rho, f32, "rho", n),
+                                            _host(omega, f32, "omega", n), _host(ngb_count, i32, "ngb_count", n),
+                                            _host(acc, f32, "acc", 3 * n), _host(dudt, f32, "dudt", n),
+                                            _host(vsig, f32, "vsig", n), C.byref(unconv)),
+                    allow=(SPH_OK, SPH_W_NOCONV))
+        self.n = n
+        return int(unconv.value)
+
+    def stats(self) -> dict:
+        s = SphStats()
+        self._check(self._lib.sph_get_stats(self._h, C.byref(s)))
+        return {k: int(getattr(s, k)) for k, _ in SphStats._fields_}
+
+
+def version() -> str:
+    return load().sph_version().decode()

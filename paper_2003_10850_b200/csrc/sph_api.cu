@@ -1,0 +1,229 @@
+// sph_api.cu -- the C ABI of include/sph.h: argument checks, buffer ownership, call sequencing.
+#include <math.h>
+#include <stdarg.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "sph_internal.cuh"
+
+int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+namespace {
+
+template <typename T>
+void dfree(T *&p)
+{
+    if (p) cudaFree(p);
+    p = nullptr;
+}
+
+int check_sticky(sph_ctx *ctx)
+{
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) return sph_fail(ctx, SPH_E_CUDA, "sticky CUDA error: %s", cudaGetErrorString(e));
+    return SPH_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+const char *sph_version(void) { return "libsph 0.1 (sm_100a)"; }
+
+const char *sph_last_error(const sph_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream)
+{
+    if (!out || !p) return SPH_E_ARG;
+    *out = nullptr;
+    if (p->kernel != SPH_KERNEL_CUBIC && p->kernel != SPH_KERNEL_WC6) return SPH_E_ARG;
+    if (!(p->box > 0.f) || !(p->gamma > 1.f) || !(p->alpha_visc >= 0.f)) return SPH_E_ARG;
+    if (p->max_iter < 1 || p->max_iter > 255 || p->leaf_cap < 0 || p->leaf_cap > SPH_MAXB) return SPH_E_ARG;
+    if (p->count_mode != 0 && p->count_mode != 1) return SPH_E_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return SPH_E_CUDA; // no CUDA device: there is no CPU fallback
+    }
+    sph_ctx *ctx = (sph_ctx *)calloc(1, sizeof(sph_ctx));
+    if (!ctx) return SPH_E_OOM;
+    ctx->prm = *p;
+    ctx->leaf_cap = p->leaf_cap ? p->leaf_cap : SPH_MAXB;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        free(ctx);
+        return SPH_E_CUDA;
+    }
+    ctx->device_sms = prop.multiProcessorCount;
+    if (cudaMalloc((void **)&ctx->cnt, sizeof(SphCounters)) != cudaSuccess) {
+        free(ctx);
+        return SPH_E_OOM;
+    }
+    cudaMemsetAsync(ctx->cnt, 0, sizeof(SphCounters), ctx->stream);
+    *out = ctx;
+    return SPH_OK;
+}
+
+int sph_destroy(sph_ctx *ctx)
+{
+    if (!ctx) return SPH_E_ARG;
+    cudaStreamSynchronize(ctx->stream);
+    dfree(ctx->keys); dfree(ctx->keys_alt); dfree(ctx->perm); dfree(ctx->perm_alt); dfree(ctx->inv);
+    dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->grp_start);
+    dfree(ctx->cnt); dfree(ctx->cub_tmp); dfree(ctx->f_xyzh); dfree(ctx->f_vc); dfree(ctx->f_raf);
+    dfree(ctx->node_hmax); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
+    dfree(ctx->agrp_start);
+    dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
+    dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
+    free(ctx);
+    return SPH_OK;
+}
+
+int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar)
+{
+    if (!ctx) return SPH_E_ARG;
+    if (n < 0 || n > 0x7fffff00ll || (n > 0 && !pos)) return sph_fail(ctx, SPH_E_ARG, "sph_build_index: bad n or pos");
+    if (!mass && !(mass_scalar > 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_build_index: mass_scalar must be > 0");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    ctx->have_index = false;
+    ctx->n = n;
+    ctx->has_mass = mass != nullptr;
+    ctx->mass_scalar = mass ? 1.f : mass_scalar;
+    ctx->err[0] = 0;
+    return sph_index_build(ctx, pos, mass);
+}
+
+int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol, float *h,
+                float *rho, float *omega, int32_t *ngb_count, int32_t *status, int64_t *n_unconverged_host)
+{
+    if (!ctx) return SPH_E_ARG;
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_density before sph_build_index");
+    if (n_unconverged_host) *n_unconverged_host = 0;
+    if (!(n_ngb_target > 0.f) || !(n_ngb_tol >= 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_density: bad target/tolerance");
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_density: n_active < 0");
+    int64_t items = active ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!h || !rho || !omega || !ngb_count) return sph_fail(ctx, SPH_E_ARG, "sph_density: NULL output array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    if ((rc = sph_density_launch(ctx, active != nullptr, items, n_ngb_target, n_ngb_tol, h, rho, omega, ngb_count, status)))
+        return rc;
+    unsigned int unconv = 0;
+    SPH_CUDA(ctx, cudaMemcpyAsync(&unconv, &ctx->cnt->n_unconv, sizeof(unconv), cudaMemcpyDeviceToHost, ctx->stream));
+    SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    SPH_CUDA(ctx, cudaGetLastError());
+    if (n_unconverged_host) *n_unconverged_host = unconv;
+    return unconv ? SPH_W_NOCONV : SPH_OK;
+}
+
+int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
+                    const float *h, const float *rho, const float *omega, float *acc, float *dudt, float *vsig_max)
+{
+    if (!ctx) return SPH_E_ARG;
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_hydro_force before sph_build_index");
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force: n_active < 0");
+    int64_t items = active ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!vel || !u || !h || !rho || !omega || !acc || !dudt || !vsig_max)
+        return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force: NULL array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    return sph_force_launch(ctx, active != nullptr, items, vel, u, h, rho, omega, acc, dudt, vsig_max);
+}
+
+int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *vel_host, const float *u_host,
+                  float mass_scalar, const int32_t *active_host, int64_t n_active, float n_ngb_target, float n_ngb_tol,
+                  float *h_host, float *rho_host, float *omega_host, int32_t *ngb_count_host, float *acc_host,
+                  float *dudt_host, float *vsig_host, int64_t *n_unconverged_host)
+{
+    if (!ctx) return SPH_E_ARG;
+    if (n < 0 || (n > 0 && (!pos_host || !vel_host || !u_host || !h_host || !rho_host || !omega_host ||
+                            !ngb_count_host || !acc_host || !dudt_host || !vsig_host)))
+        return sph_fail(ctx, SPH_E_ARG, "sph_step_host: NULL host array");
+    if (n == 0) return SPH_OK;
+    cudaStream_t st = ctx->stream;
+    if (n > ctx->cap_host) {
+        dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
+        dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
+        size_t c = (size_t)n;
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_pos, 3 * c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_vel, 3 * c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_acc, 3 * c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_u, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_h, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_rho, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_omega, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_dudt, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_vsig, c * sizeof(float)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_ngb, c * sizeof(int32_t)));
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_active, c * sizeof(int32_t)));
+        ctx->cap_host = n;
+    }
+    size_t c = (size_t)n;
+    SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_pos, pos_host, 3 * c * sizeof(float), cudaMemcpyHostToDevice, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_vel, vel_host, 3 * c * sizeof(float), cudaMemcpyHostToDevice, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_u, u_host, c * sizeof(float), cudaMemcpyHostToDevice, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_h, h_host, c * sizeof(float), cudaMemcpyHostToDevice, st));
+    const int32_t *act = nullptr;
+    if (active_host) {
+        if (n_active < 0 || n_active > n) return sph_fail(ctx, SPH_E_ARG, "sph_step_host: bad n_active");
+        SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_active, active_host, (size_t)n_active * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        act = ctx->d_active;
+        // inactive particles keep the state the caller hands in (needed as neighbours by the force pass)
+        SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_rho, rho_host, c * sizeof(float), cudaMemcpyHostToDevice, st));
+        SPH_CUDA(ctx, cudaMemcpyAsync(ctx->d_omega, omega_host, c * sizeof(float), cudaMemcpyHostToDevice, st));
+    }
+    int rc = sph_build_index(ctx, n, ctx->d_pos, nullptr, mass_scalar);
+    if (rc) return rc;
+    int rcd = sph_density(ctx, act, n_active, n_ngb_target, n_ngb_tol, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_ngb,
+                          nullptr, n_unconverged_host);
+    if (rcd != SPH_OK && rcd != SPH_W_NOCONV) return rcd;
+    rc = sph_hydro_force(ctx, act, n_active, ctx->d_vel, ctx->d_u, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_acc,
+                         ctx->d_dudt, ctx->d_vsig);
+    if (rc) return rc;
+    SPH_CUDA(ctx, cudaMemcpyAsync(h_host, ctx->d_h, c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(rho_host, ctx->d_rho, c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(omega_host, ctx->d_omega, c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(ngb_count_host, ctx->d_ngb, c * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(acc_host, ctx->d_acc, 3 * c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(dudt_host, ctx->d_dudt, c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaMemcpyAsync(vsig_host, ctx->d_vsig, c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaStreamSynchronize(st));
+    SPH_CUDA(ctx, cudaGetLastError());
+    return rcd;
+}
+
+int sph_get_stats(sph_ctx *ctx, sph_stats *out)
+{
+    if (!ctx || !out) return SPH_E_ARG;
+    memset(out, 0, sizeof(*out));
+    out->n = ctx->n;
+    out->n_nodes = ctx->n_nodes;
+    out->n_groups = ctx->n_groups;
+    out->launches = ctx->launches;
+    SphCounters h;
+    SPH_CUDA(ctx, cudaMemcpyAsync(&h, ctx->cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    out->dens_evals = (int64_t)h.dens_evals;
+    out->dens_candidates = (int64_t)h.dens_cands;
+    out->dens_pairs = (int64_t)h.dens_pairs;
+    out->force_candidates = (int64_t)h.force_cands;
+    out->force_pairs = (int64_t)h.force_pairs;
+    return SPH_OK;
+}
+
+} // extern "C"

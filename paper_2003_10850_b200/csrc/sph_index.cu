@@ -1,0 +1,302 @@
+// sph_index.cu -- steps a1-a5: Morton keys, radix sort, permute to sorted float4, octree over the
+// sorted order, group (leaf-chunk) lists for the all-active and the active-subset case.
+//
+// Replaces the paper's Hilbert keys + domain decomposition + serial tree build (§1,
+// :72 §2.1, :194-196 §4) and its N_min CPU fallback for small active sets (§2.2).
+#include <cub/cub.cuh>
+
+#include "sph_internal.cuh"
+
+namespace {
+
+// interleave 16 bits with two zero bits between consecutive bits
+__device__ __forceinline__ uint64_t part1by2_16(uint32_t v)
+{
+    uint64_t x = v & 0xffffu;
+    x = (x | (x << 16)) & 0x00000000ff0000ffull;
+    x = (x | (x << 8)) & 0x000000f00f00f00full;
+    x = (x | (x << 4)) & 0x00000c30c30c30c3ull;
+    x = (x | (x << 2)) & 0x0000249249249249ull;
+    return x;
+}
+
+__device__ __forceinline__ uint32_t cell16(float x, float scale)
+{
+    int c = __float2int_rd(x * scale);
+    c = max(0, min(c, (1 << SPH_LMAX) - 1));
+    return (uint32_t)c;
+}
+
+// a1: key generation
+__global__ void k_keys(int64_t n, const float *__restrict__ pos, float scale, uint64_t *__restrict__ keys,
+                       uint32_t *__restrict__ perm)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    uint64_t k = part1by2_16(cell16(x, scale)) | (part1by2_16(cell16(y, scale)) << 1) |
+                 (part1by2_16(cell16(z, scale)) << 2);
+    keys[i] = k;
+    perm[i] = (uint32_t)i;
+}
+
+// a3: gather into the sorted float4 copy, inverse permutation
+__global__ void k_permute(int64_t n, const float *__restrict__ pos, const float *__restrict__ mass, float mass_scalar,
+                          const uint32_t *__restrict__ perm, float4 *__restrict__ xyzm, uint32_t *__restrict__ inv)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t id = perm[i];
+    float4 p;
+    p.x = pos[3 * (int64_t)id];
+    p.y = pos[3 * (int64_t)id + 1];
+    p.z = pos[3 * (int64_t)id + 2];
+    p.w = mass ? mass[id] : mass_scalar;
+    xyzm[i] = p;
+    inv[id] = (uint32_t)i;
+}
+
+__global__ void k_tree_init(SphCounters *cnt, SphNode *nodes, uint32_t n, float box)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        SphNode r;
+        r.start = 0; r.count = n; r.child = 0; r.parent = 0;
+        r.cx = r.cy = r.cz = 0.5f * box; r.half = 0.5f * box;
+        nodes[0] = r;
+        cnt->n_nodes = 1;
+        cnt->overflow = 0;
+        cnt->n_groups = 0;
+        for (int l = 0; l < SPH_LMAX + 3; l++) { cnt->lvl_begin[l] = 1; cnt->lvl_done[l] = 0; }
+        cnt->lvl_begin[0] = 0;
+        cnt->lvl_begin[1] = 1;
+    }
+}
+
+// a4: split every node of `level` that holds more than leaf_cap particles into its 8 octants.
+// The octant of a particle at this level is a 3-bit digit of its key; the sorted order makes each
+// child a contiguous run found by binary search.
+__global__ void k_tree_split(SphCounters *cnt, SphNode *nodes, const uint64_t *__restrict__ keys, int level,
+                             uint32_t leaf_cap, uint32_t node_cap)
+{
+    uint32_t beg = cnt->lvl_begin[level], end = cnt->lvl_begin[level + 1];
+    int shift = 3 * (SPH_LMAX - 1 - level);
+    for (uint32_t nd = beg + blockIdx.x * blockDim.x + threadIdx.x; nd < end; nd += gridDim.x * blockDim.x) {
+        SphNode p = nodes[nd];
+        if (p.count <= leaf_cap) continue;
+        uint32_t c0 = atomicAdd(&cnt->n_nodes, 8u);
+        if (c0 + 8u > node_cap) { atomicExch(&cnt->overflow, 1u); continue; } // stays an oversize leaf
+        uint32_t b[9];
+        b[0] = p.start;
+        b[8] = p.start + p.count;
+        for (int k = 1; k < 8; k++) { // first slot in [b[k-1], b[8]) whose digit >= k
+            uint32_t lo = b[k - 1], hi = b[8];
+            while (lo < hi) {
+                uint32_t mid = lo + ((hi - lo) >> 1);
+                uint32_t dig = (uint32_t)(keys[mid] >> shift) & 7u;
+                if (dig < (uint32_t)k) lo = mid + 1; else hi = mid;
+            }
+            b[k] = lo;
+        }
+        float q = 0.5f * p.half;
+        for (int k = 0; k < 8; k++) {
+            SphNode c;
+            c.start = b[k]; c.count = b[k + 1] - b[k]; c.child = 0; c.parent = nd;
+            c.cx = p.cx + ((k & 1) ? q : -q);
+            c.cy = p.cy + ((k & 2) ? q : -q);
+            c.cz = p.cz + ((k & 4) ? q : -q);
+            c.half = q;
+            nodes[c0 + k] = c;
+        }
+        nodes[nd].child = c0;
+    }
+    // last block to finish publishes the end of the next level
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        unsigned int t = atomicAdd(&cnt->lvl_done[level], 1u);
+        if (t == gridDim.x - 1) {
+            __threadfence();
+            unsigned int nn = atomicAdd(&cnt->n_nodes, 0u);
+            if (nn > node_cap) { nn = node_cap - ((node_cap - 1) & 7u); cnt->n_nodes = nn; }
+            cnt->lvl_begin[level + 2] = nn;
+        }
+    }
+}
+
+// a5 (all-active case): a group is a run of <= leaf_cap consecutive sorted slots inside one leaf
+__global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict__ nodes, uint32_t leaf_cap,
+                              uint32_t *__restrict__ mark)
+{
+    uint32_t nn = cnt->n_nodes;
+    for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) {
+        SphNode p = nodes[nd];
+        if (p.child != 0 || p.count == 0) continue;
+        for (uint32_t s = 0; s < p.count; s += leaf_cap) mark[p.start + s] = 1u;
+    }
+}
+
+__global__ void k_act_slots(int64_t na, const int32_t *__restrict__ active, const uint32_t *__restrict__ inv,
+                            uint32_t *__restrict__ slot)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < na) slot[k] = inv[active[k]];
+}
+
+__global__ void k_act_flags(int64_t na, const uint32_t *__restrict__ slot, const uint32_t *__restrict__ gid,
+                            uint32_t *__restrict__ flag)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < na) flag[k] = (k == 0 || gid[slot[k]] != gid[slot[k - 1]]) ? 1u : 0u;
+}
+
+template <typename T>
+int ensure(sph_ctx *ctx, T **p, size_t count)
+{
+    if (*p) { cudaFree(*p); *p = nullptr; }
+    if (count == 0) count = 1;
+    SPH_CUDA(ctx, cudaMalloc((void **)p, count * sizeof(T)));
+    return SPH_OK;
+}
+
+int ensure_tmp(sph_ctx *ctx, size_t bytes)
+{
+    if (bytes <= ctx->cub_tmp_bytes) return SPH_OK;
+    if (ctx->cub_tmp) cudaFree(ctx->cub_tmp);
+    ctx->cub_tmp = nullptr;
+    ctx->cub_tmp_bytes = 0;
+    bytes = bytes + bytes / 4 + 4096;
+    SPH_CUDA(ctx, cudaMalloc(&ctx->cub_tmp, bytes));
+    ctx->cub_tmp_bytes = bytes;
+    return SPH_OK;
+}
+
+inline int nblocks(int64_t n, int t) { return (int)((n + t - 1) / t); }
+
+} // namespace
+
+int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
+{
+    const int64_t n = ctx->n;
+    cudaStream_t st = ctx->stream;
+    const uint32_t B = (uint32_t)ctx->leaf_cap;
+    int rc;
+    if (n > ctx->cap_n) {
+        int64_t cap = n + n / 8 + 1024;
+        if ((rc = ensure(ctx, &ctx->keys, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->keys_alt, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->perm, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->perm_alt, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->inv, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->xyzm, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->grp_mark, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->gid_of_slot, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->grp_start, cap + 1))) return rc;
+        if ((rc = ensure(ctx, &ctx->f_xyzh, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->f_vc, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->f_raf, cap))) return rc;
+        // node pool: internal nodes hold > B particles each; 8 children per internal node.
+        // Typical use is ~ 8 n / (3 B); the pool is sized generously and overflow degrades gracefully.
+        int64_t ncap = 64 + 8 * (2 * cap / (int64_t)(B > 4 ? B / 4 : 1) + 8);
+        if (ncap > 0x7fffff00ll) ncap = 0x7fffff00ll;
+        ncap = 1 + 8 * ((ncap - 1) / 8);
+        if ((rc = ensure(ctx, &ctx->nodes, ncap))) return rc;
+        if ((rc = ensure(ctx, &ctx->node_hmax, ncap))) return rc;
+        ctx->node_cap = ncap;
+        ctx->cap_n = cap;
+    }
+    ctx->n_nodes = 0;
+    ctx->n_groups = 0;
+    if (n == 0) { ctx->have_index = true; return SPH_OK; }
+
+    const int T = 256;
+    float scale = (float)(1 << SPH_LMAX) / ctx->prm.box;
+    k_keys<<<nblocks(n, T), T, 0, st>>>(n, pos, scale, ctx->keys, ctx->perm);
+    ctx->launches++;
+
+    // a2: stable LSD radix sort of (key, id) on the 48 key bits
+    size_t tb = 0;
+    SPH_CUDA(ctx, cub::DeviceRadixSort::SortPairs(nullptr, tb, ctx->keys, ctx->keys_alt, ctx->perm, ctx->perm_alt,
+                                                  (int)n, 0, SPH_KEY_BITS, st));
+    size_t tb2 = 0, tb3 = 0;
+    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(nullptr, tb2, cub::CountingInputIterator<uint32_t>(0), ctx->grp_mark,
+                                             ctx->grp_start, &ctx->cnt->n_groups, (int)n, st));
+    SPH_CUDA(ctx, cub::DeviceScan::InclusiveSum(nullptr, tb3, ctx->grp_mark, ctx->gid_of_slot, (int)n, st));
+    if (tb2 > tb) tb = tb2;
+    if (tb3 > tb) tb = tb3;
+    if ((rc = ensure_tmp(ctx, tb))) return rc;
+    size_t tbs = ctx->cub_tmp_bytes;
+    SPH_CUDA(ctx, cub::DeviceRadixSort::SortPairs(ctx->cub_tmp, tbs, ctx->keys, ctx->keys_alt, ctx->perm,
+                                                  ctx->perm_alt, (int)n, 0, SPH_KEY_BITS, st));
+    ctx->launches += 1 + 2 * ((SPH_KEY_BITS + 7) / 8); // histogram + (scan+scatter | onesweep) passes, nominal
+    const uint64_t *skeys = ctx->keys_alt;
+    const uint32_t *sperm = ctx->perm_alt;
+
+    k_permute<<<nblocks(n, T), T, 0, st>>>(n, pos, mass, ctx->mass_scalar, sperm, ctx->xyzm, ctx->inv);
+    ctx->launches++;
+
+    // a4: octree, one level per launch (a level's nodes are contiguous in the pool)
+    k_tree_init<<<1, 32, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)n, ctx->prm.box);
+    ctx->launches++;
+    int grid = ctx->device_sms * 4;
+    for (int level = 0; level < SPH_LMAX; level++) {
+        int g = level < 3 ? 1 : grid;
+        k_tree_split<<<g, 128, 0, st>>>(ctx->cnt, ctx->nodes, skeys, level, B, (uint32_t)ctx->node_cap);
+        ctx->launches++;
+    }
+    // a5: group starts in sorted order + group id of every slot
+    SPH_CUDA(ctx, cudaMemsetAsync(ctx->grp_mark, 0, sizeof(uint32_t) * n, st));
+    k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, B, ctx->grp_mark);
+    ctx->launches++;
+    tbs = ctx->cub_tmp_bytes;
+    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),
+                                             ctx->grp_mark, ctx->grp_start, &ctx->cnt->n_groups, (int)n, st));
+    tbs = ctx->cub_tmp_bytes;
+    SPH_CUDA(ctx, cub::DeviceScan::InclusiveSum(ctx->cub_tmp, tbs, ctx->grp_mark, ctx->gid_of_slot, (int)n, st));
+    ctx->launches += 4;
+
+    // perm must survive in ctx->perm (keys_alt/perm_alt hold the sorted data): swap the handles
+    { uint64_t *t = ctx->keys; ctx->keys = ctx->keys_alt; ctx->keys_alt = t; }
+    { uint32_t *t = ctx->perm; ctx->perm = ctx->perm_alt; ctx->perm_alt = t; }
+
+    unsigned int hc[4];
+    SPH_CUDA(ctx, cudaMemcpyAsync(hc, ctx->cnt, sizeof(hc), cudaMemcpyDeviceToHost, st));
+    SPH_CUDA(ctx, cudaStreamSynchronize(st));
+    SPH_CUDA(ctx, cudaGetLastError());
+    ctx->n_nodes = hc[0];
+    ctx->n_groups = hc[1];
+    ctx->have_index = true;
+    return SPH_OK;
+}
+
+// a5 (active subset): ids -> sorted slots -> sort -> groups = runs sharing an all-active group
+int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
+{
+    cudaStream_t st = ctx->stream;
+    int rc;
+    if (na > ctx->cap_act) {
+        int64_t cap = na + na / 8 + 1024;
+        if ((rc = ensure(ctx, &ctx->act_slot, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->act_slot_alt, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->act_flag, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->agrp_start, cap + 1))) return rc;
+        ctx->cap_act = cap;
+    }
+    const int T = 256;
+    k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, active, ctx->inv, ctx->act_slot_alt);
+    int bits = 1;
+    while (bits < 32 && ((int64_t)1 << bits) < ctx->n) bits++;
+    size_t tb = 0, tb2 = 0;
+    SPH_CUDA(ctx, cub::DeviceRadixSort::SortKeys(nullptr, tb, ctx->act_slot_alt, ctx->act_slot, (int)na, 0, bits, st));
+    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(nullptr, tb2, cub::CountingInputIterator<uint32_t>(0), ctx->act_flag,
+                                             ctx->agrp_start, &ctx->cnt->n_agroups, (int)na, st));
+    if (tb2 > tb) tb = tb2;
+    if ((rc = ensure_tmp(ctx, tb))) return rc;
+    size_t tbs = ctx->cub_tmp_bytes;
+    SPH_CUDA(ctx, cub::DeviceRadixSort::SortKeys(ctx->cub_tmp, tbs, ctx->act_slot_alt, ctx->act_slot, (int)na, 0, bits, st));
+    k_act_flags<<<nblocks(na, T), T, 0, st>>>(na, ctx->act_slot, ctx->gid_of_slot, ctx->act_flag);
+    tbs = ctx->cub_tmp_bytes;
+    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),
+                                             ctx->act_flag, ctx->agrp_start, &ctx->cnt->n_agroups, (int)na, st));
+    ctx->launches += 2 + 2 + 1 + 2 * ((bits + 7) / 8);
+    return SPH_OK;
+}

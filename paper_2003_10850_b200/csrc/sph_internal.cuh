@@ -1,0 +1,100 @@
+// sph_internal.cuh -- private declarations of libsph.so (CUDA path; shares nothing with oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "sph.h"
+
+#define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
+#define SPH_KEY_BITS (3 * SPH_LMAX)
+#define SPH_MAXB 32         // max actives per group (= max leaf capacity)
+#define SPH_WARPS 4         // warps per CTA of the gather kernels
+#define SPH_THREADS (32 * SPH_WARPS)
+#define SPH_SMAX 512        // candidate segments per walk batch
+#define SPH_STK 512         // walk stack entries (blocks of 8 sibling nodes)
+#define SPH_QCAP 64         // hit-queue entries per (warp, active)
+#define SPH_ABLK 4          // actives register-blocked per warp pass
+
+// octree node, 32 bytes, read as two 16-byte loads
+struct __align__(16) SphNode {
+    uint32_t start;   // first sorted slot
+    uint32_t count;   // particles in the cell
+    uint32_t child;   // index of the first of 8 consecutive children, 0 = leaf
+    uint32_t parent;  // parent node index (root: 0)
+    float cx, cy, cz; // cell centre
+    float half;       // half edge
+};
+
+// device-side counters, one block of unsigned ints / 64-bit
+struct SphCounters {
+    unsigned int n_nodes;
+    unsigned int n_groups;     // all-active groups
+    unsigned int n_agroups;    // groups of the current active subset
+    unsigned int overflow;     // node pool exhausted (graceful: oversize leaves)
+    unsigned int work;         // persistent-kernel group counter
+    unsigned int n_unconv;     // density: particles stopped without convergence
+    unsigned int lvl_begin[SPH_LMAX + 3];
+    unsigned int lvl_done[SPH_LMAX + 3];
+    unsigned long long dens_evals, dens_cands, dens_pairs, force_cands, force_pairs;
+};
+
+struct sph_ctx {
+    sph_params prm;
+    cudaStream_t stream;
+    char err[320];
+    int device_sms;
+    int64_t n;        // particles in the index
+    int64_t cap_n;    // allocated capacity (particles)
+    bool have_index;
+    bool has_mass;
+    float mass_scalar;
+    int leaf_cap;
+
+    // index (device)
+    uint64_t *keys, *keys_alt;
+    uint32_t *perm, *perm_alt, *inv;
+    float4 *xyzm;
+    SphNode *nodes;
+    int64_t node_cap;
+    uint32_t *grp_mark, *gid_of_slot, *grp_start;
+    SphCounters *cnt;
+    void *cub_tmp;
+    size_t cub_tmp_bytes;
+    int64_t n_nodes, n_groups;
+
+    // force pass (device)
+    float4 *f_xyzh, *f_vc, *f_raf;
+    float *node_hmax;
+
+    // active subset scratch (device)
+    int64_t cap_act;
+    uint32_t *act_slot, *act_slot_alt, *act_flag, *agrp_start;
+
+    // host-step device state
+    int64_t cap_host;
+    float *d_pos, *d_vel, *d_u, *d_h, *d_rho, *d_omega, *d_acc, *d_dudt, *d_vsig;
+    int32_t *d_ngb, *d_active;
+
+    int64_t launches;
+};
+
+// error helpers -------------------------------------------------------------------------------
+int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
+#define SPH_CUDA(ctx, call)                                                                          \
+    do {                                                                                             \
+        cudaError_t e_ = (call);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return sph_fail(ctx, e_ == cudaErrorMemoryAllocation ? SPH_E_OOM : SPH_E_CUDA,           \
+                            "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);    \
+    } while (0)
+
+// stages (each returns sph_status) --------------------------------------------------------------
+int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
+void sph_reset_counters(sph_ctx *ctx, int which); // 0: density, 1: force
+int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t n_active);
+int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_target, float n_tol, float *h,
+                       float *rho, float *omega, int32_t *ngb, int32_t *status);
+int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
+                     const float *rho, const float *omega, float *acc, float *dudt, float *vsig);

@@ -1,0 +1,325 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on the
+same seeded inputs.  Sizes: the oracle finishes each in seconds; they
+span many groups/tiles and ragged tails.  Full-size configs are sampled in test_gpu_fullsize.py."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import sph_oracle as O
+from paper_2003_10850_b200 import binding as B
+from paper_2003_10850_b200 import inputs as I
+from parity_util import GpuRun, check_density_e2e, check_density_stage, check_force
+
+pytestmark = pytest.mark.gpu
+
+
+def _oracle_density(ps, brute=False, count_mode=0, active=None):
+    return O.density(ps.pos, ps.h_guess, kernel=ps.kernel, n_target=ps.n_ngb, n_tol=ps.n_tol, mass_scalar=ps.mass,
+                     brute=brute, count_mode=count_mode, active=active)
+
+
+def _full_parity(ps, brute=False, label=""):
+    """Stage-isolated density, end-to-end density, stage-isolated force on one particle set."""
+    o = _oracle_density(ps, brute=brute)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    rep = {}
+    # (i) single evaluation at the oracle's final H (tol = +inf)
+    Hf = o["H"].astype(np.float32)
+    oe = O.density_eval(ps.pos, Hf, kernel=ps.kernel, mass_scalar=ps.mass, brute=brute)
+    ge = g.density(Hf, ps.n_ngb, float("inf"))
+    assert ge["unconv"] == 0 and np.all((ge["status"] & 0xff) == 1)
+    assert np.array_equal(ge["H"], Hf)
+    rep["stage"] = check_density_stage(ge, oe, label=label + " stage")
+    # (ii) end to end from the same guess
+    gd = g.density(ps.h_guess, ps.n_ngb, ps.n_tol)
+    rep["e2e"] = check_density_e2e(gd, o, ps.pos, ps.h_guess, ps.kernel, ps.mass, ps.n_ngb, ps.n_tol, label=label + " e2e")
+    conv = (gd["status"] & B.ST_CONVERGED) != 0
+    assert conv.sum() + gd["unconv"] == ps.n
+    # iteration counts agree except on edge-class particles
+    same_it = (gd["status"] & 0xff) == o["iters"]
+    assert np.all(same_it | (o["edge"] != 0))
+    # (iii) force with the oracle's (H, rho, Omega) rounded to fp32 as inputs to both sides
+    rho = o["rho"].astype(np.float32)
+    om = o["omega"].astype(np.float32)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, Hf, rho, om, kernel=ps.kernel, mass_scalar=ps.mass, brute=brute)
+    gf = g.force(ps.vel, ps.u, Hf, rho, om)
+    rep["force"] = check_force(gf, of, label=label + " force")
+    st = g.sph.stats()
+    assert st["force_pairs"] == int(of["npair"].sum()) or rep["force"]["n_edge"] > 0
+    rep["stats"] = st
+    g.close()
+    return rep
+
+
+def test_config1_bruteforce_oracle():
+    """BASELINE.json configs[0]: 4096 particles, O(N^2) brute-force oracle."""
+    ps = I.config1()
+    rep = _full_parity(ps, brute=True, label="C1")
+    print("C1", rep)
+    assert rep["stats"]["n_groups"] >= 128
+
+
+def test_config2_small():
+    """configs[1] shape at 32^3 (velocities, u spread): oracle cell list."""
+    ps = I.config2(32)
+    rep = _full_parity(ps, label="C2/32")
+    print("C2/32", rep)
+
+
+def test_config3_small_clustered():
+    """configs[2] shape at 2^16 particles, 20 Plummer spheres: wide range of H inside one run."""
+    ps = I.config3(1 << 16, 20)
+    rep = _full_parity(ps, label="C3/2^16")
+    print("C3 small", rep)
+
+
+def test_config4_small_wendland():
+    """configs[3] shape at 6*10^4 particles (Wendland C6, 295 neighbours, NFW cusps)."""
+    ps = I.config4(60000, 12, m_lo=320, m_hi=2e4)
+    rep = _full_parity(ps, label="C4/6e4")
+    print("C4 small", rep)
+
+
+def test_config5_small_active_subset():
+    """configs[4] shape: 2% of a small C4-like set active (time-bin selection), density + force on the subset."""
+    ps = I.config4(60000, 12, m_lo=320, m_hi=2e4)
+    o = _oracle_density(ps)
+    Hc, rho, om = o["H"].astype(np.float32), o["rho"].astype(np.float32), o["omega"].astype(np.float32)
+    act = I.select_active_by_timebin(ps, 1200)
+    hg = I.perturb_h(Hc, act, I.SEED_BASE + 5)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    h_in = hg.copy()
+    oa = O.density(ps.pos, hg, kernel=ps.kernel, n_target=ps.n_ngb, n_tol=ps.n_tol, mass_scalar=ps.mass, active=act)
+    gd = g.density(h_in, ps.n_ngb, ps.n_tol, active=act)
+    rep = check_density_e2e(gd, oa, ps.pos, hg, ps.kernel, ps.mass, ps.n_ngb, ps.n_tol, sel=act, label="C5 e2e")
+    # only active entries were written
+    inact = np.ones(ps.n, bool)
+    inact[act] = False
+    assert np.array_equal(gd["H"][inact], hg[inact]) and np.all(gd["rho"][inact] == -1) and np.all(gd["Nint"][inact] == -1)
+    # force on the subset, inactive neighbours contribute with their current state (R12)
+    Hs = Hc.copy(); Hs[act] = oa["H"].astype(np.float32)
+    rs = rho.copy(); rs[act] = oa["rho"].astype(np.float32)
+    oms = om.copy(); oms[act] = oa["omega"].astype(np.float32)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, Hs, rs, oms, kernel=ps.kernel, mass_scalar=ps.mass, active=act)
+    gf = g.force(ps.vel, ps.u, Hs, rs, oms, active=act)
+    repf = check_force(gf, of, sel=act, label="C5 force")
+    assert np.all(gf["acc"][inact] == 7.0) and np.all(gf["dudt"][inact] == 7.0)
+    print("C5 small", rep, repf, g.sph.stats())
+    g.close()
+
+
+def test_integer_count_mode():
+    ps = I.config1(12)
+    o = _oracle_density(ps, brute=True, count_mode=1)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass, count_mode=1)
+    gd = g.density(ps.h_guess, ps.n_ngb, ps.n_tol)
+    rep = check_density_e2e(gd, o, ps.pos, ps.h_guess, ps.kernel, ps.mass, ps.n_ngb, ps.n_tol, count_mode=1, label="int mode")
+    conv = (gd["status"] & B.ST_CONVERGED) != 0
+    assert np.all(np.abs(gd["Nint"][conv] - 64) <= 2)
+    assert gd["unconv"] == int((~conv).sum())
+    print("int mode", rep, "unconverged", gd["unconv"], "oracle", int((o["flags"] != O.F_CONVERGED).sum()))
+    g.close()
+
+
+def test_mass_array_path():
+    ps = I.config2(16)
+    rng = np.random.default_rng(11)
+    m = (ps.mass * rng.uniform(0.5, 1.5, ps.n)).astype(np.float32)
+    o = O.density(ps.pos, ps.h_guess, kernel=0, n_target=64, n_tol=2, mass=m)
+    g = GpuRun(ps.pos, 0, 1.0, mass=m)
+    gd = g.density(ps.h_guess, 64, 2)
+    check_density_e2e(gd, o, ps.pos, ps.h_guess, 0, 1.0, 64, 2, label="mass array", mass=m)
+    Hf, rho, om = o["H"].astype(np.float32), o["rho"].astype(np.float32), o["omega"].astype(np.float32)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, Hf, rho, om, kernel=0, mass=m)
+    gf = g.force(ps.vel, ps.u, Hf, rho, om)
+    check_force(gf, of, label="mass array force")
+    g.close()
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_perfect_lattice_pins_on_gpu(kernel):
+    """The lattice pins of the oracle hold on the CUDA path too: N_int = 81 / 305, rho ~ m n, a = 0."""
+    pos = I.perfect_lattice(16)
+    n = pos.shape[0]
+    nt, nint, hc = (64.0, 81, 2.48232) if kernel == 0 else (295.0, 305, 4.12941)
+    g = GpuRun(pos, kernel, 1.0 / n)
+    gd = g.density(np.full(n, 1.05 * hc / 16, np.float32), nt, 0.01)
+    assert gd["unconv"] == 0
+    assert np.all(gd["Nint"] == nint)
+    assert np.abs(gd["rho"] - 1.0).max() < 2e-3 and np.ptp(gd["rho"]) < 1e-5
+    assert np.abs(gd["H"] * 16 / hc - 1).max() < 1e-4
+    gf = g.force(np.zeros((n, 3), np.float32), np.ones(n, np.float32), gd["H"], gd["rho"], gd["omega"])
+    of = O.hydro_force(pos, np.zeros((n, 3), np.float32), np.ones(n, np.float32), gd["H"], gd["rho"], gd["omega"],
+                       kernel=kernel, mass_scalar=1.0 / n, active=np.arange(8, dtype=np.int32))
+    assert np.abs(gf["acc"]).max() < 1e-5 * of["asum"].max()
+    assert np.all(gf["dudt"] == 0)
+    assert np.allclose(gf["vsig"], 2 * math.sqrt(10.0 / 9.0), rtol=1e-6)
+    g.close()
+
+
+def test_momentum_conservation_on_gpu():
+    ps = I.config2(24)
+    g = GpuRun(ps.pos, 0, ps.mass)
+    gd = g.density(ps.h_guess, 64, 2)
+    gf = g.force(ps.vel, ps.u, gd["H"], gd["rho"], gd["omega"])
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, gd["H"], gd["rho"], gd["omega"], kernel=0, mass_scalar=ps.mass,
+                       active=np.arange(64, dtype=np.int32))
+    scale = of["asum"].mean() * ps.n
+    tot = gf["acc"].astype(np.float64).sum(0)
+    assert np.abs(tot).max() < 1e-6 * scale  # sum m a = 0 to fp32 rounding
+    e = ((ps.vel.astype(np.float64) * gf["acc"]).sum(1) + gf["dudt"]).sum()
+    assert abs(e) < 1e-5 * np.abs(gf["dudt"]).sum()
+    g.close()
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_empty_and_tiny():
+    sph = B.Sph(kernel=0)
+    z = torch.zeros(0, device="cuda")
+    sph.sph_build_index(torch.zeros((0, 3), device="cuda"), None, 1.0)
+    assert sph.sph_density(z, z, z, torch.zeros(0, device="cuda", dtype=torch.int32), 64, 2) == 0
+    sph.close()
+    # one particle: only the self term; cannot reach 64 -> H grows to the cap, flagged
+    pos = np.array([[0.3, 0.3, 0.3]], np.float32)
+    g = GpuRun(pos, 0, 1.0)
+    gd = g.density(np.array([0.1], np.float32), 64, 2)
+    o = O.density(pos, np.array([0.1], np.float32), kernel=0, n_target=64, n_tol=2, mass_scalar=1.0, brute=True)
+    assert gd["unconv"] == 1 and (gd["status"][0] & B.ST_STALLED)
+    assert abs(gd["H"][0] - 0.49999) < 1e-6 and gd["Nint"][0] == 1 and o["Nint"][0] == 1
+    assert abs(gd["rho"][0] - o["rho"][0]) < 1e-5 * o["rho"][0]
+    gf = g.force(np.zeros((1, 3), np.float32), np.ones(1, np.float32), gd["H"], gd["rho"], gd["omega"])
+    assert np.all(gf["acc"] == 0) and gf["vsig"][0] == 0 and gf["dudt"][0] == 0
+    g.close()
+
+
+def test_edge_active_empty_list():
+    ps = I.config1(8)
+    g = GpuRun(ps.pos, 0, ps.mass)
+    gd = g.density(ps.h_guess, 64, 2, active=np.zeros(0, np.int32))
+    assert gd["unconv"] == 0 and np.all(gd["rho"] == -1)
+    g.close()
+
+
+def test_edge_two_particles_through_the_wall_and_coincident():
+    # neighbours across the periodic boundary on all three axes + a coincident pair
+    pos = np.array([[0.01, 0.995, 0.5], [0.97, 0.005, 0.5], [0.97, 0.005, 0.5], [0.5, 0.5, 0.5]], np.float32)
+    h = np.array([0.1, 0.1, 0.12, 0.2], np.float32)
+    u = np.array([1.0, 2.0, 0.5, 1.0], np.float32)
+    vel = np.array([[0.1, 0, 0], [-0.2, 0.1, 0], [0.3, 0, 0.1], [0, 0, 0]], np.float32)
+    oe = O.density_eval(pos, h, kernel=0, mass_scalar=0.25, brute=True)
+    g = GpuRun(pos, 0, 0.25)
+    ge = g.density(h, 3.0, float("inf"))
+    check_density_stage(ge, oe, label="wall")
+    assert list(ge["Nint"]) == [3, 3, 3, 1]
+    rho, om = oe["rho"].astype(np.float32), oe["omega"].astype(np.float32)
+    of = O.hydro_force(pos, vel, u, h, rho, om, kernel=0, mass_scalar=0.25, brute=True)
+    gf = g.force(vel, u, h, rho, om)
+    check_force(gf, of, label="wall force")
+    assert of["npair"].tolist() == [2, 2, 2, 0]
+    g.close()
+
+
+def test_edge_large_support_pairwrap_mode():
+    """H comparable to the box: the per-pair nearest-image fallback (every cell visited once)."""
+    rng = np.random.default_rng(21)
+    n = 700
+    pos = rng.uniform(0, 1, (n, 3)).astype(np.float32)
+    h = rng.uniform(0.3, 0.49, n).astype(np.float32)
+    oe = O.density_eval(pos, h, kernel=1, mass_scalar=1.0 / n, brute=True)
+    g = GpuRun(pos, 1, 1.0 / n)
+    ge = g.density(h, 100.0, float("inf"))
+    rep = check_density_stage(ge, oe, label="pairwrap")
+    vel = rng.normal(0, 1, (n, 3)).astype(np.float32)
+    u = rng.uniform(0.5, 2, n).astype(np.float32)
+    rho, om = oe["rho"].astype(np.float32), oe["omega"].astype(np.float32)
+    of = O.hydro_force(pos, vel, u, h, rho, om, kernel=1, mass_scalar=1.0 / n, brute=True)
+    gf = g.force(vel, u, h, rho, om)
+    repf = check_force(gf, of, label="pairwrap force")
+    print("pairwrap", rep, repf)
+    g.close()
+
+
+def test_edge_mixed_supports_symmetric_set():
+    """A few huge-H particles among small-H ones: the force set r < max(H_i, H_j) must find them."""
+    ps = I.config2(16)
+    o = _oracle_density(ps)
+    Hf = o["H"].astype(np.float32)
+    rng = np.random.default_rng(5)
+    big = rng.choice(ps.n, 12, replace=False)
+    Hf[big] *= 2.7
+    oe = O.density_eval(ps.pos, Hf, kernel=0, mass_scalar=ps.mass)
+    rho, om = oe["rho"].astype(np.float32), oe["omega"].astype(np.float32)
+    g = GpuRun(ps.pos, 0, ps.mass)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, Hf, rho, om, kernel=0, mass_scalar=ps.mass)
+    gf = g.force(ps.vel, ps.u, Hf, rho, om)
+    check_force(gf, of, label="mixed H")
+    assert g.sph.stats()["force_pairs"] == int(of["npair"].sum()) or (of["edge"] != 0).any()
+    g.close()
+
+
+def test_edge_oversize_leaf_many_coincident():
+    """More coincident particles than a leaf can hold: the leaf is chunked into several groups."""
+    rng = np.random.default_rng(2)
+    base = rng.uniform(0, 1, (300, 3)).astype(np.float32)
+    clump = np.tile(np.array([[0.123, 0.456, 0.789]], np.float32), (100, 1))
+    pos = np.concatenate([base, clump])
+    n = pos.shape[0]
+    h = np.full(n, 0.2, np.float32)
+    oe = O.density_eval(pos, h, kernel=0, mass_scalar=1.0 / n, brute=True)
+    g = GpuRun(pos, 0, 1.0 / n)
+    ge = g.density(h, 50.0, float("inf"))
+    check_density_stage(ge, oe, label="clump")
+    u = np.ones(n, np.float32)
+    vel = rng.normal(0, 1, (n, 3)).astype(np.float32)
+    rho, om = oe["rho"].astype(np.float32), oe["omega"].astype(np.float32)
+    of = O.hydro_force(pos, vel, u, h, rho, om, kernel=0, mass_scalar=1.0 / n, brute=True)
+    gf = g.force(vel, u, h, rho, om)
+    check_force(gf, of, label="clump force")
+    g.close()
+
+
+def test_box_not_one_and_small_leaf_cap():
+    ps = I.config2(16)
+    s = 2.0
+    pos = (ps.pos * s).astype(np.float32)
+    hg = (ps.h_guess * s).astype(np.float32)
+    o = O.density(pos, hg, kernel=0, n_target=64, n_tol=2, mass_scalar=ps.mass, box=s)
+    g = GpuRun(pos, 0, ps.mass, box=s, leaf_cap=8)
+    gd = g.density(hg, 64, 2)
+    check_density_e2e(gd, o, pos, hg, 0, ps.mass, 64, 2, label="box=2", box=s)
+    g.close()
+
+
+def test_step_host_matches_device_calls():
+    ps = I.config2(16)
+    n = ps.n
+    g = GpuRun(ps.pos, 0, ps.mass)
+    gd = g.density(ps.h_guess, 64, 2)
+    gf = g.force(ps.vel, ps.u, gd["H"], gd["rho"], gd["omega"])
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h = pin(ps.h_guess.copy())
+    rho, om, du, vs = (torch.zeros(n).pin_memory() for _ in range(4))
+    ngb = torch.zeros(n, dtype=torch.int32).pin_memory()
+    acc = torch.zeros((n, 3)).pin_memory()
+    sph = B.Sph(kernel=0)
+    unconv = sph.sph_step_host(pin(ps.pos), pin(ps.vel), pin(ps.u), ps.mass, h, rho, om, ngb, acc, du, vs, 64, 2)
+    assert unconv == 0
+    assert np.array_equal(h.numpy(), gd["H"]) and np.array_equal(ngb.numpy(), gd["Nint"])
+    assert np.allclose(rho.numpy(), gd["rho"], rtol=1e-6)
+    assert np.allclose(acc.numpy(), gf["acc"], rtol=1e-4, atol=1e-6 * np.abs(gf["acc"]).max())
+    sph.close()
+    g.close()
+
+
+def test_errors_are_return_codes():
+    sph = B.Sph(kernel=0)
+    z = torch.zeros(4, device="cuda")
+    with pytest.raises(B.SphError) as e:
+        sph.n = 4
+        sph.sph_density(z, z.clone(), z.clone(), torch.zeros(4, device="cuda", dtype=torch.int32), 64, 2)
+    assert e.value.code == B.SPH_E_NOINDEX
+    sph.close()
+    with pytest.raises(B.SphError):
+        B.Sph(kernel=7)
