@@ -107,8 +107,9 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
  *   omega[id]     1 + (H_i / 3 rho_i) d rho_i / d H_i,
  *   ngb_count[id] integer count #{j : r_ij < H_i} at the returned H (self included),
  *   status[id]    evaluations used | SPH_ST_* flags (status may be NULL).
- *   active        [n_active] device int32 particle ids (unique, in range) or NULL = all particles
- *                 (then n_active is ignored);
+ *   active        [n_active] device int32 particle ids (unique, in range); NULL with n_active != 0
+ *                 (conventionally -1) means all particles; n_active == 0 is the empty list (nothing
+ *                 is computed or written, whatever the pointer);
  *   n_ngb_tol     +inf means "evaluate once at the given h";
  *   n_unconverged_host  HOST pointer (may be NULL): number of active particles that stopped
  *                 without SPH_ST_CONVERGED.

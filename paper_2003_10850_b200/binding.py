@@ -128,7 +128,7 @@ class Sph:
     def sph_density(self, h, rho, omega, ngb_count, n_ngb_target, n_ngb_tol, active=None, status=None):
         """Returns the number of active particles that stopped without convergence."""
         n = self.n
-        na = 0 if active is None else active.numel()
+        na = -1 if active is None else active.numel()
         unconv = C.c_int64(0)
         self._check(self._lib.sph_density(self._h, _dev(active, torch.int32, "active"), na, float(n_ngb_target),
                                           float(n_ngb_tol), _dev(h, torch.float32, "h", n),
@@ -140,7 +140,7 @@ class Sph:
 
     def sph_hydro_force(self, vel, u, h, rho, omega, acc, dudt, vsig_max, active=None):
         n = self.n
-        na = 0 if active is None else active.numel()
+        na = -1 if active is None else active.numel()
         self._check(self._lib.sph_hydro_force(self._h, _dev(active, torch.int32, "active"), na,
                                               _dev(vel, torch.float32, "vel", 3 * n), _dev(u, torch.float32, "u", n),
                                               _dev(h, torch.float32, "h", n), _dev(rho, torch.float32, "rho", n),
@@ -153,7 +153,7 @@ class Sph:
                       n_ngb_tol, active=None):
         """Whole pass with HOST (ideally pinned) tensors; returns the unconverged count."""
         n = pos.shape[0]
-        na = 0 if active is None else active.numel()
+        na = -1 if active is None else active.numel()
         unconv = C.c_int64(0)
         f32, i32 = torch.float32, torch.int32
         self._check(self._lib.sph_step_host(self._h, n, _host(pos, f32, "pos", 3 * n), _host(vel, f32, "vel", 3 * n),

@@ -26,11 +26,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+           "-Wno-deprecated-declarations", "-Xcompiler", "-Wno-deprecated-declarations",
            "--shared", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
+    if os.environ.get("SPH_DEBUG"):  # device-side bounds asserts (development only)
+        cmd.insert(1, "-DSPH_DEBUG=1")
     subprocess.check_call(cmd)
     return LIB
 

@@ -112,8 +112,9 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
     if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_density before sph_build_index");
     if (n_unconverged_host) *n_unconverged_host = 0;
     if (!(n_ngb_target > 0.f) || !(n_ngb_tol >= 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_density: bad target/tolerance");
+    const bool subset = active != nullptr || n_active == 0; // (NULL, 0) is the empty list, (NULL, != 0) is "all"
     if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_density: n_active < 0");
-    int64_t items = active ? n_active : ctx->n;
+    int64_t items = subset ? n_active : ctx->n;
     if (ctx->n == 0 || items == 0) return SPH_OK;
     if (!h || !rho || !omega || !ngb_count) return sph_fail(ctx, SPH_E_ARG, "sph_density: NULL output array");
     int rc = check_sticky(ctx);
@@ -134,8 +135,9 @@ int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const
 {
     if (!ctx) return SPH_E_ARG;
     if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_hydro_force before sph_build_index");
+    const bool subset = active != nullptr || n_active == 0;
     if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force: n_active < 0");
-    int64_t items = active ? n_active : ctx->n;
+    int64_t items = subset ? n_active : ctx->n;
     if (ctx->n == 0 || items == 0) return SPH_OK;
     if (!vel || !u || !h || !rho || !omega || !acc || !dudt || !vsig_max)
         return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force: NULL array");
@@ -189,6 +191,7 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
     }
     int rc = sph_build_index(ctx, n, ctx->d_pos, nullptr, mass_scalar);
     if (rc) return rc;
+    if (!active_host && n_active != 0) n_active = -1; // all active
     int rcd = sph_density(ctx, act, n_active, n_ngb_target, n_ngb_tol, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_ngb,
                           nullptr, n_unconverged_host);
     if (rcd != SPH_OK && rcd != SPH_W_NOCONV) return rcd;

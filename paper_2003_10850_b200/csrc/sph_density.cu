@@ -13,12 +13,13 @@ namespace {
 
 struct DensArgs {
     const SphNode *nodes;
+    uint32_t n_nodes;
     const float4 *xyzm;
     const uint32_t *perm;
     const uint32_t *gstart;     // group starts (indices into the item list)
     const unsigned int *n_groups;
     const uint32_t *item_slot;  // NULL: item index == sorted slot (all active)
-    uint32_t n_items;
+    uint32_t n_items, n_total;
     SphCounters *cnt;
     float L;
     float n_target, n_tol;
@@ -87,7 +88,6 @@ __device__ __forceinline__ void dens_unit(DensShared &sh, const float4 *__restri
     unsigned tail[A], head[A];
     int k[A];
     const float tx = sh.ws.thr[0], ty = sh.ws.thr[1], tz = sh.ws.thr[2];
-    const float invL = 1.f / L;
 #pragma unroll
     for (int a = 0; a < A; a++) {
         k[a] = sh.ulist[ub + a];
@@ -124,14 +124,14 @@ __device__ __forceinline__ void dens_unit(DensShared &sh, const float4 *__restri
 
     for (int j0 = c0; j0 < c1; j0 += 32) {
         int j = j0 + lane;
-        float4 c = (j < c1) ? tile[j] : make_float4(3e18f, 3e18f, 3e18f, 0.f);
+        float4 c = (j < c1) ? tile[j] : make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
 #pragma unroll
         for (int a = 0; a < A; a++) {
-            float dx = xi[a] - c.x, dy = yi[a] - c.y, dz = zi[a] - c.z;
+            float dx, dy, dz;
             if (PAIRWRAP) {
-                dx -= L * rintf(dx * invL);
-                dy -= L * rintf(dy * invL);
-                dz -= L * rintf(dz * invL);
+                dx = image_diff(xi[a], c.x, L); dy = image_diff(yi[a], c.y, L); dz = image_diff(zi[a], c.z, L);
+            } else {
+                dx = xi[a] - c.x; dy = yi[a] - c.y; dz = zi[a] - c.z;
             }
             float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             bool hit = r2 < h2[a];
@@ -212,8 +212,10 @@ __global__ void __launch_bounds__(SPH_THREADS) k_density(DensArgs a)
         const uint32_t i0 = a.gstart[g];
         const uint32_t i1 = (g + 1 < n_groups) ? a.gstart[g + 1] : a.n_items;
         const int na = (int)(i1 - i0);
+        SPH_ASSERT(i1 > i0 && i1 <= a.n_items && na <= SPH_MAXB);
         if (tid < na) {
             uint32_t slot = a.item_slot ? a.item_slot[i0 + tid] : i0 + tid;
+            SPH_ASSERT(slot < a.n_total);
             float4 p = a.xyzm[slot];
             uint32_t id = a.perm[slot];
             sh.aslot[tid] = id;
@@ -256,7 +258,7 @@ __global__ void __launch_bounds__(SPH_THREADS) k_density(DensArgs a)
             bool more_walk;
             do {
                 __syncthreads(); // everyone is done with the previous batch's lists
-                if (warp == 0) walk_batch<false>(sh.ws, a.nodes, nullptr, L, DENS_TILE);
+                if (warp == 0) walk_batch<false>(sh.ws, a.nodes, nullptr, L, DENS_TILE, a.n_nodes);
                 __syncthreads();
                 const uint32_t total = sh.ws.total;
                 more_walk = sh.ws.sp > 0;
@@ -389,12 +391,14 @@ int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_targe
 {
     DensArgs a;
     a.nodes = ctx->nodes;
+    a.n_nodes = (uint32_t)ctx->n_nodes;
     a.xyzm = ctx->xyzm;
     a.perm = ctx->perm;
     a.gstart = subset ? ctx->agrp_start : ctx->grp_start;
     a.n_groups = subset ? &ctx->cnt->n_agroups : &ctx->cnt->n_groups;
     a.item_slot = subset ? ctx->act_slot : nullptr;
     a.n_items = (uint32_t)n_items;
+    a.n_total = (uint32_t)ctx->n;
     a.cnt = ctx->cnt;
     a.L = ctx->prm.box;
     a.n_target = n_target;

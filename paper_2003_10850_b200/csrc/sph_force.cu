@@ -13,6 +13,7 @@ namespace {
 
 struct ForceArgs {
     const SphNode *nodes;
+    uint32_t n_nodes;
     const float *node_hmax;
     const float4 *xyzh, *vc, *raf; // sorted: (x,y,z,H) (vx,vy,vz,c) (rho, A, m, slot)
     const uint32_t *perm;
@@ -67,7 +68,6 @@ __device__ __forceinline__ void force_unit(ForceShared &sh, const float4 *__rest
     int cn[A];
     unsigned tail[A], head[A];
     const float tx = sh.ws.thr[0], ty = sh.ws.thr[1], tz = sh.ws.thr[2];
-    const float invL = 1.f / L;
 #pragma unroll
     for (int a = 0; a < A; a++) {
         int k = ub + a;
@@ -90,11 +90,11 @@ __device__ __forceinline__ void force_unit(ForceShared &sh, const float4 *__rest
             int j = qw[a * SPH_QCAP + p];
             float4 P0 = t0[j], P1 = t1[j], P2 = t2[j];
             if (__float_as_uint(P2.w) != sh.aslot[k]) { // j != i
-                float dx = xi[a] - P0.x, dy = yi[a] - P0.y, dz = zi[a] - P0.z;
+                float dx, dy, dz;
                 if (PAIRWRAP) {
-                    dx -= L * rintf(dx * invL);
-                    dy -= L * rintf(dy * invL);
-                    dz -= L * rintf(dz * invL);
+                    dx = image_diff(xi[a], P0.x, L); dy = image_diff(yi[a], P0.y, L); dz = image_diff(zi[a], P0.z, L);
+                } else {
+                    dx = xi[a] - P0.x; dy = yi[a] - P0.y; dz = zi[a] - P0.z;
                 }
                 float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                 float rinv = rsqrtf(fmaxf(r2, 1e-37f));
@@ -125,15 +125,15 @@ __device__ __forceinline__ void force_unit(ForceShared &sh, const float4 *__rest
 
     for (int j0 = c0; j0 < c1; j0 += 32) {
         int j = j0 + lane;
-        float4 c = (j < c1) ? t0[j] : make_float4(3e18f, 3e18f, 3e18f, 0.f);
+        float4 c = (j < c1) ? t0[j] : make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
         float hj2 = c.w * c.w;
 #pragma unroll
         for (int a = 0; a < A; a++) {
-            float dx = xi[a] - c.x, dy = yi[a] - c.y, dz = zi[a] - c.z;
+            float dx, dy, dz;
             if (PAIRWRAP) {
-                dx -= L * rintf(dx * invL);
-                dy -= L * rintf(dy * invL);
-                dz -= L * rintf(dz * invL);
+                dx = image_diff(xi[a], c.x, L); dy = image_diff(yi[a], c.y, L); dz = image_diff(zi[a], c.z, L);
+            } else {
+                dx = xi[a] - c.x; dy = yi[a] - c.y; dz = zi[a] - c.z;
             }
             float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             bool hit = r2 < fmaxf(h2[a], hj2);
@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(SPH_THREADS) k_force(ForceArgs a)
         bool more_walk;
         do {
             __syncthreads();
-            if (warp == 0) walk_batch<true>(sh.ws, a.nodes, a.node_hmax, L, FORCE_TILE);
+            if (warp == 0) walk_batch<true>(sh.ws, a.nodes, a.node_hmax, L, FORCE_TILE, a.n_nodes);
             __syncthreads();
             const uint32_t total = sh.ws.total;
             more_walk = sh.ws.sp > 0;
@@ -362,6 +362,7 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
 
     ForceArgs a;
     a.nodes = ctx->nodes;
+    a.n_nodes = (uint32_t)ctx->n_nodes;
     a.node_hmax = ctx->node_hmax;
     a.xyzh = ctx->f_xyzh; a.vc = ctx->f_vc; a.raf = ctx->f_raf;
     a.perm = ctx->perm;

@@ -10,6 +10,22 @@
 #include "sph_internal.cuh"
 
 #define FULLMASK 0xffffffffu
+// padding coordinate of lanes past the end of a candidate range: every comparison with NaN is
+// false, in the plain and in the per-pair nearest-image frame alike
+#define SPH_NANF __int_as_float(0x7fc00000)
+
+// Minimum-image difference of two coordinates in [0, L) with the relative accuracy of a plain fp32
+// difference: x - L is exact for x >= L/2 (Sterbenz), so the wrapped branch subtracts two nearby
+// numbers instead of rounding the large difference first (which would leave an error of ulp(L) on a
+// result that may be 1e-3 L).
+__device__ __forceinline__ float image_diff(float xi, float cx, float L)
+{
+    float d = xi - cx;
+    const float hl = 0.5f * L;
+    if (d >= hl) d = (xi - L) - cx;
+    else if (d < -hl) d = xi - (cx - L);
+    return d;
+}
 
 __device__ __forceinline__ unsigned lanemask_lt()
 {
@@ -69,7 +85,7 @@ __device__ __forceinline__ SphNode load_node(const SphNode *__restrict__ nodes, 
 // lane) so that the stack holds at most 32 entries per tree level.
 template <bool FORCE>
 __device__ void walk_batch(WalkShared &ws, const SphNode *__restrict__ nodes, const float *__restrict__ node_hmax,
-                           float L, uint32_t tile_cap)
+                           float L, uint32_t tile_cap, uint32_t n_nodes)
 {
     const int lane = threadIdx.x & 31;
     int sp = ws.sp, n_seg = 0;
@@ -89,6 +105,7 @@ __device__ void walk_batch(WalkShared &ws, const SphNode *__restrict__ nodes, co
             if (lane == 0) ws.stack[0] = root.child;
             sp = 1;
         }
+        __syncwarp();
     }
     // stop a batch once it holds a few tiles worth of candidates (bounds smem lists, keeps tiles full)
     while (sp > 0 && n_seg <= SPH_SMAX - 32 && total_est < 4u * tile_cap) {
@@ -97,6 +114,7 @@ __device__ void walk_batch(WalkShared &ws, const SphNode *__restrict__ nodes, co
         int e = lane >> 3;
         bool valid = e < npop;
         uint32_t idx = valid ? ws.stack[sp + e] + (lane & 7) : 0u;
+        SPH_ASSERT(sp + 4 <= SPH_STK && idx < n_nodes);
         SphNode nd = load_node(nodes, idx);
         float reach = ws.hg;
         if (FORCE) reach = fmaxf(reach, __ldg(node_hmax + idx));
@@ -112,6 +130,7 @@ __device__ void walk_batch(WalkShared &ws, const SphNode *__restrict__ nodes, co
         unsigned me = __ballot_sync(FULLMASK, emit);
         if (emit) {
             int p = n_seg + __popc(me & lanemask_lt());
+            SPH_ASSERT(p < SPH_SMAX);
             ws.seg_start[p] = nd.start;
             ws.seg_pre[p] = nd.count;
             maxhalf = fmaxf(maxhalf, nd.half);
@@ -123,6 +142,7 @@ __device__ void walk_batch(WalkShared &ws, const SphNode *__restrict__ nodes, co
         for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(FULLMASK, c, o);
         total_est += c;
         unsigned mp = __ballot_sync(FULLMASK, push);
+        SPH_ASSERT(sp + __popc(mp) <= SPH_STK);
         if (push) ws.stack[sp + __popc(mp & lanemask_lt())] = nd.child;
         sp += __popc(mp);
         __syncwarp();
@@ -180,13 +200,15 @@ __device__ __forceinline__ void stage_tile(const WalkShared &ws, float4 *const *
         uint32_t lo = max(p0, t_lo), hi = min(p1, t_hi);
         uint32_t gsrc = ws.seg_start[s] - p0;
         for (uint32_t e = lo + lane; e < hi; e += 32) {
-            float4 v = __ldg(src[0] + gsrc + e);
+            SPH_ASSERT(e - t_lo < tile_cap);
+            const uint32_t gi = gsrc + e; // modulo 2^32: seg_start - p0 may wrap
+            float4 v = __ldg(src[0] + gi);
             v.x -= (v.x >= tx) ? L : 0.f;
             v.y -= (v.y >= ty) ? L : 0.f;
             v.z -= (v.z >= tz) ? L : 0.f;
             tiles[0][e - t_lo] = v;
 #pragma unroll
-            for (int a = 1; a < NARR; a++) tiles[a][e - t_lo] = __ldg(src[a] + gsrc + e);
+            for (int a = 1; a < NARR; a++) tiles[a][e - t_lo] = __ldg(src[a] + gi);
         }
     }
 }

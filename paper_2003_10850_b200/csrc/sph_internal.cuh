@@ -7,6 +7,13 @@
 
 #include "sph.h"
 
+#ifdef SPH_DEBUG
+#include <assert.h>
+#define SPH_ASSERT(c) assert(c)
+#else
+#define SPH_ASSERT(c) ((void)0)
+#endif
+
 #define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
 #define SPH_KEY_BITS (3 * SPH_LMAX)
 #define SPH_MAXB 32         // max actives per group (= max leaf capacity)

@@ -71,7 +71,7 @@ def check_density_stage(g, o, sel=None, label=""):
     rel = np.abs(grho - o["rho"]) / o["rho"]
     assert rel.max() <= RTOL_RHO, f"{label}: rho rel err {rel.max():.3e}"
     om_o = o["omega"]
-    relo = np.abs(gom - om_o) / np.abs(om_o)
+    relo = np.abs(gom - om_o) / np.where(om_o != 0, np.abs(om_o), 1.0)  # a lone particle has Omega = 0 exactly
     assert relo.max() <= RTOL_RHO, f"{label}: omega rel err {relo.max():.3e}"
     return dict(n_edge=int(edge.sum()), n_mismatch=int(mism.sum()), rho_err=float(rel.max()), omega_err=float(relo.max()))
 
