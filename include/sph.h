@@ -78,6 +78,11 @@ typedef struct {
     /* counters of the most recent sph_hydro_force call */
     int64_t force_candidates;
     int64_t force_pairs;       /* true pairs r < max(H_i,H_j), self excluded */
+    /* device times (CUDA events on the context's stream) of the most recent calls, milliseconds */
+    float t_index_ms;          /* sph_build_index: all kernels a1-a5 */
+    float t_density_kernel_ms; /* the persistent gather + h-iteration kernel alone (a6-a9) */
+    float t_force_prep_ms;     /* sorted force state + per-node max H (a9/a4 refresh) */
+    float t_force_kernel_ms;   /* the hydro-force gather kernel alone (a10-a11) */
 } sph_stats;
 
 /* Create a context. `cuda_stream` is a cudaStream_t (NULL = legacy default stream). */
@@ -153,6 +158,15 @@ int sph_get_stats(sph_ctx *ctx, sph_stats *out_host);
 
 /* Text of the most recent error of this context ("" if none). Never NULL; valid until the next call. */
 const char *sph_last_error(const sph_ctx *ctx);
+
+/*
+ * FP32 FMA issue-rate probe (measurement support, not part of the path): runs a register-only
+ * chain of fused multiply-adds on every SM for about `iters` x 4096 FMAs per thread and returns the
+ * achieved rate in TFLOP/s (2 flop per FMA) in *tflops_host.  packed != 0 uses the two-wide
+ * fma.rn.f32x2 form of sm_100.  Synchronises.  Used by bench.py to report the ALU roofline
+ * denominator measured on the same device next to the derived one.
+ */
+int sph_fp32_peak(sph_ctx *ctx, int iters, int packed, double *tflops_host);
 
 /* Library version string and the compute capability it was built for ("sm_100a"). */
 const char *sph_version(void);

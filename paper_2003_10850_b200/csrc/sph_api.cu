@@ -71,6 +71,12 @@ int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream)
         return SPH_E_OOM;
     }
     cudaMemsetAsync(ctx->cnt, 0, sizeof(SphCounters), ctx->stream);
+    for (int i = 0; i < 8; i++)
+        if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) {
+            cudaFree(ctx->cnt);
+            free(ctx);
+            return SPH_E_CUDA;
+        }
     *out = ctx;
     return SPH_OK;
 }
@@ -86,6 +92,7 @@ int sph_destroy(sph_ctx *ctx)
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
     dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
+    for (int i = 0; i < 8; i++) cudaEventDestroy(ctx->ev[i]);
     free(ctx);
     return SPH_OK;
 }
@@ -102,7 +109,11 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
     ctx->has_mass = mass != nullptr;
     ctx->mass_scalar = mass ? 1.f : mass_scalar;
     ctx->err[0] = 0;
-    return sph_index_build(ctx, pos, mass);
+    cudaEventRecord(ctx->ev[0], ctx->stream);
+    rc = sph_index_build(ctx, pos, mass);
+    cudaEventRecord(ctx->ev[1], ctx->stream);
+    ctx->ev_set[0] = true;
+    return rc;
 }
 
 int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol, float *h,
@@ -226,6 +237,12 @@ int sph_get_stats(sph_ctx *ctx, sph_stats *out)
     out->dens_pairs = (int64_t)h.dens_pairs;
     out->force_candidates = (int64_t)h.force_cands;
     out->force_pairs = (int64_t)h.force_pairs;
+    float *t[4] = {&out->t_index_ms, &out->t_density_kernel_ms, &out->t_force_prep_ms, &out->t_force_kernel_ms};
+    for (int i = 0; i < 4; i++)
+        if (ctx->ev_set[i] && cudaEventElapsedTime(t[i], ctx->ev[2 * i], ctx->ev[2 * i + 1]) != cudaSuccess) {
+            *t[i] = 0.f;
+            cudaGetLastError();
+        }
     return SPH_OK;
 }
 

@@ -413,10 +413,13 @@ int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_targe
     int grid = ctx->device_sms * 5;
     if (est_groups < grid) grid = (int)(est_groups > 0 ? est_groups : 1);
     int rc;
+    cudaEventRecord(ctx->ev[2], ctx->stream);
     if (ctx->prm.kernel == SPH_KERNEL_CUBIC)
         rc = ctx->has_mass ? launch<SPH_KERNEL_CUBIC, true>(ctx, a, grid) : launch<SPH_KERNEL_CUBIC, false>(ctx, a, grid);
     else
         rc = ctx->has_mass ? launch<SPH_KERNEL_WC6, true>(ctx, a, grid) : launch<SPH_KERNEL_WC6, false>(ctx, a, grid);
+    cudaEventRecord(ctx->ev[3], ctx->stream);
+    ctx->ev_set[1] = true;
     ctx->launches++;
     return rc;
 }

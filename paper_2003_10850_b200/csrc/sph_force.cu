@@ -353,12 +353,15 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     cudaStream_t st = ctx->stream;
     const int64_t n = ctx->n;
     const int T = 256;
+    cudaEventRecord(ctx->ev[4], st);
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
                                                        ctx->f_xyzh, ctx->f_vc, ctx->f_raf);
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->node_hmax, 0, sizeof(float) * ctx->n_nodes, st));
     k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
     sph_reset_counters(ctx, 1);
     ctx->launches += 3;
+    cudaEventRecord(ctx->ev[5], st);
+    ctx->ev_set[2] = true;
 
     ForceArgs a;
     a.nodes = ctx->nodes;
@@ -377,7 +380,10 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     int64_t est_groups = subset ? n_items : ctx->n_groups;
     int grid = ctx->device_sms * 3;
     if (est_groups < grid) grid = (int)(est_groups > 0 ? est_groups : 1);
+    cudaEventRecord(ctx->ev[6], st);
     int rc = ctx->prm.kernel == SPH_KERNEL_CUBIC ? launch<SPH_KERNEL_CUBIC>(ctx, a, grid) : launch<SPH_KERNEL_WC6>(ctx, a, grid);
+    cudaEventRecord(ctx->ev[7], st);
+    ctx->ev_set[3] = true;
     ctx->launches++;
     return rc;
 }

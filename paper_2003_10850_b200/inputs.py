@@ -146,10 +146,10 @@ def config3(n: int = 1 << 21, n_spheres: int = 200, seed: int | None = None) -> 
     def profile(k, r):
         return 3.0 * per[k] / (4.0 * math.pi * a[k] ** 3) * (1.0 + (r / a[k]) ** 2) ** -2.5
 
-    hg, _ = _analytic_density_guess(pos.astype(np.float64), n_bg, centres, 30.0 * a, profile, 64.0, rng)
+    hg, nd = _analytic_density_guess(pos.astype(np.float64), n_bg, centres, 30.0 * a, profile, 64.0, rng)
     halo = np.concatenate([np.full(n_bg, -1), np.repeat(np.arange(n_spheres), per)]).astype(np.int32)
     return ParticleSet("C3", pos, vel, u, hg, 1.0 / n, KERNEL_CUBIC, 64.0, 2.0,
-                       aux={"halo": halo, "a": a, "centres": centres, "per": per})
+                       aux={"halo": halo, "a": a, "centres": centres, "per": per, "n_density": nd})
 
 
 def _nfw_m(x):
@@ -203,11 +203,11 @@ def config4(n: int = 10_000_000, n_halos: int = 2000, seed: int | None = None,
         x = np.maximum(r / r_s[k], 1e-4)
         return per[k] / (4.0 * math.pi * r_s[k] ** 3 * mc[k]) / (x * (1.0 + x) ** 2)
 
-    hg, _ = _analytic_density_guess(pos.astype(np.float64), n_bg, centres, r_vir, profile, 295.0, rng)
+    hg, nd = _analytic_density_guess(pos.astype(np.float64), n_bg, centres, r_vir, profile, 295.0, rng)
     halo = np.concatenate([np.full(n_bg, -1), np.repeat(np.arange(n_halos), per)]).astype(np.int32)
     return ParticleSet("C4", pos, vel, u, hg, 1.0 / n, KERNEL_WC6, 295.0, 2.0,
                        aux={"halo": halo, "radius": np.concatenate(radii), "per": per, "conc": conc,
-                            "r_s": r_s, "r_vir": r_vir, "centres": centres, "n_bg": n_bg})
+                            "r_s": r_s, "r_vir": r_vir, "centres": centres, "n_bg": n_bg, "n_density": nd})
 
 
 def select_active_by_timebin(ps: ParticleSet, n_active: int) -> np.ndarray:

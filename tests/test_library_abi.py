@@ -11,7 +11,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def _declared():
     src = open(os.path.join(ROOT, "include", "sph.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sph_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sph_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_symbols_exported():
@@ -20,7 +20,7 @@ def test_header_symbols_exported():
     lib = ctypes.CDLL(build.build())
     names = _declared()
     assert {"sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
-            "sph_get_stats", "sph_last_error", "sph_version"} <= set(names)
+            "sph_get_stats", "sph_fp32_peak", "sph_last_error", "sph_version"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
     lib.sph_version.restype = ctypes.c_char_p
