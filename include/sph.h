@@ -63,7 +63,7 @@ typedef struct {
     float alpha_visc;  /* artificial viscosity alpha (1.0), R9 */
     int count_mode;    /* 0: kernel-weighted neighbour number drives the h iteration, 1: integer count (R2) */
     int max_iter;      /* cap on evaluations per particle (64); 1..255 */
-    int leaf_cap;      /* octree leaf capacity = max active particles per group; 0 = default (32); <= 32 */
+    int group_cap;     /* max active particles per group (one warp per group); 0 = default (8); <= 32 */
 } sph_params;
 
 typedef struct {
@@ -92,8 +92,8 @@ int sph_destroy(sph_ctx *ctx);
 /*
  * Build the spatial index over n particles (steps a1-a5 of DESIGN.md): 48-bit Morton keys
  * (16 bits per axis), radix sort of (key, id), sorted float4 copy (x,y,z,m), inverse permutation,
- * an octree over the sorted order whose leaves hold <= leaf_cap particles, and the leaf-chunk group
- * list.  Replaces the paper's Hilbert keys + domain decomposition + tree build (§1,
+ * an octree over the sorted order whose leaves hold <= 32 particles, and the group list (every leaf
+ * cut into balanced runs of <= group_cap consecutive particles).  Replaces the paper's Hilbert keys + domain decomposition + tree build (§1,
  * :194-196 §4).
  *   pos   [n*3] device, x,y,z per particle, 0 <= x < box (values outside are clamped into the
  *         boundary cells for the search and otherwise used as given);

@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph.so")
 SOURCES = ["sph_api.cu", "sph_index.cu", "sph_density.cu", "sph_force.cu", "sph_probe.cu"]
-HEADERS = ["sph_internal.cuh", "sph_gather.cuh", os.path.join(ROOT, "include", "sph.h")]
+HEADERS = ["sph_internal.cuh", "sph_warp.cuh", os.path.join(ROOT, "include", "sph.h")]
 
 
 def _stale() -> bool:

@@ -5,15 +5,17 @@
 // module (§1).  Formulas: DESIGN.md readings R8-R12.  The neighbour set is symmetric,
 // r_ij < max(H_i, H_j) (R10): the walk prunes a node only if it is farther from the group than both
 // the group's reach and the largest support radius inside the node.
-#include "sph_gather.cuh"
-
-#define FORCE_TILE 1024 // candidates per shared-memory tile (3 float4 each, 48 KB)
+//
+// Same warp-per-group mapping as sph_density.cu: lane = (active, stream); candidates' (x,y,z,H) are
+// streamed through the warp's ring by bulk copies and tested; a hit pushes the candidate's sorted slot
+// onto the lane's queue; queued hits are evaluated in bulk, fetching the pair's remaining state
+// (velocity, sound speed, rho, A, m) from the sorted arrays through L1.
+#include "sph_warp.cuh"
 
 namespace {
 
 struct ForceArgs {
     const SphNode *nodes;
-    uint32_t n_nodes;
     const float *node_hmax;
     const float4 *xyzh, *vc, *raf; // sorted: (x,y,z,H) (vx,vy,vz,c) (rho, A, m, slot)
     const uint32_t *perm;
@@ -44,253 +46,232 @@ __device__ __forceinline__ float kern_sigma()
     return KERNEL == SPH_KERNEL_CUBIC ? 2.54647908947032537f : 6.78895304126365994f;
 }
 
-struct ForceShared {
-    WalkShared ws;
-    float ax[SPH_MAXB], ay[SPH_MAXB], az[SPH_MAXB], aH[SPH_MAXB];
-    float aHinv[SPH_MAXB], aF4[SPH_MAXB]; // 1/H_i, sigma/H_i^4
-    float avx[SPH_MAXB], avy[SPH_MAXB], avz[SPH_MAXB], ac[SPH_MAXB], arho[SPH_MAXB], aA[SPH_MAXB];
-    uint32_t aslot[SPH_MAXB], aid[SPH_MAXB];
-    double fx[SPH_MAXB], fy[SPH_MAXB], fz[SPH_MAXB], fdu[SPH_MAXB];
-    int fvs[SPH_MAXB]; // max signal velocity as float bits (>= 0: integer order == float order)
-    int aCnt[SPH_MAXB];
-    int n_u, g;
-    unsigned short q[SPH_WARPS][SPH_ABLK][SPH_QCAP];
+struct ForceWarp {
+    float4 ring[SPH_NSLOT * SPH_CH];
+    WarpWalk ws;
+    uint32_t q[SPH_QCAP * 32];          // hit queue: sorted slot of the neighbour
+    uint32_t gidx[SPH_NSLOT * SPH_CH];  // sorted slot of every candidate in the ring
+    uint64_t bars[SPH_NSLOT];
 };
 
-template <int KERNEL, bool PAIRWRAP, int A>
-__device__ __forceinline__ void force_unit(ForceShared &sh, const float4 *__restrict__ t0, const float4 *__restrict__ t1,
-                                           const float4 *__restrict__ t2, int c0, int c1, int ub, float L, float alpha)
+// per-lane state of the lane's active and its running sums
+struct ForceLane {
+    float xi, yi, zi, h2, hinv, f4;  // position, H^2, 1/H, sigma/H^4
+    float vx, vy, vz, c, rho, A;
+    uint32_t slot;
+    float px, py, pz, pdu, pvs;
+    int cn, cnt;
+};
+
+// evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
+template <int KERNEL, bool PAIRWRAP>
+__device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned lt = lanemask_lt();
-    float xi[A], yi[A], zi[A], h2[A];
-    float px[A], py[A], pz[A], pdu[A], pvs[A];
-    int cn[A];
-    unsigned tail[A], head[A];
-    const float tx = sh.ws.thr[0], ty = sh.ws.thr[1], tz = sh.ws.thr[2];
-#pragma unroll
-    for (int a = 0; a < A; a++) {
-        int k = ub + a;
-        float x = sh.ax[k], y = sh.ay[k], z = sh.az[k], H = sh.aH[k];
-        xi[a] = x - ((x >= tx) ? L : 0.f);
-        yi[a] = y - ((y >= ty) ? L : 0.f);
-        zi[a] = z - ((z >= tz) ? L : 0.f);
-        h2[a] = H * H;
-        px[a] = py[a] = pz[a] = pdu[a] = pvs[a] = 0.f;
-        cn[a] = 0;
-        tail[a] = head[a] = 0u;
-    }
-    unsigned short *qw = &sh.q[warp][0][0];
-
-    auto flush = [&](int a, int nvalid) {
-        __syncwarp();
-        if (lane < nvalid) {
-            const int k = ub + a;
-            unsigned p = (head[a] + lane) & (SPH_QCAP - 1);
-            int j = qw[a * SPH_QCAP + p];
-            float4 P0 = t0[j], P1 = t1[j], P2 = t2[j];
-            if (__float_as_uint(P2.w) != sh.aslot[k]) { // j != i
-                float dx, dy, dz;
-                if (PAIRWRAP) {
-                    dx = image_diff(xi[a], P0.x, L); dy = image_diff(yi[a], P0.y, L); dz = image_diff(zi[a], P0.z, L);
-                } else {
-                    dx = xi[a] - P0.x; dy = yi[a] - P0.y; dz = zi[a] - P0.z;
-                }
-                float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                float rinv = rsqrtf(fmaxf(r2, 1e-37f));
-                float r = r2 * rinv;
-                float hinv_j = __fdividef(1.f, P0.w);
-                float hj2 = hinv_j * hinv_j;
-                float Fi = sh.aF4[k] * kern_dw<KERNEL>(r * sh.aHinv[k]);
-                float Fj = kern_sigma<KERNEL>() * hj2 * hj2 * kern_dw<KERNEL>(r * hinv_j);
-                float dvx = sh.avx[k] - P1.x, dvy = sh.avy[k] - P1.y, dvz = sh.avz[k] - P1.z;
-                float vr = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx)) * rinv;
-                float mu = fminf(vr, 0.f);
-                float vs = sh.ac[k] + P1.w - 3.f * mu;
-                float Pi = -alpha * vs * mu * __fdividef(1.f, sh.arho[k] + P2.x);
-                float Fbar = 0.5f * (Fi + Fj);
-                float AiFi = sh.aA[k] * Fi;
-                float pv = Pi * Fbar;
-                float t = P2.z * (AiFi + fmaf(P2.y, Fj, pv));
-                float tr = t * rinv;
-                px[a] = fmaf(-tr, dx, px[a]);
-                py[a] = fmaf(-tr, dy, py[a]);
-                pz[a] = fmaf(-tr, dz, pz[a]);
-                pdu[a] = fmaf(P2.z * fmaf(0.5f, pv, AiFi), vr, pdu[a]);
-                pvs[a] = fmaxf(pvs[a], vs);
-            }
-        }
-        __syncwarp();
-    };
-
-    for (int j0 = c0; j0 < c1; j0 += 32) {
-        int j = j0 + lane;
-        float4 c = (j < c1) ? t0[j] : make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
-        float hj2 = c.w * c.w;
-#pragma unroll
-        for (int a = 0; a < A; a++) {
+    const int m = min(n, A.cnt), base = A.cnt - m;
+    const float L = a.L, alpha = a.alpha;
+#pragma unroll 2
+    for (int k = 0; k < n; k++) {
+        if (k < m) {
+            const uint32_t j = qp[(base + k) * 32];
+            const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + j), P2 = __ldg(a.raf + j);
             float dx, dy, dz;
             if (PAIRWRAP) {
-                dx = image_diff(xi[a], c.x, L); dy = image_diff(yi[a], c.y, L); dz = image_diff(zi[a], c.z, L);
+                dx = image_diff(A.xi, P0.x, L); dy = image_diff(A.yi, P0.y, L); dz = image_diff(A.zi, P0.z, L);
             } else {
-                dx = xi[a] - c.x; dy = yi[a] - c.y; dz = zi[a] - c.z;
+                dx = A.xi - P0.x; dy = A.yi - P0.y; dz = A.zi - P0.z;
             }
-            float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            bool hit = r2 < fmaxf(h2[a], hj2);
-            unsigned m = __ballot_sync(FULLMASK, hit);
-            if (m) {
-                if (hit) {
-                    unsigned p = (tail[a] + __popc(m & lt)) & (SPH_QCAP - 1);
-                    qw[a * SPH_QCAP + p] = (unsigned short)j;
-                }
-                int nh = __popc(m);
-                tail[a] += nh;
-                cn[a] += nh;
-                if (tail[a] - head[a] >= 32u) {
-                    flush(a, 32);
-                    head[a] += 32u;
-                }
-            }
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
+            const float r = r2 * rinv;
+            const float hinv_j = __fdividef(1.f, P0.w);
+            const float hj2 = hinv_j * hinv_j;
+            const float Fi = A.f4 * kern_dw<KERNEL>(r * A.hinv);
+            const float Fj = kern_sigma<KERNEL>() * hj2 * hj2 * kern_dw<KERNEL>(r * hinv_j);
+            const float dvx = A.vx - P1.x, dvy = A.vy - P1.y, dvz = A.vz - P1.z;
+            const float vr = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx)) * rinv;
+            const float mu = fminf(vr, 0.f);
+            const float vs = A.c + P1.w - 3.f * mu;
+            const float Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
+            const float Fbar = 0.5f * (Fi + Fj);
+            const float AiFi = A.A * Fi;
+            const float pv = Pi * Fbar;
+            const bool other = j != A.slot; // j == i: no self force, no self signal velocity
+            // select, not multiply by zero: a lone particle has Omega = 0, hence A = inf
+            const float tr = other ? P2.z * (AiFi + fmaf(P2.y, Fj, pv)) * rinv : 0.f;
+            const float du = other ? P2.z * fmaf(0.5f, pv, AiFi) * vr : 0.f;
+            A.px = fmaf(-tr, dx, A.px);
+            A.py = fmaf(-tr, dy, A.py);
+            A.pz = fmaf(-tr, dz, A.pz);
+            A.pdu += du;
+            A.pvs = fmaxf(A.pvs, other ? vs : 0.f);
         }
     }
-#pragma unroll
-    for (int a = 0; a < A; a++) {
-        int rem = (int)(tail[a] - head[a]);
-        if (rem > 0) flush(a, rem);
-        double X = warp_sum_d((double)px[a]), Y = warp_sum_d((double)py[a]), Z = warp_sum_d((double)pz[a]);
-        double U = warp_sum_d((double)pdu[a]);
-        float V = warp_max(pvs[a]);
-        if (lane == 0) {
-            int k = ub + a;
-            atomicAdd(&sh.fx[k], X);
-            atomicAdd(&sh.fy[k], Y);
-            atomicAdd(&sh.fz[k], Z);
-            atomicAdd(&sh.fdu[k], U);
-            atomicMax(&sh.fvs[k], __float_as_int(V));
-            atomicAdd(&sh.aCnt[k], cn[a]);
-        }
-    }
+    A.cn += m;
+    A.cnt = base;
 }
 
 template <int KERNEL, bool PAIRWRAP>
-__device__ __forceinline__ void force_units(ForceShared &sh, const float4 *t0, const float4 *t1, const float4 *t2, int tn,
-                                            float L, float alpha)
+__device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,
+                                              const uint32_t *__restrict__ gp, uint32_t *__restrict__ qp, ForceLane &A,
+                                              int s, int f, bool live)
 {
-    const int warp = threadIdx.x >> 5;
-    const int n_u = sh.n_u;
-    UnitPlan pl = plan_units(n_u);
-    int units = pl.nb * pl.parts;
-    for (int un = warp; un < units; un += SPH_WARPS) {
-        int b = un / pl.parts, part = un - b * pl.parts;
-        int ub = (b * n_u) / pl.nb, ue = ((b + 1) * n_u) / pl.nb;
-        int per = (((tn + pl.parts - 1) / pl.parts) + 31) & ~31;
-        int c0 = min(part * per, tn), c1 = min(c0 + per, tn);
-        int A = ue - ub;
-        if (A <= 0 || c0 >= c1) continue;
-        switch (A) {
-        case 1: force_unit<KERNEL, PAIRWRAP, 1>(sh, t0, t1, t2, c0, c1, ub, L, alpha); break;
-        case 2: force_unit<KERNEL, PAIRWRAP, 2>(sh, t0, t1, t2, c0, c1, ub, L, alpha); break;
-        case 3: force_unit<KERNEL, PAIRWRAP, 3>(sh, t0, t1, t2, c0, c1, ub, L, alpha); break;
-        default: force_unit<KERNEL, PAIRWRAP, 4>(sh, t0, t1, t2, c0, c1, ub, L, alpha); break;
+    const int steps = SPH_CH / f;
+    const float4 *cp = slotp + s;
+    const uint32_t *gpp = gp + s;
+    const float L = a.L;
+    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
+        const int nt = min(SPH_QSTEP, steps - t0);
+        const int mx = __reduce_max_sync(FULLMASK, A.cnt);
+        if (mx + nt > SPH_QCAP) {
+            const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
+            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + nt - SPH_QCAP));
+        }
+#pragma unroll 4
+        for (int t = 0; t < nt; t++) {
+            const float4 c = *cp;
+            float dx, dy, dz;
+            if (PAIRWRAP) {
+                dx = image_diff(A.xi, c.x, L); dy = image_diff(A.yi, c.y, L); dz = image_diff(A.zi, c.z, L);
+            } else {
+                dx = A.xi - c.x; dy = A.yi - c.y; dz = A.zi - c.z;
+            }
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            if (r2 < fmaxf(A.h2, c.w * c.w)) {
+                qp[A.cnt * 32] = *gpp;
+                A.cnt++;
+            }
+            cp += f;
+            gpp += f;
         }
     }
 }
 
 template <int KERNEL>
-__global__ void __launch_bounds__(SPH_THREADS) k_force(ForceArgs a)
+__global__ void __launch_bounds__(SPH_THREADS, 3) k_force(ForceArgs a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *t0 = reinterpret_cast<float4 *>(smem_raw);
-    float4 *t1 = t0 + FORCE_TILE;
-    float4 *t2 = t1 + FORCE_TILE;
-    __shared__ ForceShared sh;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    ForceWarp &W = reinterpret_cast<ForceWarp *>(smem_raw)[warp];
     const float L = a.L;
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_cands = 0, st_pairs = 0;
+    RingCtl<1> rc;
+    rc.nfill = rc.ncons = 0;
+    rc.kseg = 0;
+    if (lane == 0) {
+        for (int i = 0; i < SPH_NSLOT; i++) mbar_init(&W.bars[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    fence_proxy_async();
+    __syncwarp();
+    const float4 *const src[1] = {a.xyzh};
+    uint32_t *qp = W.q + lane;
 
+    unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups
     for (;;) {
-        __syncthreads();
-        if (tid == 0) sh.g = (int)atomicAdd(&a.cnt->work, 1u);
-        __syncthreads();
-        const unsigned int g = (unsigned int)sh.g;
-        if (g >= n_groups) break;
-        const uint32_t i0 = a.gstart[g];
-        const uint32_t i1 = (g + 1 < n_groups) ? a.gstart[g + 1] : a.n_items;
-        const int na = (int)(i1 - i0);
-        if (tid < na) {
-            uint32_t slot = a.item_slot ? a.item_slot[i0 + tid] : i0 + tid;
-            float4 p0 = a.xyzh[slot], p1 = a.vc[slot], p2 = a.raf[slot];
-            sh.aslot[tid] = slot;
-            sh.aid[tid] = a.perm[slot];
-            sh.ax[tid] = p0.x; sh.ay[tid] = p0.y; sh.az[tid] = p0.z; sh.aH[tid] = p0.w;
-            float hinv = 1.f / p0.w, h2i = hinv * hinv;
-            sh.aHinv[tid] = hinv;
-            sh.aF4[tid] = kern_sigma<KERNEL>() * h2i * h2i;
-            sh.avx[tid] = p1.x; sh.avy[tid] = p1.y; sh.avz[tid] = p1.z; sh.ac[tid] = p1.w;
-            sh.arho[tid] = p2.x; sh.aA[tid] = p2.y;
-            sh.fx[tid] = sh.fy[tid] = sh.fz[tid] = sh.fdu[tid] = 0.0;
-            sh.fvs[tid] = 0;
-            sh.aCnt[tid] = 0;
+        if (gnext == gend) {
+            if (lane == 0) gnext = atomicAdd(&a.cnt->work, (unsigned int)SPH_GBLOCK);
+            gnext = __shfl_sync(FULLMASK, gnext, 0);
+            if (gnext >= n_groups) break;
+            gend = min(gnext + SPH_GBLOCK, n_groups);
         }
-        if (tid == 0) sh.n_u = na;
-        __syncthreads();
-        if (warp == 0) {
-            float x0 = 3e38f, x1 = -3e38f, y0 = 3e38f, y1 = -3e38f, z0 = 3e38f, z1 = -3e38f, hm = 0.f;
-            if (lane < na) {
-                x0 = x1 = sh.ax[lane]; y0 = y1 = sh.ay[lane]; z0 = z1 = sh.az[lane];
-                hm = sh.aH[lane];
+        const unsigned int grp = gnext++;
+        const uint32_t i0 = a.gstart[grp];
+        const uint32_t i1 = (grp + 1 < n_groups) ? a.gstart[grp + 1] : a.n_items;
+        const int g = (int)(i1 - i0);
+        const int f = streams_for(g);
+        const bool live = lane < g * f;
+        const int ai = live ? lane % g : 0, s = live ? lane / g : 0;
+        ForceLane A;
+        {
+            const uint32_t slot = a.item_slot ? a.item_slot[i0 + ai] : i0 + ai;
+            const float4 p0 = a.xyzh[slot], p1 = a.vc[slot], p2 = a.raf[slot];
+            A.slot = slot;
+            A.xi = live ? p0.x : SPH_NANF; // dead lanes never hit
+            A.yi = p0.y; A.zi = p0.z;
+            A.h2 = p0.w * p0.w;
+            A.hinv = 1.f / p0.w;
+            const float h2i = A.hinv * A.hinv;
+            A.f4 = kern_sigma<KERNEL>() * h2i * h2i;
+            A.vx = p1.x; A.vy = p1.y; A.vz = p1.z; A.c = p1.w;
+            A.rho = p2.x; A.A = p2.y;
+            A.px = A.py = A.pz = A.pdu = A.pvs = 0.f;
+            A.cn = A.cnt = 0;
+            // bounding box and reach of the group
+            const float inf = __int_as_float(0x7f800000);
+            const float x0 = warp_min(live ? p0.x : inf), x1 = warp_max(live ? p0.x : -inf);
+            const float y0 = warp_min(live ? p0.y : inf), y1 = warp_max(live ? p0.y : -inf);
+            const float z0 = warp_min(live ? p0.z : inf), z1 = warp_max(live ? p0.z : -inf);
+            const float hg = warp_max(live ? p0.w : 0.f);
+            const float gcx = 0.5f * (x0 + x1), ghx = 0.5f * (x1 - x0) * (1.f + 1e-6f);
+            const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
+            const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
+
+            WalkCtl ctl;
+            ctl.sp = -1;
+            unsigned long long cands = 0;
+            bool anywrap = false;
+            do {
+                walk_batch<true>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
+                cands += ctl.total;
+                // queued hits of an earlier batch are evaluated in the frame they were found in
+                if (ctl.pairwrap != anywrap) {
+                    const int mxq = __reduce_max_sync(FULLMASK, A.cnt);
+                    if (anywrap) drain<KERNEL, true>(a, qp, A, mxq); else drain<KERNEL, false>(a, qp, A, mxq);
+                    anywrap = ctl.pairwrap;
+                }
+                const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
+                rc.kseg = 0;
+                uint32_t nf = 0;
+                for (; nf < nch && nf < SPH_NSLOT - 1; nf++) ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf, W.gidx);
+                for (uint32_t c = 0; c < nch; c++) {
+                    if (nf < nch) { ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf, W.gidx); nf++; }
+                    const uint32_t slot = ring_wait<1>(rc, W.bars);
+                    float4 *slotp = W.ring + slot * SPH_CH;
+                    const uint32_t nval = min((uint32_t)SPH_CH, ctl.total - c * SPH_CH);
+                    if (nval < SPH_CH) {
+                        for (uint32_t j = nval + lane; j < SPH_CH; j += 32) slotp[j] = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
+                        fence_proxy_async();
+                    }
+                    __syncwarp(); // gidx of this slot (written by the filling lanes) is visible to all
+                    if (anywrap) consume_chunk<KERNEL, true>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live);
+                    else consume_chunk<KERNEL, false>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live);
+                }
+            } while (ctl.sp > 0);
+            {
+                const int mxq = __reduce_max_sync(FULLMASK, A.cnt);
+                if (anywrap) drain<KERNEL, true>(a, qp, A, mxq); else drain<KERNEL, false>(a, qp, A, mxq);
             }
-            x0 = warp_min(x0); x1 = warp_max(x1);
-            y0 = warp_min(y0); y1 = warp_max(y1);
-            z0 = warp_min(z0); z1 = warp_max(z1);
-            hm = warp_max(hm);
-            if (lane == 0) {
-                sh.ws.gc[0] = 0.5f * (x0 + x1); sh.ws.gh[0] = 0.5f * (x1 - x0) * (1.f + 1e-6f);
-                sh.ws.gc[1] = 0.5f * (y0 + y1); sh.ws.gh[1] = 0.5f * (y1 - y0) * (1.f + 1e-6f);
-                sh.ws.gc[2] = 0.5f * (z0 + z1); sh.ws.gh[2] = 0.5f * (z1 - z0) * (1.f + 1e-6f);
-                sh.ws.hg = hm;
-                sh.ws.sp = -1;
+            // cross-stream totals
+            double X = (double)A.px, Y = (double)A.py, Z = (double)A.pz, U = (double)A.pdu;
+            float V = A.pvs;
+            int cn = A.cn;
+            for (int d = 1; d < f; d <<= 1) {
+                const bool take = live && s + d < f;
+                const int from = take ? lane + g * d : lane;
+                const double tX = __shfl_sync(FULLMASK, X, from), tY = __shfl_sync(FULLMASK, Y, from);
+                const double tZ = __shfl_sync(FULLMASK, Z, from), tU = __shfl_sync(FULLMASK, U, from);
+                const float tV = __shfl_sync(FULLMASK, V, from);
+                const int tn = __shfl_sync(FULLMASK, cn, from);
+                if (take) { X += tX; Y += tY; Z += tZ; U += tU; V = fmaxf(V, tV); cn += tn; }
             }
-            __syncwarp();
-        }
-        unsigned long long grp_cands = 0;
-        bool more_walk;
-        do {
-            __syncthreads();
-            if (warp == 0) walk_batch<true>(sh.ws, a.nodes, a.node_hmax, L, FORCE_TILE, a.n_nodes);
-            __syncthreads();
-            const uint32_t total = sh.ws.total;
-            more_walk = sh.ws.sp > 0;
-            grp_cands += total;
-            for (uint32_t tb = 0; tb < total; tb += FORCE_TILE) {
-                float4 *tiles[3] = {t0, t1, t2};
-                const float4 *srcs[3] = {a.xyzh, a.vc, a.raf};
-                stage_tile<3>(sh.ws, tiles, srcs, tb, FORCE_TILE, L);
-                __syncthreads();
-                int tn = (int)min((uint32_t)FORCE_TILE, total - tb);
-                if (sh.ws.pairwrap) force_units<KERNEL, true>(sh, t0, t1, t2, tn, L, a.alpha);
-                else force_units<KERNEL, false>(sh, t0, t1, t2, tn, L, a.alpha);
-                __syncthreads();
+            // a11: scatter to the caller's particle id
+            if (lane < g) {
+                const uint32_t id = a.perm[slot];
+                a.acc[3 * (size_t)id] = (float)X;
+                a.acc[3 * (size_t)id + 1] = (float)Y;
+                a.acc[3 * (size_t)id + 2] = (float)Z;
+                a.dudt[id] = (float)U;
+                a.vsig[id] = V;
             }
-        } while (more_walk);
-        // a11: scatter to the caller's particle id
-        if (tid < na) {
-            uint32_t id = sh.aid[tid];
-            a.acc[3 * (size_t)id] = (float)sh.fx[tid];
-            a.acc[3 * (size_t)id + 1] = (float)sh.fy[tid];
-            a.acc[3 * (size_t)id + 2] = (float)sh.fz[tid];
-            a.dudt[id] = (float)sh.fdu[tid];
-            a.vsig[id] = __int_as_float(sh.fvs[tid]);
-        }
-        if (warp == 0) {
-            unsigned long long pr = (lane < na) ? (unsigned long long)(sh.aCnt[lane] - 1) : 0ull; // minus self
+            unsigned long long pr = (lane < g) ? (unsigned long long)(cn - 1) : 0ull; // minus self
 #pragma unroll
             for (int o = 16; o; o >>= 1) pr += __shfl_xor_sync(FULLMASK, pr, o);
-            if (lane == 0) { st_pairs += pr; st_cands += grp_cands * (unsigned long long)na; }
+            st_pairs += pr;
+            st_cands += cands * (unsigned long long)g;
         }
     }
-    if (tid == 0) {
+    if (lane == 0) {
         if (st_cands) atomicAdd(&a.cnt->force_cands, st_cands);
         if (st_pairs) atomicAdd(&a.cnt->force_pairs, st_pairs);
     }
@@ -336,11 +317,18 @@ __global__ void k_node_hmax(const SphCounters *cnt, const SphNode *__restrict__ 
 }
 
 template <int KERNEL>
-int launch(sph_ctx *ctx, const ForceArgs &a, int grid)
+int launch(sph_ctx *ctx, const ForceArgs &a, int64_t est_groups)
 {
-    size_t dyn = 3 * sizeof(float4) * FORCE_TILE;
-    SPH_CUDA(ctx, cudaFuncSetAttribute(k_force<KERNEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
-    k_force<KERNEL><<<grid, SPH_THREADS, dyn, ctx->stream>>>(a);
+    size_t dyn = sizeof(ForceWarp) * SPH_WARPS;
+    auto kfn = k_force<KERNEL>;
+    SPH_CUDA(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
+    int per_sm = 1;
+    SPH_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kfn, SPH_THREADS, dyn));
+    if (per_sm < 1) return sph_fail(ctx, SPH_E_INTERNAL, "k_force does not fit on an SM");
+    int64_t grid = (int64_t)ctx->device_sms * per_sm;
+    int64_t need = (est_groups + SPH_WARPS * SPH_GBLOCK - 1) / (SPH_WARPS * SPH_GBLOCK);
+    if (need < grid) grid = need > 0 ? need : 1;
+    kfn<<<(int)grid, SPH_THREADS, dyn, ctx->stream>>>(a);
     SPH_CUDA(ctx, cudaGetLastError());
     return SPH_OK;
 }
@@ -365,7 +353,6 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
 
     ForceArgs a;
     a.nodes = ctx->nodes;
-    a.n_nodes = (uint32_t)ctx->n_nodes;
     a.node_hmax = ctx->node_hmax;
     a.xyzh = ctx->f_xyzh; a.vc = ctx->f_vc; a.raf = ctx->f_raf;
     a.perm = ctx->perm;
@@ -378,10 +365,8 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     a.alpha = ctx->prm.alpha_visc;
     a.acc = acc; a.dudt = dudt; a.vsig = vsig;
     int64_t est_groups = subset ? n_items : ctx->n_groups;
-    int grid = ctx->device_sms * 3;
-    if (est_groups < grid) grid = (int)(est_groups > 0 ? est_groups : 1);
     cudaEventRecord(ctx->ev[6], st);
-    int rc = ctx->prm.kernel == SPH_KERNEL_CUBIC ? launch<SPH_KERNEL_CUBIC>(ctx, a, grid) : launch<SPH_KERNEL_WC6>(ctx, a, grid);
+    int rc = ctx->prm.kernel == SPH_KERNEL_CUBIC ? launch<SPH_KERNEL_CUBIC>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6>(ctx, a, est_groups);
     cudaEventRecord(ctx->ev[7], st);
     ctx->ev_set[3] = true;
     ctx->launches++;

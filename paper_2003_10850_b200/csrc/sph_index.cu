@@ -123,15 +123,17 @@ __global__ void k_tree_split(SphCounters *cnt, SphNode *nodes, const uint64_t *_
     }
 }
 
-// a5 (all-active case): a group is a run of <= leaf_cap consecutive sorted slots inside one leaf
-__global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict__ nodes, uint32_t leaf_cap,
+// a5 (all-active case): every leaf is cut into ceil(count / grp_cap) balanced runs of consecutive
+// sorted slots; a run is a group (consecutive Morton order keeps a run spatially compact)
+__global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict__ nodes, uint32_t grp_cap,
                               uint32_t *__restrict__ mark)
 {
     uint32_t nn = cnt->n_nodes;
     for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) {
         SphNode p = nodes[nd];
         if (p.child != 0 || p.count == 0) continue;
-        for (uint32_t s = 0; s < p.count; s += leaf_cap) mark[p.start + s] = 1u;
+        const uint32_t ns = (p.count + grp_cap - 1) / grp_cap;
+        for (uint32_t s = 0; s < ns; s++) mark[p.start + (uint32_t)(((uint64_t)s * p.count) / ns)] = 1u;
     }
 }
 
@@ -178,7 +180,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
 {
     const int64_t n = ctx->n;
     cudaStream_t st = ctx->stream;
-    const uint32_t B = (uint32_t)ctx->leaf_cap;
+    const uint32_t B = SPH_LEAF;
     int rc;
     if (n > ctx->cap_n) {
         int64_t cap = n + n / 8 + 1024;
@@ -245,7 +247,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     }
     // a5: group starts in sorted order + group id of every slot
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->grp_mark, 0, sizeof(uint32_t) * n, st));
-    k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, B, ctx->grp_mark);
+    k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)ctx->grp_cap, ctx->grp_mark);
     ctx->launches++;
     tbs = ctx->cub_tmp_bytes;
     SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),

@@ -16,13 +16,19 @@
 
 #define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
 #define SPH_KEY_BITS (3 * SPH_LMAX)
-#define SPH_MAXB 32         // max actives per group (= max leaf capacity)
-#define SPH_WARPS 4         // warps per CTA of the gather kernels
+#define SPH_LEAF 32         // octree leaf capacity = largest candidate segment (one bulk copy)
+#define SPH_MAXB 32         // max actives per group (a warp: one lane per active and stream)
+#define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)
+#define SPH_WARPS 4         // warps per CTA of the gather kernels (warps are independent)
 #define SPH_THREADS (32 * SPH_WARPS)
-#define SPH_SMAX 512        // candidate segments per walk batch
-#define SPH_STK 512         // walk stack entries (blocks of 8 sibling nodes)
-#define SPH_QCAP 64         // hit-queue entries per (warp, active)
-#define SPH_ABLK 4          // actives register-blocked per warp pass
+#define SPH_SMAX 256        // candidate segments per walk batch (per warp)
+#define SPH_STK 256         // walk stack entries (blocks of 8 sibling nodes, per warp)
+#define SPH_STK4 112        // 4-block pops only while the stack is at most this deep
+#define SPH_CH 120          // candidates per ring chunk (divisible by 1..6, 8, 10, 12, 15, 20, 24, 30)
+#define SPH_NSLOT 3         // ring slots per warp
+#define SPH_QCAP 48         // per-lane hit-queue entries
+#define SPH_QSTEP 16        // test steps between queue-capacity checks
+#define SPH_GBLOCK 4         // consecutive groups a warp takes per work-counter increment
 
 // octree node, 32 bytes, read as two 16-byte loads
 struct __align__(16) SphNode {
@@ -57,7 +63,7 @@ struct sph_ctx {
     bool have_index;
     bool has_mass;
     float mass_scalar;
-    int leaf_cap;
+    int grp_cap;      // max actives per group
 
     // index (device)
     uint64_t *keys, *keys_alt;

@@ -280,13 +280,13 @@ def test_edge_oversize_leaf_many_coincident():
     g.close()
 
 
-def test_box_not_one_and_small_leaf_cap():
+def test_box_not_one_and_small_group_cap():
     ps = I.config2(16)
     s = 2.0
     pos = (ps.pos * s).astype(np.float32)
     hg = (ps.h_guess * s).astype(np.float32)
     o = O.density(pos, hg, kernel=0, n_target=64, n_tol=2, mass_scalar=ps.mass, box=s)
-    g = GpuRun(pos, 0, ps.mass, box=s, leaf_cap=8)
+    g = GpuRun(pos, 0, ps.mass, box=s, group_cap=8)
     gd = g.density(hg, 64, 2)
     check_density_e2e(gd, o, pos, hg, 0, ps.mass, 64, 2, label="box=2", box=s)
     g.close()
