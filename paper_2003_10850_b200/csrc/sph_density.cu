@@ -44,25 +44,34 @@ struct KernelConst<SPH_KERNEL_WC6> {
     static constexpr double sigma = 6.7889530412636599415; // 1365/(64 pi)
 };
 
-// w(q) and d(q) = 3 w + q w' from u = q^2 (R1); -sigma H^-4 d is dW/dH
+// packed f32x2 helpers (sm_100: FADD2 / FMUL2 / FFMA2 do two lanes of fp32 per issue slot)
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+
+// w(q) and d(q) = 3 w + q w' for two hits at once, from u = q^2 (R1); -sigma H^-4 d is dW/dH.
+// u = 1 gives w = d = 0 exactly (used to pad an odd tail).
 template <int KERNEL>
-__device__ __forceinline__ void kern_wd(float u, float &w, float &d)
+__device__ __forceinline__ void kern_wd2(float2 u, float2 &w, float2 &d)
 {
-    float q = u * rsqrtf(fmaxf(u, 1e-30f));
+    float2 q;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(q.x) : "f"(u.x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(q.y) : "f"(u.y));
+    const float2 t = __ffma2_rn(q, f2(-1.f), f2(1.f)), t2 = __fmul2_rn(t, t);
     if (KERNEL == SPH_KERNEL_CUBIC) {
-        float t = 1.f - q, t2 = t * t;
-        float wa = fmaf(u, fmaf(6.f, q, -6.f), 1.f), da = fmaf(u, fmaf(36.f, q, -30.f), 3.f);
-        float wb = 2.f * t2 * t, db = 6.f * t2 * fmaf(-2.f, q, 1.f);
-        bool in = q <= 0.5f;
-        w = in ? wa : wb;
-        d = in ? da : db;
+        // q <= 1/2: w = 1 - 6u + 6uq, d = 3 - 30u + 36uq;  else: w = 2 t^3, d = 6 t^2 (1 - 2q)
+        const float2 wa = __ffma2_rn(u, __ffma2_rn(f2(6.f), q, f2(-6.f)), f2(1.f));
+        const float2 da = __ffma2_rn(u, __ffma2_rn(f2(36.f), q, f2(-30.f)), f2(3.f));
+        const float2 wb = __fmul2_rn(__fmul2_rn(f2(2.f), t2), t);
+        const float2 db = __fmul2_rn(__fmul2_rn(f2(6.f), t2), __ffma2_rn(f2(-2.f), q, f2(1.f)));
+        w = f2(q.x <= 0.5f ? wa.x : wb.x, q.y <= 0.5f ? wa.y : wb.y);
+        d = f2(q.x <= 0.5f ? da.x : db.x, q.y <= 0.5f ? da.y : db.y);
     } else {
         // w = t^8 (1 + 8q + 25q^2 + 32q^3);  3w + q w' = t^7 (3 + 21q + 29q^2 - 133q^3 - 448q^4)
-        float t = 1.f - q, t2 = t * t, t4 = t2 * t2, t7 = t4 * t2 * t;
-        float p1 = fmaf(q, fmaf(q, fmaf(32.f, q, 25.f), 8.f), 1.f);
-        float p2 = fmaf(q, fmaf(q, fmaf(q, fmaf(-448.f, q, -133.f), 29.f), 21.f), 3.f);
-        w = t7 * t * p1;
-        d = t7 * p2;
+        const float2 t4 = __fmul2_rn(t2, t2), t7 = __fmul2_rn(__fmul2_rn(t4, t2), t);
+        const float2 p1 = __ffma2_rn(q, __ffma2_rn(q, __ffma2_rn(f2(32.f), q, f2(25.f)), f2(8.f)), f2(1.f));
+        const float2 p2 = __ffma2_rn(q, __ffma2_rn(q, __ffma2_rn(q, __ffma2_rn(f2(-448.f), q, f2(-133.f)), f2(29.f)), f2(21.f)), f2(3.f));
+        w = __fmul2_rn(__fmul2_rn(t7, t), p1);
+        d = __fmul2_rn(t7, p2);
     }
 }
 
@@ -81,30 +90,34 @@ struct DensWarp {
     int ulist[SPH_MAXB];                     // actives still iterating
 };
 
-// per-lane accumulators of one evaluation
+// per-lane accumulators of one evaluation (packed: two partial sums each)
 struct DensAcc {
-    float s0, s1, r0, r1;
-    int cn, cnt; // hits evaluated so far / hits waiting in the queue
+    float2 s, ds, r, dr; // sum w, sum d, sum m w, sum m d
+    int cn, cnt;         // hits evaluated so far / hits waiting in the queue
 };
 
-// evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
+// evaluate the m newest queued hits of every lane, two per step (n = warp-wide maximum of m)
 template <int KERNEL, bool HAS_MASS>
 __device__ __forceinline__ void drain(const float *__restrict__ qp, const float *__restrict__ qmp, DensAcc &A, int n,
                                       float ih2)
 {
     const int m = min(n, A.cnt), base = A.cnt - m;
+    const float2 ih22 = f2(ih2);
 #pragma unroll 2
-    for (int k = 0; k < n; k++) {
+    for (int k = 0; k < n; k += 2) {
         if (k < m) {
-            float u = qp[(base + k) * 32] * ih2;
-            float w, d;
-            kern_wd<KERNEL>(u, w, d);
-            A.s0 += w;
-            A.s1 += d;
+            const bool two = k + 1 < m;
+            const float r0 = qp[(base + k) * 32], r1 = two ? qp[(base + k + 1) * 32] : 0.f;
+            float2 u = __fmul2_rn(f2(r0, r1), ih22);
+            if (!two) u.y = 1.f; // odd tail: w = d = 0
+            float2 w, d;
+            kern_wd2<KERNEL>(u, w, d);
+            A.s = __fadd2_rn(A.s, w);
+            A.ds = __fadd2_rn(A.ds, d);
             if (HAS_MASS) {
-                float mj = qmp[(base + k) * 32];
-                A.r0 = fmaf(mj, w, A.r0);
-                A.r1 = fmaf(mj, d, A.r1);
+                const float2 mj = f2(qmp[(base + k) * 32], two ? qmp[(base + k + 1) * 32] : 0.f);
+                A.r = __ffma2_rn(mj, w, A.r);
+                A.dr = __ffma2_rn(mj, d, A.dr);
             }
         }
     }
@@ -112,40 +125,56 @@ __device__ __forceinline__ void drain(const float *__restrict__ qp, const float 
     A.cnt = base;
 }
 
-// Test the candidates of one ring slot against this lane's active: lane (a, s) takes candidates
-// s, s + f, s + 2f, ... of the chunk; a hit pushes r^2 (and the mass) onto the lane's queue.
+// Test the candidates of one prepared ring slot against this lane's active: lane (a, s) takes the
+// candidate pairs s, s + f, s + 2f, ... of the chunk; both distances of a pair come out of one packed
+// f32x2 chain; a hit pushes r^2 (and the mass) onto the lane's queue.
 template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(const float4 *__restrict__ slotp, float *__restrict__ qp,
                                               float *__restrict__ qmp, DensAcc &A, int s, int f, bool live, float xi,
                                               float yi, float zi, float h2, float ih2, float L)
 {
-    const int steps = SPH_CH / f;
-    const float4 *cp = slotp + s;
+    const int steps = (SPH_CH / 2) / f;
+    const float4 *cp = slotp + 2 * s;
+    const float2 nx = f2(-xi), ny = f2(-yi), nz = f2(-zi);
     for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, steps - t0);
-        // queue capacity: room for nt more hits in every lane, else evaluate queued hits first
+        // queue capacity: room for 2 nt more hits in every lane, else evaluate queued hits first
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
-        if (mx + nt > SPH_QCAP) {
+        if (mx + 2 * nt > SPH_QCAP) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, HAS_MASS>(qp, qmp, A, max(mn, mx + nt - SPH_QCAP), ih2);
+            drain<KERNEL, HAS_MASS>(qp, qmp, A, max(mn, mx + 2 * nt - SPH_QCAP), ih2);
         }
-#pragma unroll 4
+        // queue write cursor as a 32-bit shared-memory address (one STS + one add per hit)
+        const uint32_t q0 = smem_u32(qp);
+        uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
+        const uint32_t mofs = HAS_MASS ? smem_u32(qmp) - q0 : 0u;
+#pragma unroll 2
         for (int t = 0; t < nt; t++) {
-            const float4 c = *cp;
-            cp += f;
-            float dx, dy, dz;
+            const float4 c0 = cp[0], c1 = cp[1]; // (x0,x1,y0,y1) (z0,z1,w0,w1)
+            cp += 2 * f;
+            float2 r2;
             if (PAIRWRAP) {
-                dx = image_diff(xi, c.x, L); dy = image_diff(yi, c.y, L); dz = image_diff(zi, c.z, L);
+                const float dx0 = image_diff(xi, c0.x, L), dx1 = image_diff(xi, c0.y, L);
+                const float dy0 = image_diff(yi, c0.z, L), dy1 = image_diff(yi, c0.w, L);
+                const float dz0 = image_diff(zi, c1.x, L), dz1 = image_diff(zi, c1.y, L);
+                r2 = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
             } else {
-                dx = xi - c.x; dy = yi - c.y; dz = zi - c.z;
+                const float2 dx = __fadd2_rn(f2(c0.x, c0.y), nx), dy = __fadd2_rn(f2(c0.z, c0.w), ny);
+                const float2 dz = __fadd2_rn(f2(c1.x, c1.y), nz);
+                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (r2 < h2) {
-                qp[A.cnt * 32] = r2;
-                if (HAS_MASS) qmp[A.cnt * 32] = c.w;
-                A.cnt++;
+            if (r2.x < h2) {
+                sts_f32(qw, r2.x);
+                if (HAS_MASS) sts_f32(qw + mofs, c1.z);
+                qw += 128u;
+            }
+            if (r2.y < h2) {
+                sts_f32(qw, r2.y);
+                if (HAS_MASS) sts_f32(qw + mofs, c1.w);
+                qw += 128u;
             }
         }
+        A.cnt = (int)((qw - q0) >> 7);
     }
 }
 
@@ -175,7 +204,7 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
 
     DensAcc A;
-    A.s0 = A.s1 = A.r0 = A.r1 = 0.f;
+    A.s = A.ds = A.r = A.dr = f2(0.f);
     A.cn = A.cnt = 0;
     float *qp = W.q + lane, *qmp = W.qm + (HAS_MASS ? lane : 0);
     const float4 *const src[1] = {a.xyzm};
@@ -184,6 +213,10 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     do {
         walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
         cands += ctl.total;
+        // this lane's active in the batch's frame
+        const float xf = ctl.pairwrap ? xi : recentre(xi, ctl.thx, L);
+        const float yf = ctl.pairwrap ? yi : recentre(yi, ctl.thy, L);
+        const float zf = ctl.pairwrap ? zi : recentre(zi, ctl.thz, L);
         const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
         rc.kseg = 0;
         uint32_t nf = 0;
@@ -192,20 +225,16 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
             if (nf < nch) { ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf); nf++; }
             const uint32_t slot = ring_wait<1>(rc, W.bars);
             float4 *slotp = W.ring + slot * SPH_CH;
-            const uint32_t nval = min((uint32_t)SPH_CH, ctl.total - c * SPH_CH);
-            if (nval < SPH_CH) { // ragged tail: pad with NaN (every comparison with NaN is false)
-                for (uint32_t j = nval + lane; j < SPH_CH; j += 32) slotp[j] = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
-                fence_proxy_async();
-                __syncwarp();
-            }
-            if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(slotp, qp, qmp, A, s, f, live, xi, yi, zi, h2, ih2, L);
-            else consume_chunk<KERNEL, HAS_MASS, false>(slotp, qp, qmp, A, s, f, live, xi, yi, zi, h2, ih2, L);
+            slot_prepare(slotp, min((uint32_t)SPH_CH, ctl.total - c * SPH_CH), ctl, L);
+            if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(slotp, qp, qmp, A, s, f, live, xf, yf, zf, h2, ih2, L);
+            else consume_chunk<KERNEL, HAS_MASS, false>(slotp, qp, qmp, A, s, f, live, xf, yf, zf, h2, ih2, L);
         }
     } while (ctl.sp > 0);
     drain<KERNEL, HAS_MASS>(qp, qmp, A, __reduce_max_sync(FULLMASK, A.cnt), ih2);
 
     // cross-stream totals: lane a + g*s adds lane a + g*(s+d) for d = 1, 2, 4, ...
-    S = (double)A.s0; D = (double)A.s1; R = (double)A.r0; DR = (double)A.r1;
+    S = (double)A.s.x + (double)A.s.y; D = (double)A.ds.x + (double)A.ds.y;
+    R = (double)A.r.x + (double)A.r.y; DR = (double)A.dr.x + (double)A.dr.y;
     nint = A.cn;
     for (int d = 1; d < f; d <<= 1) {
         const bool take = live && s + d < f;
@@ -221,7 +250,7 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
 }
 
 template <int KERNEL, bool HAS_MASS>
-__global__ void __launch_bounds__(SPH_THREADS, 3) k_density(DensArgs a)
+__global__ void __launch_bounds__(SPH_THREADS, 4) k_density(DensArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

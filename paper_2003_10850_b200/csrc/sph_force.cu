@@ -63,12 +63,22 @@ struct ForceLane {
     int cn, cnt;
 };
 
+// frame of the batch the queued hits were found in (see walk_batch)
+struct Frame {
+    float thx, thy, thz;
+    bool pairwrap;
+};
+
 // evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
 template <int KERNEL, bool PAIRWRAP>
-__device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n)
+__device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
+                                      const Frame &fr)
 {
     const int m = min(n, A.cnt), base = A.cnt - m;
     const float L = a.L, alpha = a.alpha;
+    const float xf = PAIRWRAP ? A.xi : recentre(A.xi, fr.thx, L);
+    const float yf = PAIRWRAP ? A.yi : recentre(A.yi, fr.thy, L);
+    const float zf = PAIRWRAP ? A.zi : recentre(A.zi, fr.thz, L);
 #pragma unroll 2
     for (int k = 0; k < n; k++) {
         if (k < m) {
@@ -78,7 +88,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             if (PAIRWRAP) {
                 dx = image_diff(A.xi, P0.x, L); dy = image_diff(A.yi, P0.y, L); dz = image_diff(A.zi, P0.z, L);
             } else {
-                dx = A.xi - P0.x; dy = A.yi - P0.y; dz = A.zi - P0.z;
+                dx = xf - recentre(P0.x, fr.thx, L); dy = yf - recentre(P0.y, fr.thy, L); dz = zf - recentre(P0.z, fr.thz, L);
             }
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
@@ -110,44 +120,70 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
     A.cnt = base;
 }
 
+template <int KERNEL>
+__device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
+                                          const Frame &fr)
+{
+    if (fr.pairwrap) drain<KERNEL, true>(a, qp, A, n, fr);
+    else drain<KERNEL, false>(a, qp, A, n, fr);
+}
+
+// Test the candidate pairs of one prepared ring slot against this lane's active (symmetric set, R10):
+// hit if r^2 < max(H_i, H_j)^2; a hit pushes the candidate's sorted slot onto the lane's queue.
 template <int KERNEL, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,
                                               const uint32_t *__restrict__ gp, uint32_t *__restrict__ qp, ForceLane &A,
-                                              int s, int f, bool live)
+                                              int s, int f, bool live, const Frame &fr)
 {
-    const int steps = SPH_CH / f;
-    const float4 *cp = slotp + s;
-    const uint32_t *gpp = gp + s;
+    const int steps = (SPH_CH / 2) / f;
+    const float4 *cp = slotp + 2 * s;
+    uint32_t ga = smem_u32(gp + 2 * s);
     const float L = a.L;
+    const float xf = PAIRWRAP ? A.xi : recentre(A.xi, fr.thx, L);
+    const float yf = PAIRWRAP ? A.yi : recentre(A.yi, fr.thy, L);
+    const float zf = PAIRWRAP ? A.zi : recentre(A.zi, fr.thz, L);
+    const float2 nx = make_float2(-xf, -xf), ny = make_float2(-yf, -yf), nz = make_float2(-zf, -zf);
     for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, steps - t0);
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
-        if (mx + nt > SPH_QCAP) {
+        if (mx + 2 * nt > SPH_QCAP) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + nt - SPH_QCAP));
+            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP), fr);
         }
-#pragma unroll 4
+        const uint32_t q0 = smem_u32(qp);
+        uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
+#pragma unroll 2
         for (int t = 0; t < nt; t++) {
-            const float4 c = *cp;
-            float dx, dy, dz;
+            const float4 c0 = cp[0], c1 = cp[1]; // (x0,x1,y0,y1) (z0,z1,h0,h1)
+            cp += 2 * f;
+            float2 r2;
             if (PAIRWRAP) {
-                dx = image_diff(A.xi, c.x, L); dy = image_diff(A.yi, c.y, L); dz = image_diff(A.zi, c.z, L);
+                const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);
+                const float dy0 = image_diff(A.yi, c0.z, L), dy1 = image_diff(A.yi, c0.w, L);
+                const float dz0 = image_diff(A.zi, c1.x, L), dz1 = image_diff(A.zi, c1.y, L);
+                r2 = make_float2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
             } else {
-                dx = A.xi - c.x; dy = A.yi - c.y; dz = A.zi - c.z;
+                const float2 dx = __fadd2_rn(make_float2(c0.x, c0.y), nx), dy = __fadd2_rn(make_float2(c0.z, c0.w), ny);
+                const float2 dz = __fadd2_rn(make_float2(c1.x, c1.y), nz);
+                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            if (r2 < fmaxf(A.h2, c.w * c.w)) {
-                qp[A.cnt * 32] = *gpp;
-                A.cnt++;
+            const float2 hj2 = __fmul2_rn(make_float2(c1.z, c1.w), make_float2(c1.z, c1.w));
+            if (r2.x < fmaxf(A.h2, hj2.x)) {
+                sts_u32(qw, lds_u32(ga));
+                qw += 128u;
             }
-            cp += f;
-            gpp += f;
+            if (r2.y < fmaxf(A.h2, hj2.y)) {
+                sts_u32(qw, lds_u32(ga + 4u));
+                qw += 128u;
+            }
+            ga += 8u * (uint32_t)f;
         }
+        A.cnt = (int)((qw - q0) >> 7);
     }
 }
 
 template <int KERNEL>
-__global__ void __launch_bounds__(SPH_THREADS, 3) k_force(ForceArgs a)
+__global__ void __launch_bounds__(SPH_THREADS, 4) k_force(ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -210,15 +246,16 @@ __global__ void __launch_bounds__(SPH_THREADS, 3) k_force(ForceArgs a)
             WalkCtl ctl;
             ctl.sp = -1;
             unsigned long long cands = 0;
-            bool anywrap = false;
+            Frame fr;
+            fr.thx = fr.thy = fr.thz = __int_as_float(0x7f800000);
+            fr.pairwrap = false;
             do {
                 walk_batch<true>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
                 cands += ctl.total;
                 // queued hits of an earlier batch are evaluated in the frame they were found in
-                if (ctl.pairwrap != anywrap) {
-                    const int mxq = __reduce_max_sync(FULLMASK, A.cnt);
-                    if (anywrap) drain<KERNEL, true>(a, qp, A, mxq); else drain<KERNEL, false>(a, qp, A, mxq);
-                    anywrap = ctl.pairwrap;
+                if (ctl.pairwrap != fr.pairwrap || ctl.thx != fr.thx || ctl.thy != fr.thy || ctl.thz != fr.thz) {
+                    drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+                    fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
                 }
                 const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
                 rc.kseg = 0;
@@ -228,20 +265,13 @@ __global__ void __launch_bounds__(SPH_THREADS, 3) k_force(ForceArgs a)
                     if (nf < nch) { ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf, W.gidx); nf++; }
                     const uint32_t slot = ring_wait<1>(rc, W.bars);
                     float4 *slotp = W.ring + slot * SPH_CH;
-                    const uint32_t nval = min((uint32_t)SPH_CH, ctl.total - c * SPH_CH);
-                    if (nval < SPH_CH) {
-                        for (uint32_t j = nval + lane; j < SPH_CH; j += 32) slotp[j] = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
-                        fence_proxy_async();
-                    }
-                    __syncwarp(); // gidx of this slot (written by the filling lanes) is visible to all
-                    if (anywrap) consume_chunk<KERNEL, true>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live);
-                    else consume_chunk<KERNEL, false>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live);
+                    // (the __syncwarp inside also makes this slot's gidx, written by the filling lanes, visible)
+                    slot_prepare(slotp, min((uint32_t)SPH_CH, ctl.total - c * SPH_CH), ctl, L);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live, fr);
                 }
             } while (ctl.sp > 0);
-            {
-                const int mxq = __reduce_max_sync(FULLMASK, A.cnt);
-                if (anywrap) drain<KERNEL, true>(a, qp, A, mxq); else drain<KERNEL, false>(a, qp, A, mxq);
-            }
+            drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
             // cross-stream totals
             double X = (double)A.px, Y = (double)A.py, Z = (double)A.pz, U = (double)A.pdu;
             float V = A.pvs;

@@ -49,6 +49,22 @@ __device__ __forceinline__ float warp_min(float v)
 // mbarrier / bulk-copy primitives (sm_90+; SASS: SYNCS.*, UBLKCP)
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+__device__ __forceinline__ void sts_f32(uint32_t addr, float v)
+{
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -96,8 +112,14 @@ struct WalkCtl { // warp-uniform registers
     int sp;        // stack pointer; -1: walk not started
     int n_seg;
     uint32_t total;
-    bool pairwrap; // per-pair nearest image needed for this batch
+    // Frame of this batch (see the end of walk_batch): per axis, coordinates >= thr are shifted by -L
+    // (thr = +inf: axis untouched); pairwrap: per-pair nearest image needed instead.
+    float thx, thy, thz;
+    bool pairwrap;
 };
+
+// coordinate in the batch's frame: exact (x - L is exact for x >= L/2, Sterbenz)
+__device__ __forceinline__ float recentre(float x, float thr, float L) { return x >= thr ? x - L : x; }
 
 __device__ __forceinline__ SphNode load_node(const SphNode *__restrict__ nodes, uint32_t i)
 {
@@ -195,13 +217,23 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
     ctl.sp = sp;
     ctl.n_seg = n_seg;
     ctl.total = carry;
-    // Frame choice.  If the group, its reach and every candidate cell stay clear of the box faces,
-    // plain differences of raw coordinates ARE the minimum-image differences; otherwise (a group next
-    // to a face, or a reach comparable to the box) every pair takes the nearest image explicitly.
-    float ext = maxreach * (1.f + 1e-5f) + 2.f * maxhalf + 4.f * pad;
-    bool inside = gcx - ghx - ext >= 0.f && gcx + ghx + ext < L && gcy - ghy - ext >= 0.f && gcy + ghy + ext < L &&
-                  gcz - ghz - ext >= 0.f && gcz + ghz + ext < L;
-    ctl.pairwrap = !inside;
+    // Frame choice, per axis.  ext bounds how far any candidate of this batch can lie from the group's
+    // bounding box.  (i) The group, its reach and every candidate cell stay clear of both box faces:
+    // plain differences of raw coordinates ARE the minimum-image differences (thr = +inf).  (ii) They
+    // cross a face but span less than half the box: map every coordinate x >= L/2 to x - L (exact), for
+    // actives and candidates alike; all of them then lie in one interval inside (-L/2, L/2) and plain differences are
+    // again the minimum-image differences, while a candidate outside that span can only look farther
+    // away than it is, never closer.  (iii) Otherwise (a reach comparable to the box): per-pair image.
+    const float inf = __int_as_float(0x7f800000);
+    const float ext = maxreach * (1.f + 1e-5f) + 2.f * maxhalf + 4.f * pad;
+    const float hl = 0.5f * L, ql = 0.249f * L; // span = 2 (gh + ext) < L/2
+    const bool okx = gcx - ghx - ext >= 0.f && gcx + ghx + ext < L;
+    const bool oky = gcy - ghy - ext >= 0.f && gcy + ghy + ext < L;
+    const bool okz = gcz - ghz - ext >= 0.f && gcz + ghz + ext < L;
+    ctl.thx = okx ? inf : hl;
+    ctl.thy = oky ? inf : hl;
+    ctl.thz = okz ? inf : hl;
+    ctl.pairwrap = (!okx && ghx + ext >= ql) || (!oky && ghy + ext >= ql) || (!okz && ghz + ext >= ql);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -224,7 +256,8 @@ __device__ __forceinline__ void ring_fill(const WarpWalk &ws, const WalkCtl &ctl
     const uint32_t lo = chunk * SPH_CH, hi = min(lo + SPH_CH, ctl.total);
     const uint32_t slot = rc.nfill % SPH_NSLOT;
     uint64_t *bar = bars + slot;
-    __syncwarp(); // every lane is done reading the slot's previous contents
+    fence_proxy_async(); // the lanes' generic-proxy writes to the slot (slot_prepare) precede the bulk copies
+    __syncwarp();        // every lane is done reading the slot's previous contents
     if (lane == 0) mbar_expect_tx(bar, (hi - lo) * 16u * NARR);
     int k0 = rc.kseg;
     for (;;) {
@@ -260,12 +293,34 @@ __device__ __forceinline__ uint32_t ring_wait(RingCtl<NARR> &rc, uint64_t *bars)
     return slot;
 }
 
-// Lane layout of a group of n_u actives: lane = a + g * s with a < g = n_u the active and s < f the
-// candidate stream; f is the largest divisor of SPH_CH with g * f <= 32, so that every chunk splits
-// evenly over the streams.
+// After a chunk has landed: bring the slot into the layout the test loops read.  Candidates 2p and 2p+1
+// (two float4 (x,y,z,w)) become the pair records (x0,x1,y0,y1), (z0,z1,w0,w1) in the same 32 bytes, so
+// that a lane loads register pairs ready for packed f32x2 arithmetic; coordinates move into the batch's
+// frame (recentre); entries beyond the ragged tail become NaN (every comparison with NaN is false).
+__device__ __forceinline__ void slot_prepare(float4 *slotp, uint32_t nval, const WalkCtl &ctl, float L)
+{
+    const int lane = threadIdx.x & 31;
+    const float thx = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thx;
+    const float thy = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thy;
+    const float thz = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thz;
+#pragma unroll
+    for (int p = lane; p < SPH_CH / 2; p += 32) {
+        float4 c0 = slotp[2 * p], c1 = slotp[2 * p + 1];
+        if (2u * p >= nval) c0 = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
+        if (2u * p + 1u >= nval) c1 = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
+        slotp[2 * p] = make_float4(recentre(c0.x, thx, L), recentre(c1.x, thx, L), recentre(c0.y, thy, L),
+                                   recentre(c1.y, thy, L));
+        slotp[2 * p + 1] = make_float4(recentre(c0.z, thz, L), recentre(c1.z, thz, L), c0.w, c1.w);
+    }
+    __syncwarp();
+}
+
+// Lane layout of a group of g actives: lane = a + g * s with a < g the active and s < f the candidate
+// stream; f is the largest divisor of SPH_CH / 2 (candidate pairs per chunk) with g * f <= 32, so that
+// every chunk splits evenly over the streams.
 __device__ __forceinline__ int streams_for(int g)
 {
     int f = 32 / g;
-    while (SPH_CH % f) f--;
+    while ((SPH_CH / 2) % f) f--;
     return f;
 }
