@@ -194,6 +194,8 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--group-cap", type=int, default=0, help="actives per group (0 = library default)")
+    ap.add_argument("--group-node", type=int, default=0, help="group-node capacity (0 = library default)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -226,7 +228,7 @@ def main():
     ngb = torch.zeros(n, device="cuda", dtype=torch.int32)
     acc = torch.zeros((n, 3), device="cuda")
     stream = torch.cuda.current_stream()
-    sph = B.Sph(kernel=ps.kernel, stream=stream)
+    sph = B.Sph(kernel=ps.kernel, stream=stream, group_cap=args.group_cap, group_node=args.group_node)
     n_active = n if active is None else int(active.numel())
     flush = None if n * 76 > 126e6 else torch.empty(64 << 20, device="cuda", dtype=torch.float32)
 
@@ -298,7 +300,7 @@ def main():
         hacc = pin(np.zeros((n, 3), np.float32))
         hact = None if active_np is None else pin(active_np)
         hg_pin = pin(hg_np)
-        sph2 = B.Sph(kernel=ps.kernel, stream=stream)
+        sph2 = B.Sph(kernel=ps.kernel, stream=stream, group_cap=args.group_cap, group_node=args.group_node)
         tt = []
         for k in range(1 + args.steps):
             hh.copy_(hg_pin)

@@ -63,7 +63,9 @@ typedef struct {
     float alpha_visc;  /* artificial viscosity alpha (1.0), R9 */
     int count_mode;    /* 0: kernel-weighted neighbour number drives the h iteration, 1: integer count (R2) */
     int max_iter;      /* cap on evaluations per particle (64); 1..255 */
-    int group_cap;     /* max active particles per group (one warp per group); 0 = default (8); <= 32 */
+    int group_cap;     /* max active particles per group (one warp per group); 0 = default; <= 32 */
+    int group_node;    /* groups are cut from the highest octree nodes holding <= this many particles;
+                          0 = default (2 * group_cap); raised to the leaf capacity (32) if smaller */
 } sph_params;
 
 typedef struct {

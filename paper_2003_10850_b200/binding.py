@@ -24,7 +24,7 @@ EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_h
 
 class SphParams(C.Structure):
     _fields_ = [("kernel", C.c_int), ("box", C.c_float), ("gamma", C.c_float), ("alpha_visc", C.c_float),
-                ("count_mode", C.c_int), ("max_iter", C.c_int), ("group_cap", C.c_int)]
+                ("count_mode", C.c_int), ("max_iter", C.c_int), ("group_cap", C.c_int), ("group_node", C.c_int)]
 
 
 class SphStats(C.Structure):
@@ -93,11 +93,11 @@ class Sph:
     """One libsph context (sph_create ... sph_destroy) bound to a torch CUDA stream."""
 
     def __init__(self, kernel=KERNEL_CUBIC, box=1.0, gamma=5.0 / 3.0, alpha_visc=1.0, count_mode=0, max_iter=64,
-                 group_cap=0, stream: "torch.cuda.Stream | None" = None):
+                 group_cap=0, group_node=0, stream: "torch.cuda.Stream | None" = None):
         self._lib = load()
         self._h = C.c_void_p()
         self.stream = stream if stream is not None else torch.cuda.current_stream()
-        p = SphParams(kernel, box, gamma, alpha_visc, count_mode, max_iter, group_cap)
+        p = SphParams(kernel, box, gamma, alpha_visc, count_mode, max_iter, group_cap, group_node)
         rc = self._lib.sph_create(C.byref(self._h), C.byref(p), C.c_void_p(self.stream.cuda_stream))
         if rc != SPH_OK:
             self._h = C.c_void_p()

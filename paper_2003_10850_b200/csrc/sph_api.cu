@@ -47,7 +47,7 @@ int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream)
     *out = nullptr;
     if (p->kernel != SPH_KERNEL_CUBIC && p->kernel != SPH_KERNEL_WC6) return SPH_E_ARG;
     if (!(p->box > 0.f) || !(p->gamma > 1.f) || !(p->alpha_visc >= 0.f)) return SPH_E_ARG;
-    if (p->max_iter < 1 || p->max_iter > 255 || p->group_cap < 0 || p->group_cap > SPH_MAXB) return SPH_E_ARG;
+    if (p->max_iter < 1 || p->max_iter > 255 || p->group_cap < 0 || p->group_cap > SPH_MAXB || p->group_node < 0) return SPH_E_ARG;
     if (p->count_mode != 0 && p->count_mode != 1) return SPH_E_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -58,6 +58,7 @@ int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream)
     if (!ctx) return SPH_E_OOM;
     ctx->prm = *p;
     ctx->grp_cap = p->group_cap ? p->group_cap : SPH_GCAP_DEFAULT;
+    ctx->grp_node = p->group_node > 0 ? p->group_node : 2 * ctx->grp_cap;
     ctx->stream = (cudaStream_t)cuda_stream;
     int dev = 0;
     cudaDeviceProp prop;

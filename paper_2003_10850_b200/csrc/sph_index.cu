@@ -123,15 +123,18 @@ __global__ void k_tree_split(SphCounters *cnt, SphNode *nodes, const uint64_t *_
     }
 }
 
-// a5 (all-active case): every leaf is cut into ceil(count / grp_cap) balanced runs of consecutive
-// sorted slots; a run is a group (consecutive Morton order keeps a run spatially compact)
+// a5 (all-active case): the group nodes are the highest octree nodes that hold <= node_cap particles
+// (a leaf that holds more, e.g. coincident particles, is its own group node); every group node is cut
+// into ceil(count / grp_cap) balanced runs of consecutive sorted slots; a run is a group (consecutive
+// Morton order inside a small cell keeps a run spatially compact)
 __global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict__ nodes, uint32_t grp_cap,
-                              uint32_t *__restrict__ mark)
+                              uint32_t node_cap, uint32_t *__restrict__ mark)
 {
     uint32_t nn = cnt->n_nodes;
     for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) {
         SphNode p = nodes[nd];
-        if (p.child != 0 || p.count == 0) continue;
+        if (p.count == 0 || (p.count > node_cap && p.child != 0)) continue;
+        if (nd != 0 && nodes[p.parent].count <= node_cap) continue; // an ancestor is the group node
         const uint32_t ns = (p.count + grp_cap - 1) / grp_cap;
         for (uint32_t s = 0; s < ns; s++) mark[p.start + (uint32_t)(((uint64_t)s * p.count) / ns)] = 1u;
     }
@@ -247,7 +250,8 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     }
     // a5: group starts in sorted order + group id of every slot
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->grp_mark, 0, sizeof(uint32_t) * n, st));
-    k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)ctx->grp_cap, ctx->grp_mark);
+    k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)ctx->grp_cap,
+                                        (uint32_t)(ctx->grp_node > SPH_LEAF ? ctx->grp_node : SPH_LEAF), ctx->grp_mark);
     ctx->launches++;
     tbs = ctx->cub_tmp_bytes;
     SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),

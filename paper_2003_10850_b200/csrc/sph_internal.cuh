@@ -64,6 +64,7 @@ struct sph_ctx {
     bool has_mass;
     float mass_scalar;
     int grp_cap;      // max actives per group
+    int grp_node;     // groups are cut from the highest octree nodes holding <= this many particles
 
     // index (device)
     uint64_t *keys, *keys_alt;

@@ -181,16 +181,30 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
         bool pass = valid && nd.count > 0 && d2 <= rp * rp;
         bool leaf = nd.child == 0;
         bool emit = pass && leaf, push = pass && !leaf;
-        unsigned me = __ballot_sync(FULLMASK, emit);
+        // Sibling leaves are consecutive runs of the sorted order: a run of emitted siblings (empty ones
+        // in between do not matter) becomes ONE segment, emitted by the run's first lane.
+        const unsigned me = __ballot_sync(FULLMASK, emit);
+        const unsigned mbrk = __ballot_sync(FULLMASK, valid && nd.count > 0 && !emit);
+        const unsigned blk = 0xffu << (lane & 24);                 // the 8 lanes of this lane's sibling block
+        const unsigned below = blk & lanemask_lt(), above = blk & ~lanemask_lt() & ~(1u << lane);
+        const unsigned prevs = (me | mbrk) & below;                 // non-empty siblings before this one
+        const bool head = emit && (prevs == 0u || ((mbrk >> (31 - __clz(prevs))) & 1u));
+        const unsigned nb = mbrk & above;                           // first break after this lane ends the run
+        const unsigned runm = me & (above | (1u << lane)) & (nb ? ((1u << (__ffs(nb) - 1)) - 1u) : 0xffffffffu);
+        const int last = 31 - __clz(runm | (1u << lane));           // last emitted sibling of the run
+        const uint32_t endpos = __shfl_sync(FULLMASK, nd.start + nd.count, last);
+        const unsigned mh = __ballot_sync(FULLMASK, head);
         if (emit) {
-            int p = n_seg + __popc(me & lanemask_lt());
-            SPH_ASSERT(p < SPH_SMAX);
-            ws.seg_start[p] = nd.start;
-            ws.seg_pre[p] = nd.count;
             maxhalf = fmaxf(maxhalf, nd.half);
             maxreach = fmaxf(maxreach, reach);
         }
-        n_seg += __popc(me);
+        if (head) {
+            int p = n_seg + __popc(mh & lanemask_lt());
+            SPH_ASSERT(p < SPH_SMAX);
+            ws.seg_start[p] = nd.start;
+            ws.seg_pre[p] = endpos - nd.start;
+        }
+        n_seg += __popc(mh);
         unsigned mp = __ballot_sync(FULLMASK, push);
         SPH_ASSERT(sp + __popc(mp) <= SPH_STK);
         if (push) ws.stack[sp + __popc(mp & lanemask_lt())] = nd.child;

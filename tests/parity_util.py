@@ -23,10 +23,10 @@ def dev(a, dtype=None):
 class GpuRun:
     """One context + device arrays for a ParticleSet-like input."""
 
-    def __init__(self, pos, kernel, mass_scalar, box=1.0, mass=None, count_mode=0, max_iter=64, alpha=1.0, group_cap=0):
+    def __init__(self, pos, kernel, mass_scalar, box=1.0, mass=None, count_mode=0, max_iter=64, alpha=1.0, group_cap=0, group_node=0):
         self.n = pos.shape[0]
         self.sph = B.Sph(kernel=kernel, box=box, count_mode=count_mode, max_iter=max_iter, alpha_visc=alpha,
-                         group_cap=group_cap)
+                         group_cap=group_cap, group_node=group_node)
         self.pos = dev(pos, torch.float32)
         self.mass = None if mass is None else dev(mass, torch.float32)
         self.sph.sph_build_index(self.pos, self.mass, mass_scalar)
