@@ -78,11 +78,11 @@ __device__ __forceinline__ void kern_wd2(float2 u, float2 &w, float2 &d)
 // per-warp shared memory
 template <bool HAS_MASS>
 struct DensWarp {
-    float4 ring[SPH_NSLOT * SPH_CH];
+    float4 slot[SPH_CH];                     // one chunk of candidates as pair records
+    alignas(16) uint32_t head[128];                      // gather scratch (segment heads of the chunk)
     WarpWalk ws;
     float q[SPH_QCAP * 32];                  // hit queue: entry k of lane l at [k * 32 + l] (r^2)
     float qm[HAS_MASS ? SPH_QCAP * 32 : 32]; // mass of the hit
-    uint64_t bars[SPH_NSLOT];
     double lo[SPH_MAXB], hi[SPH_MAXB];       // bracket of the h iteration (R7)
     float ax[SPH_MAXB], ay[SPH_MAXB], az[SPH_MAXB], aH[SPH_MAXB];
     uint32_t aid[SPH_MAXB];
@@ -90,98 +90,116 @@ struct DensWarp {
     int ulist[SPH_MAXB];                     // actives still iterating
 };
 
-// per-lane accumulators of one evaluation (packed: two partial sums each)
-struct DensAcc {
-    float2 s, ds, r, dr; // sum w, sum d, sum m w, sum m d
-    int cn, cnt;         // hits evaluated so far / hits waiting in the queue
+// per-lane state of one evaluation: lane (a, s) = active a, candidate stream s
+struct DensLane {
+    float2 s, ds, r, dr; // packed partial sums: sum w, sum d, sum m w, sum m d
+    float2 nx, ny, nz;   // minus the active's position in the batch's frame, duplicated for f32x2
+    float xi, yi, zi;    // raw position (per-pair image path)
+    float h2, ih2;       // H^2 (-1 in dead lanes: never hit), 1 / H^2
+    uint32_t q0, qw;     // hit queue of this lane: base and write cursor (shared-memory addresses, stride 128 B)
+    uint32_t mofs;       // offset from a queue entry to its mass entry
+    uint32_t ca;         // shared-memory address of this stream's first pair record of the chunk
+    uint32_t cstride;    // bytes between consecutive pair records of this stream (32 f)
+    int steps;           // pair records per chunk for this stream (SPH_CH / 2 / f)
+    int cn;              // hits evaluated so far
 };
 
-// evaluate the m newest queued hits of every lane, two per step (n = warp-wide maximum of m)
-template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void drain(const float *__restrict__ qp, const float *__restrict__ qmp, DensAcc &A, int n,
-                                      float ih2)
+__device__ __forceinline__ float lds_f32(uint32_t addr)
 {
-    const int m = min(n, A.cnt), base = A.cnt - m;
-    const float2 ih22 = f2(ih2);
-#pragma unroll 2
-    for (int k = 0; k < n; k += 2) {
-        if (k < m) {
-            const bool two = k + 1 < m;
-            const float r0 = qp[(base + k) * 32], r1 = two ? qp[(base + k + 1) * 32] : 0.f;
-            float2 u = __fmul2_rn(f2(r0, r1), ih22);
-            if (!two) u.y = 1.f; // odd tail: w = d = 0
-            float2 w, d;
-            kern_wd2<KERNEL>(u, w, d);
-            A.s = __fadd2_rn(A.s, w);
-            A.ds = __fadd2_rn(A.ds, d);
-            if (HAS_MASS) {
-                const float2 mj = f2(qmp[(base + k) * 32], two ? qmp[(base + k + 1) * 32] : 0.f);
-                A.r = __ffma2_rn(mj, w, A.r);
-                A.dr = __ffma2_rn(mj, d, A.dr);
-            }
-        }
-    }
-    A.cn += m;
-    A.cnt = base;
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+    return v;
 }
 
-// Test the candidates of one prepared ring slot against this lane's active: lane (a, s) takes the
-// candidate pairs s, s + f, s + 2f, ... of the chunk; both distances of a pair come out of one packed
-// f32x2 chain; a hit pushes r^2 (and the mass) onto the lane's queue.
-template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
-__device__ __forceinline__ void consume_chunk(const float4 *__restrict__ slotp, float *__restrict__ qp,
-                                              float *__restrict__ qmp, DensAcc &A, int s, int f, bool live, float xi,
-                                              float yi, float zi, float h2, float ih2, float L)
+// Evaluate the newest min(n, queued) hits of every lane, two per step, without branches: a lane that
+// runs out of entries evaluates u = 1, where w = d = 0 exactly (n is warp-uniform).
+template <int KERNEL, bool HAS_MASS>
+__device__ __forceinline__ void drain(DensLane &A, int n)
 {
-    const int steps = (SPH_CH / 2) / f;
-    const float4 *cp = slotp + 2 * s;
-    const float2 nx = f2(-xi), ny = f2(-yi), nz = f2(-zi);
-    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
-        const int nt = min(SPH_QSTEP, steps - t0);
-        // queue capacity: room for 2 nt more hits in every lane, else evaluate queued hits first
-        const int mx = __reduce_max_sync(FULLMASK, A.cnt);
-        if (mx + 2 * nt > SPH_QCAP) {
-            const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, HAS_MASS>(qp, qmp, A, max(mn, mx + 2 * nt - SPH_QCAP), ih2);
-        }
-        // queue write cursor as a 32-bit shared-memory address (one STS + one add per hit)
-        const uint32_t q0 = smem_u32(qp);
-        uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
-        const uint32_t mofs = HAS_MASS ? smem_u32(qmp) - q0 : 0u;
+    const int m = min(n, (int)((A.qw - A.q0) >> 7));
+    const uint32_t end = A.qw;
+    uint32_t ra = end - (uint32_t)m * 128u;
+    A.qw = ra;
+    A.cn += m;
+    const float2 ih22 = f2(A.ih2);
 #pragma unroll 2
+    for (int k = 0; k < n; k += 2, ra += 256u) {
+        const bool v0 = ra < end, v1 = ra + 128u < end;
+        const float r0 = v0 ? lds_f32(ra) : 0.f, r1 = v1 ? lds_f32(ra + 128u) : 0.f;
+        float2 u = __fmul2_rn(f2(r0, r1), ih22);
+        u.x = v0 ? u.x : 1.f;
+        u.y = v1 ? u.y : 1.f;
+        float2 w, d;
+        kern_wd2<KERNEL>(u, w, d);
+        A.s = __fadd2_rn(A.s, w);
+        A.ds = __fadd2_rn(A.ds, d);
+        if (HAS_MASS) {
+            const float2 mj = f2(v0 ? lds_f32(ra + A.mofs) : 0.f, v1 ? lds_f32(ra + 128u + A.mofs) : 0.f);
+            A.r = __ffma2_rn(mj, w, A.r);
+            A.dr = __ffma2_rn(mj, d, A.dr);
+        }
+    }
+}
+
+__device__ __forceinline__ void lds_pair(uint32_t addr, float4 &c0, float2 &c1, float2 &m)
+{
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(c0.x), "=f"(c0.y), "=f"(c0.z), "=f"(c0.w) : "r"(addr) : "memory");
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+16];" : "=f"(c1.x), "=f"(c1.y), "=f"(m.x), "=f"(m.y) : "r"(addr) : "memory");
+}
+
+// Test the candidates of the gathered chunk against this lane's active: lane (a, s) takes the pair
+// records s, s + f, s + 2f, ...; both distances of a pair come out of one packed f32x2 chain; a hit
+// pushes r^2 (and the mass) onto the lane's queue.
+template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
+__device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
+{
+    uint32_t ca = A.ca;
+    for (int t0 = 0; t0 < A.steps; t0 += SPH_QSTEP) {
+        const int nt = min(SPH_QSTEP, A.steps - t0);
+        // queue capacity: room for 2 nt more hits in every lane, else evaluate queued hits first
+        const int cnt = (int)((A.qw - A.q0) >> 7);
+        const int mx = __reduce_max_sync(FULLMASK, cnt);
+        if (mx + 2 * nt > SPH_QCAP) {
+            const int mn = __reduce_min_sync(FULLMASK, live ? cnt : 0x7fffffff);
+            drain<KERNEL, HAS_MASS>(A, max(mn, mx + 2 * nt - SPH_QCAP));
+        }
+        uint32_t qw = A.qw;
+#pragma unroll 3
         for (int t = 0; t < nt; t++) {
-            const float4 c0 = cp[0], c1 = cp[1]; // (x0,x1,y0,y1) (z0,z1,w0,w1)
-            cp += 2 * f;
+            float4 c0; // (x0,x1,y0,y1)
+            float2 c1, cm; // (z0,z1) (w0,w1)
+            lds_pair(ca, c0, c1, cm);
+            ca += A.cstride;
             float2 r2;
             if (PAIRWRAP) {
-                const float dx0 = image_diff(xi, c0.x, L), dx1 = image_diff(xi, c0.y, L);
-                const float dy0 = image_diff(yi, c0.z, L), dy1 = image_diff(yi, c0.w, L);
-                const float dz0 = image_diff(zi, c1.x, L), dz1 = image_diff(zi, c1.y, L);
+                const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);
+                const float dy0 = image_diff(A.yi, c0.z, L), dy1 = image_diff(A.yi, c0.w, L);
+                const float dz0 = image_diff(A.zi, c1.x, L), dz1 = image_diff(A.zi, c1.y, L);
                 r2 = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
             } else {
-                const float2 dx = __fadd2_rn(f2(c0.x, c0.y), nx), dy = __fadd2_rn(f2(c0.z, c0.w), ny);
-                const float2 dz = __fadd2_rn(f2(c1.x, c1.y), nz);
+                const float2 dx = __fadd2_rn(f2(c0.x, c0.y), A.nx), dy = __fadd2_rn(f2(c0.z, c0.w), A.ny);
+                const float2 dz = __fadd2_rn(c1, A.nz);
                 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
-            if (r2.x < h2) {
+            if (r2.x < A.h2) {
                 sts_f32(qw, r2.x);
-                if (HAS_MASS) sts_f32(qw + mofs, c1.z);
+                if (HAS_MASS) sts_f32(qw + A.mofs, cm.x);
                 qw += 128u;
             }
-            if (r2.y < h2) {
+            if (r2.y < A.h2) {
                 sts_f32(qw, r2.y);
-                if (HAS_MASS) sts_f32(qw + mofs, c1.w);
+                if (HAS_MASS) sts_f32(qw + A.mofs, cm.y);
                 qw += 128u;
             }
         }
-        A.cnt = (int)((qw - q0) >> 7);
+        A.qw = qw;
     }
 }
 
 // One evaluation of the group's iterating actives at their current H: walk, stream, test, evaluate.
 // Returns the cross-stream totals in the lanes of stream 0 (lane a < g).
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, RingCtl<1> &rc, int g, double &S,
+__device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, int g, double &S,
                                          double &D, double &R, double &DR, int &nint, unsigned long long &cands)
 {
     const int lane = threadIdx.x & 31;
@@ -191,8 +209,6 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     const int ai = live ? lane % g : 0, s = live ? lane / g : 0;
     const int k = W.ulist[ai];
     const float xi = W.ax[k], yi = W.ay[k], zi = W.az[k], H = W.aH[k];
-    const float h2 = live ? H * H : -1.f; // dead lanes never hit
-    const float ih2 = 1.f / (H * H);
     // bounding box and reach of the actives still iterating
     const float inf = __int_as_float(0x7f800000);
     float x0 = warp_min(live ? xi : inf), x1 = warp_max(live ? xi : -inf);
@@ -203,34 +219,36 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
     const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
 
-    DensAcc A;
+    DensLane A;
     A.s = A.ds = A.r = A.dr = f2(0.f);
-    A.cn = A.cnt = 0;
-    float *qp = W.q + lane, *qmp = W.qm + (HAS_MASS ? lane : 0);
-    const float4 *const src[1] = {a.xyzm};
+    A.cn = 0;
+    A.xi = xi; A.yi = yi; A.zi = zi;
+    A.h2 = live ? H * H : -1.f; // dead lanes never hit
+    A.ih2 = 1.f / (H * H);
+    A.q0 = A.qw = smem_u32(W.q + lane);
+    A.mofs = HAS_MASS ? smem_u32(W.qm + lane) - A.q0 : 0u;
+    A.ca = smem_u32(W.slot) + 32u * (uint32_t)s;
+    A.cstride = 32u * (uint32_t)f;
+    A.steps = (SPH_CH / 2) / f;
     WalkCtl ctl;
     ctl.sp = -1;
     do {
         walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
         cands += ctl.total;
         // this lane's active in the batch's frame
-        const float xf = ctl.pairwrap ? xi : recentre(xi, ctl.thx, L);
-        const float yf = ctl.pairwrap ? yi : recentre(yi, ctl.thy, L);
-        const float zf = ctl.pairwrap ? zi : recentre(zi, ctl.thz, L);
+        A.nx = f2(-(ctl.pairwrap ? xi : recentre(xi, ctl.thx, L)));
+        A.ny = f2(-(ctl.pairwrap ? yi : recentre(yi, ctl.thy, L)));
+        A.nz = f2(-(ctl.pairwrap ? zi : recentre(zi, ctl.thz, L)));
         const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
-        rc.kseg = 0;
-        uint32_t nf = 0;
-        for (; nf < nch && nf < SPH_NSLOT - 1; nf++) ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf);
+        GatherCtl gc;
+        gc.kseg = 0;
         for (uint32_t c = 0; c < nch; c++) {
-            if (nf < nch) { ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf); nf++; }
-            const uint32_t slot = ring_wait<1>(rc, W.bars);
-            float4 *slotp = W.ring + slot * SPH_CH;
-            slot_prepare(slotp, min((uint32_t)SPH_CH, ctl.total - c * SPH_CH), ctl, L);
-            if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(slotp, qp, qmp, A, s, f, live, xf, yf, zf, h2, ih2, L);
-            else consume_chunk<KERNEL, HAS_MASS, false>(slotp, qp, qmp, A, s, f, live, xf, yf, zf, h2, ih2, L);
+            gather_chunk(W.ws, ctl, gc, c, W.head, W.slot, nullptr, a.xyzm, L);
+            if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(A, live, L);
+            else consume_chunk<KERNEL, HAS_MASS, false>(A, live, L);
         }
     } while (ctl.sp > 0);
-    drain<KERNEL, HAS_MASS>(qp, qmp, A, __reduce_max_sync(FULLMASK, A.cnt), ih2);
+    drain<KERNEL, HAS_MASS>(A, __reduce_max_sync(FULLMASK, (int)((A.qw - A.q0) >> 7)));
 
     // cross-stream totals: lane a + g*s adds lane a + g*(s+d) for d = 1, 2, 4, ...
     S = (double)A.s.x + (double)A.s.y; D = (double)A.ds.x + (double)A.ds.y;
@@ -258,16 +276,6 @@ __global__ void __launch_bounds__(SPH_THREADS, 4) k_density(DensArgs a)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_evals = 0, st_cands = 0, st_pairs = 0; // meaningful in lane 0 only
     unsigned int st_unconv = 0;
-    RingCtl<1> rc;
-    rc.nfill = rc.ncons = 0;
-    rc.kseg = 0;
-    if (lane == 0) {
-        for (int i = 0; i < SPH_NSLOT; i++) mbar_init(&W.bars[i], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    fence_proxy_async();
-    __syncwarp();
-
     unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups (neighbouring groups share candidates in L1/L2)
     for (;;) {
         if (gnext == gend) {
@@ -301,7 +309,7 @@ __global__ void __launch_bounds__(SPH_THREADS, 4) k_density(DensArgs a)
             double S, D, R, DR;
             int nint;
             unsigned long long cands = 0;
-            evaluate<KERNEL, HAS_MASS>(W, a, rc, n_u, S, D, R, DR, nint, cands);
+            evaluate<KERNEL, HAS_MASS>(W, a, n_u, S, D, R, DR, nint, cands);
 
             // a8: safeguarded Newton update (R7), one lane per particle, fp64 scalars
             bool more = false, bad = false;

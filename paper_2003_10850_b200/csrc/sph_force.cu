@@ -47,11 +47,11 @@ __device__ __forceinline__ float kern_sigma()
 }
 
 struct ForceWarp {
-    float4 ring[SPH_NSLOT * SPH_CH];
+    float4 slot[SPH_CH];                // one chunk of candidates as pair records (x,y,z,H)
+    alignas(16) uint32_t head[128];                 // gather scratch
     WarpWalk ws;
     uint32_t q[SPH_QCAP * 32];          // hit queue: sorted slot of the neighbour
-    uint32_t gidx[SPH_NSLOT * SPH_CH];  // sorted slot of every candidate in the ring
-    uint64_t bars[SPH_NSLOT];
+    alignas(16) uint32_t gidx[SPH_CH];              // sorted slot of every candidate of the chunk
 };
 
 // per-lane state of the lane's active and its running sums
@@ -191,16 +191,6 @@ __global__ void __launch_bounds__(SPH_THREADS, 4) k_force(ForceArgs a)
     const float L = a.L;
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_cands = 0, st_pairs = 0;
-    RingCtl<1> rc;
-    rc.nfill = rc.ncons = 0;
-    rc.kseg = 0;
-    if (lane == 0) {
-        for (int i = 0; i < SPH_NSLOT; i++) mbar_init(&W.bars[i], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    fence_proxy_async();
-    __syncwarp();
-    const float4 *const src[1] = {a.xyzh};
     uint32_t *qp = W.q + lane;
 
     unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups
@@ -258,17 +248,12 @@ __global__ void __launch_bounds__(SPH_THREADS, 4) k_force(ForceArgs a)
                     fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
                 }
                 const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
-                rc.kseg = 0;
-                uint32_t nf = 0;
-                for (; nf < nch && nf < SPH_NSLOT - 1; nf++) ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf, W.gidx);
+                GatherCtl gc;
+                gc.kseg = 0;
                 for (uint32_t c = 0; c < nch; c++) {
-                    if (nf < nch) { ring_fill<1>(W.ws, ctl, rc, W.ring, W.bars, src, nf, W.gidx); nf++; }
-                    const uint32_t slot = ring_wait<1>(rc, W.bars);
-                    float4 *slotp = W.ring + slot * SPH_CH;
-                    // (the __syncwarp inside also makes this slot's gidx, written by the filling lanes, visible)
-                    slot_prepare(slotp, min((uint32_t)SPH_CH, ctl.total - c * SPH_CH), ctl, L);
-                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live, fr);
-                    else consume_chunk<KERNEL, false>(a, slotp, W.gidx + slot * SPH_CH, qp, A, s, f, live, fr);
+                    gather_chunk(W.ws, ctl, gc, c, W.head, W.slot, W.gidx, a.xyzh, L);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                 }
             } while (ctl.sp > 0);
             drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);

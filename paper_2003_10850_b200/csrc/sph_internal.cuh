@@ -24,10 +24,9 @@
 #define SPH_SMAX 128        // candidate segments per walk batch (per warp)
 #define SPH_STK 192         // walk stack entries (blocks of 8 sibling nodes, per warp)
 #define SPH_STK4 48         // 4-block pops only while the stack is at most this deep
-#define SPH_CH 120          // candidates per ring chunk (divisible by 1..6, 8, 10, 12, 15, 20, 24, 30)
-#define SPH_NSLOT 3         // ring slots per warp
-#define SPH_QCAP 40         // per-lane hit-queue entries
-#define SPH_QSTEP 8         // candidate-pair steps (2 tests each) between queue-capacity checks
+#define SPH_CH 120          // candidates per chunk (60 pairs: divisible by 1..6, 10, 12, 15, 20, 30)
+#define SPH_QCAP 48         // per-lane hit-queue entries
+#define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #define SPH_GBLOCK 4         // consecutive groups a warp takes per work-counter increment
 
 // octree node, 32 bytes, read as two 16-byte loads

@@ -1,11 +1,11 @@
 // sph_warp.cuh -- device code shared by the warp-per-group gather kernels (steps a5/a6):
-// per-warp octree walk that emits candidate leaf segments, and the per-warp shared-memory ring that
-// the candidate segments are streamed into by 1-D bulk copies (TMA, cp.async.bulk + mbarrier).
+// per-warp octree walk that emits candidate leaf segments, and the cooperative gather that stages a
+// chunk of candidates in the warp's shared-memory slot as pair records for packed f32x2 tests.
 //
 // One WARP owns one group of <= 32 active particles that are consecutive in the sorted order inside
 // one octree leaf -- the paper's "tree walk over groups of one or more active particles"
 // (§1).  Warps never synchronise with one another: walk latency of one group hides
-// behind the pair arithmetic of the others.  The ring chunk plays the role of the paper's N_chunk
+// behind the pair arithmetic of the others.  The chunk plays the role of the paper's N_chunk
 // (PAPER.md:104 §2.4, :108 §3): candidates are consumed in fixed-size chunks, not as whole lists.
 #pragma once
 
@@ -46,7 +46,7 @@ __device__ __forceinline__ float warp_min(float v)
 }
 
 // ---------------------------------------------------------------------------------------------
-// mbarrier / bulk-copy primitives (sm_90+; SASS: SYNCS.*, UBLKCP)
+// shared-memory primitives
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void sts_f32(uint32_t addr, float v)
@@ -63,41 +63,6 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
-}
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-// global -> shared 1-D bulk copy; bytes % 16 == 0, both addresses 16-byte aligned
-__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst_smem)),
-                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async()
-{
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -251,80 +216,100 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
 }
 
 // ---------------------------------------------------------------------------------------------
-// Candidate ring of one warp: SPH_NSLOT slots of SPH_CH candidates per streamed array.  A batch's
-// candidates form one flat index space [0, total) (segment k covers [seg_pre[k], seg_pre[k+1])); chunk c
-// = flat range [c*CH, c*CH+CH) lands in slot (nfill % NSLOT).  Each segment piece inside the chunk is
-// one bulk copy issued by one lane; the slot's mbarrier completes when all its bytes have arrived.
-template <int NARR>
-struct RingCtl { // warp-uniform registers
-    uint32_t nfill, ncons; // chunks filled / consumed since kernel start (slot + parity derive from them)
-    int kseg;              // first segment that overlaps the next chunk to fill
+// Candidate staging.  A batch's candidates form one flat index space [0, total) (segment k covers
+// [seg_pre[k], seg_pre[k+1])); chunk c = flat range [c*CH, c*CH+CH).  The warp gathers a chunk into its
+// shared-memory slot itself: lane l takes the four consecutive entries 4l..4l+3, finds their segments
+// (segment heads are marked in `head`, then a warp max-scan carries the latest head forward), loads the
+// four float4 records (one 64-byte run per lane unless a segment boundary intervenes), moves the
+// coordinates into the batch's frame (recentre) and writes them as PAIR records
+//   (x0,x1,y0,y1) (z0,z1,w0,w1)
+// so that the test loops load register pairs ready for packed f32x2 arithmetic.  Entries beyond the
+// ragged tail become NaN (every comparison with NaN is false).
+//
+// Why not TMA bulk copies here (they were the first design, profiles/r1c): octree leaves hold ~8
+// particles on average, so a chunk is ~10 pieces of ~100 bytes at arbitrary 16-byte offsets; every
+// piece is one UBLKCP issued through uniform registers, which the compiler serialises lane by lane
+// (ELECT / R2UR / UBLKCP, ~10 issue slots and a long-scoreboard wait per piece): 30 % of the kernel's
+// time went there.  Tiles this small and irregular are not TMA's case; per-lane 16-byte loads are.
+struct GatherCtl { // warp-uniform registers
+    int kseg; // first segment that overlaps the next chunk to gather
 };
 
-template <int NARR>
-__device__ __forceinline__ void ring_fill(const WarpWalk &ws, const WalkCtl &ctl, RingCtl<NARR> &rc, float4 *ring,
-                                          uint64_t *bars, const float4 *const (&src)[NARR], uint32_t chunk,
-                                          uint32_t *gidx = nullptr /* [NSLOT*CH]: sorted slot of every ring entry */)
+__device__ __forceinline__ float4 ldg_nc(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
+// head: [128] words of warp scratch; slotp: [SPH_CH] float4; gidx: [SPH_CH] sorted slot of every entry or NULL
+__device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &ctl, GatherCtl &gc, uint32_t chunk,
+                                             uint32_t *head, float4 *slotp, uint32_t *gidx,
+                                             const float4 *__restrict__ src, float L)
 {
     const int lane = threadIdx.x & 31;
     const uint32_t lo = chunk * SPH_CH, hi = min(lo + SPH_CH, ctl.total);
-    const uint32_t slot = rc.nfill % SPH_NSLOT;
-    uint64_t *bar = bars + slot;
-    fence_proxy_async(); // the lanes' generic-proxy writes to the slot (slot_prepare) precede the bulk copies
-    __syncwarp();        // every lane is done reading the slot's previous contents
-    if (lane == 0) mbar_expect_tx(bar, (hi - lo) * 16u * NARR);
-    int k0 = rc.kseg;
+    __syncwarp(); // every lane is done reading the slot's previous contents
+    reinterpret_cast<uint4 *>(head)[lane] = make_uint4(0u, 0u, 0u, 0u);
+    __syncwarp();
+    int k0 = gc.kseg;
     for (;;) {
-        int k = k0 + lane;
-        bool in = k < ctl.n_seg;
-        uint32_t p0 = in ? ws.seg_pre[k] : 0xffffffffu, p1 = in ? ws.seg_pre[k + 1] : 0xffffffffu;
-        uint32_t a = max(p0, lo), b = min(p1, hi);
-        if (in && a < b) {
-            const uint32_t g = ws.seg_start[k] + (a - p0);
-#pragma unroll
-            for (int r = 0; r < NARR; r++)
-                bulk_g2s(ring + (size_t)(r * SPH_NSLOT + slot) * SPH_CH + (a - lo), src[r] + g, (b - a) * 16u, bar);
-            if (gidx)
-                for (uint32_t e = 0; e < b - a; e++) gidx[slot * SPH_CH + (a - lo) + e] = g + e;
-        }
+        const int k = k0 + lane;
+        const bool in = k < ctl.n_seg;
+        const uint32_t p0 = in ? ws.seg_pre[k] : 0xffffffffu, p1 = in ? ws.seg_pre[k + 1] : 0xffffffffu;
+        if (in && p0 < hi && p1 > lo) head[max(p0, lo) - lo] = (uint32_t)k + 1u;
         // first segment of this window that reaches beyond the chunk = first segment of the next chunk
-        unsigned m = __ballot_sync(FULLMASK, in && p1 > hi);
+        const unsigned m = __ballot_sync(FULLMASK, in && p1 > hi);
         if (m) { k0 += __ffs(m) - 1; break; }
         k0 += 32;
         if (k0 >= ctl.n_seg) { k0 = ctl.n_seg; break; }
     }
-    rc.kseg = k0;
-    rc.nfill++;
-}
-
-// wait for the next chunk; returns its slot
-template <int NARR>
-__device__ __forceinline__ uint32_t ring_wait(RingCtl<NARR> &rc, uint64_t *bars)
-{
-    const uint32_t slot = rc.ncons % SPH_NSLOT, parity = (rc.ncons / SPH_NSLOT) & 1u;
-    mbar_wait(bars + slot, parity);
-    rc.ncons++;
-    return slot;
-}
-
-// After a chunk has landed: bring the slot into the layout the test loops read.  Candidates 2p and 2p+1
-// (two float4 (x,y,z,w)) become the pair records (x0,x1,y0,y1), (z0,z1,w0,w1) in the same 32 bytes, so
-// that a lane loads register pairs ready for packed f32x2 arithmetic; coordinates move into the batch's
-// frame (recentre); entries beyond the ragged tail become NaN (every comparison with NaN is false).
-__device__ __forceinline__ void slot_prepare(float4 *slotp, uint32_t nval, const WalkCtl &ctl, float L)
-{
-    const int lane = threadIdx.x & 31;
-    const float thx = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thx;
-    const float thy = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thy;
-    const float thz = ctl.pairwrap ? __int_as_float(0x7f800000) : ctl.thz;
+    gc.kseg = k0;
+    __syncwarp();
+    const uint4 h = reinterpret_cast<const uint4 *>(head)[lane];
+    // heads are segment numbers + 1 and grow with the position: the latest head is the largest
+    uint32_t sc = max(max(h.x, h.y), max(h.z, h.w));
 #pragma unroll
-    for (int p = lane; p < SPH_CH / 2; p += 32) {
-        float4 c0 = slotp[2 * p], c1 = slotp[2 * p + 1];
-        if (2u * p >= nval) c0 = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
-        if (2u * p + 1u >= nval) c1 = make_float4(SPH_NANF, SPH_NANF, SPH_NANF, 0.f);
-        slotp[2 * p] = make_float4(recentre(c0.x, thx, L), recentre(c1.x, thx, L), recentre(c0.y, thy, L),
-                                   recentre(c1.y, thy, L));
-        slotp[2 * p + 1] = make_float4(recentre(c0.z, thz, L), recentre(c1.z, thz, L), c0.w, c1.w);
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(FULLMASK, sc, o);
+        if (lane >= o) sc = max(sc, t);
+    }
+    uint32_t prev = __shfl_up_sync(FULLMASK, sc, 1);
+    if (lane == 0) prev = 0u;
+    if (lane < SPH_CH / 4) {
+        uint32_t kk[4];
+        kk[0] = max(h.x, prev); kk[1] = max(h.y, kk[0]); kk[2] = max(h.z, kk[1]); kk[3] = max(h.w, kk[2]);
+        float4 c[4];
+        uint32_t j[4];
+        const uint32_t p0 = lo + 4u * lane;
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+            // entries beyond the ragged tail re-read the last valid one and are turned into NaN below
+            const uint32_t p = min(p0 + i, hi - 1u);
+            const uint32_t k = max(kk[i], 1u) - 1u;
+            j[i] = ws.seg_start[k] + (p - ws.seg_pre[k]);
+            c[i] = ldg_nc(src + j[i]);
+        }
+        if (p0 + 3u >= hi) {
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                if (p0 + i >= hi) c[i].x = SPH_NANF;
+        }
+        const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // warp-uniform
+        if (rec) {
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                c[i].x = recentre(c[i].x, ctl.thx, L);
+                c[i].y = recentre(c[i].y, ctl.thy, L);
+                c[i].z = recentre(c[i].z, ctl.thz, L);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i += 2) {
+            slotp[4 * lane + i] = make_float4(c[i].x, c[i + 1].x, c[i].y, c[i + 1].y);
+            slotp[4 * lane + i + 1] = make_float4(c[i].z, c[i + 1].z, c[i].w, c[i + 1].w);
+        }
+        if (gidx) reinterpret_cast<uint4 *>(gidx)[lane] = make_uint4(j[0], j[1], j[2], j[3]);
     }
     __syncwarp();
 }
