@@ -79,7 +79,6 @@ __device__ __forceinline__ void kern_wd2(float2 u, float2 &w, float2 &d)
 template <bool HAS_MASS>
 struct DensWarp {
     float4 slot[SPH_CH];                     // one chunk of candidates as pair records
-    alignas(16) uint32_t head[128];                      // gather scratch (segment heads of the chunk)
     WarpWalk ws;
     float q[SPH_QCAP * 32];                  // hit queue: entry k of lane l at [k * 32 + l] (r^2)
     float qm[HAS_MASS ? SPH_QCAP * 32 : 32]; // mass of the hit
@@ -243,7 +242,7 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
         GatherCtl gc;
         gc.kseg = 0;
         for (uint32_t c = 0; c < nch; c++) {
-            gather_chunk(W.ws, ctl, gc, c, W.head, W.slot, nullptr, a.xyzm, L);
+            gather_chunk(W.ws, ctl, gc, c, W.slot, nullptr, a.xyzm, L);
             if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(A, live, L);
             else consume_chunk<KERNEL, HAS_MASS, false>(A, live, L);
         }

@@ -48,7 +48,6 @@ __device__ __forceinline__ float kern_sigma()
 
 struct ForceWarp {
     float4 slot[SPH_CH];                // one chunk of candidates as pair records (x,y,z,H)
-    alignas(16) uint32_t head[128];                 // gather scratch
     WarpWalk ws;
     uint32_t q[SPH_QCAP * 32];          // hit queue: sorted slot of the neighbour
     alignas(16) uint32_t gidx[SPH_CH];              // sorted slot of every candidate of the chunk
@@ -251,7 +250,7 @@ __global__ void __launch_bounds__(SPH_THREADS, 4) k_force(ForceArgs a)
                 GatherCtl gc;
                 gc.kseg = 0;
                 for (uint32_t c = 0; c < nch; c++) {
-                    gather_chunk(W.ws, ctl, gc, c, W.head, W.slot, W.gidx, a.xyzh, L);
+                    gather_chunk(W.ws, ctl, gc, c, W.slot, W.gidx, a.xyzh, L);
                     if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                     else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                 }

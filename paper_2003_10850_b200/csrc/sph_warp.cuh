@@ -219,7 +219,7 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
 // Candidate staging.  A batch's candidates form one flat index space [0, total) (segment k covers
 // [seg_pre[k], seg_pre[k+1])); chunk c = flat range [c*CH, c*CH+CH).  The warp gathers a chunk into its
 // shared-memory slot itself: lane l takes the four consecutive entries 4l..4l+3, finds their segments
-// (segment heads are marked in `head`, then a warp max-scan carries the latest head forward), loads the
+// (segment heads become bits of a warp-uniform mask; the rank of a position is a population count), loads the
 // four float4 records (one 64-byte run per lane unless a segment boundary intervenes), moves the
 // coordinates into the batch's frame (recentre) and writes them as PAIR records
 //   (x0,x1,y0,y1) (z0,z1,w0,w1)
@@ -242,22 +242,29 @@ __device__ __forceinline__ float4 ldg_nc(const float4 *p)
     return v;
 }
 
-// head: [128] words of warp scratch; slotp: [SPH_CH] float4; gidx: [SPH_CH] sorted slot of every entry or NULL
+// slotp: [SPH_CH] float4; gidx: [SPH_CH] sorted slot of every entry or NULL
 __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &ctl, GatherCtl &gc, uint32_t chunk,
-                                             uint32_t *head, float4 *slotp, uint32_t *gidx,
-                                             const float4 *__restrict__ src, float L)
+                                             float4 *slotp, uint32_t *gidx, const float4 *__restrict__ src, float L)
 {
     const int lane = threadIdx.x & 31;
     const uint32_t lo = chunk * SPH_CH, hi = min(lo + SPH_CH, ctl.total);
-    __syncwarp(); // every lane is done reading the slot's previous contents
-    reinterpret_cast<uint4 *>(head)[lane] = make_uint4(0u, 0u, 0u, 0u);
-    __syncwarp();
-    int k0 = gc.kseg;
+    // Bit p of the 128-bit mask (w0..w3) is set where a segment begins at chunk position p (the first
+    // overlapping segment counts as beginning at 0): the segment of position p is
+    // kfirst + (number of set bits at positions <= p) - 1.  One lane per segment sets its bit; the words
+    // are OR-reduced across the warp (REDUX), no shared memory and no scan.
+    const int kfirst = gc.kseg;
+    uint32_t w0 = 0u, w1 = 0u, w2 = 0u, w3 = 0u;
+    int k0 = kfirst;
     for (;;) {
         const int k = k0 + lane;
         const bool in = k < ctl.n_seg;
         const uint32_t p0 = in ? ws.seg_pre[k] : 0xffffffffu, p1 = in ? ws.seg_pre[k + 1] : 0xffffffffu;
-        if (in && p0 < hi && p1 > lo) head[max(p0, lo) - lo] = (uint32_t)k + 1u;
+        const bool ov = in && p0 < hi && p1 > lo;
+        const uint32_t pos = max(p0, lo) - lo, bit = ov ? 1u << (pos & 31u) : 0u, wd = pos >> 5;
+        w0 |= __reduce_or_sync(FULLMASK, wd == 0u ? bit : 0u);
+        w1 |= __reduce_or_sync(FULLMASK, wd == 1u ? bit : 0u);
+        w2 |= __reduce_or_sync(FULLMASK, wd == 2u ? bit : 0u);
+        w3 |= __reduce_or_sync(FULLMASK, wd == 3u ? bit : 0u);
         // first segment of this window that reaches beyond the chunk = first segment of the next chunk
         const unsigned m = __ballot_sync(FULLMASK, in && p1 > hi);
         if (m) { k0 += __ffs(m) - 1; break; }
@@ -265,20 +272,12 @@ __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &
         if (k0 >= ctl.n_seg) { k0 = ctl.n_seg; break; }
     }
     gc.kseg = k0;
-    __syncwarp();
-    const uint4 h = reinterpret_cast<const uint4 *>(head)[lane];
-    // heads are segment numbers + 1 and grow with the position: the latest head is the largest
-    uint32_t sc = max(max(h.x, h.y), max(h.z, h.w));
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(FULLMASK, sc, o);
-        if (lane >= o) sc = max(sc, t);
-    }
-    uint32_t prev = __shfl_up_sync(FULLMASK, sc, 1);
-    if (lane == 0) prev = 0u;
+    __syncwarp(); // every lane is done reading the slot's previous contents
     if (lane < SPH_CH / 4) {
-        uint32_t kk[4];
-        kk[0] = max(h.x, prev); kk[1] = max(h.y, kk[0]); kk[2] = max(h.z, kk[1]); kk[3] = max(h.w, kk[2]);
+        // this lane's entries 4 lane .. 4 lane + 3 lie in one mask word
+        const int wl = lane >> 3, sh = (4 * lane) & 31;
+        const uint32_t wmine = wl == 0 ? w0 : wl == 1 ? w1 : wl == 2 ? w2 : w3;
+        const int below = (wl > 0 ? __popc(w0) : 0) + (wl > 1 ? __popc(w1) : 0) + (wl > 2 ? __popc(w2) : 0);
         float4 c[4];
         uint32_t j[4];
         const uint32_t p0 = lo + 4u * lane;
@@ -286,7 +285,8 @@ __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &
         for (int i = 0; i < 4; i++) {
             // entries beyond the ragged tail re-read the last valid one and are turned into NaN below
             const uint32_t p = min(p0 + i, hi - 1u);
-            const uint32_t k = max(kk[i], 1u) - 1u;
+            const int k = kfirst + below + __popc(wmine & (0xffffffffu >> (31 - sh - i))) - 1;
+            SPH_ASSERT(k >= kfirst && k < ctl.n_seg);
             j[i] = ws.seg_start[k] + (p - ws.seg_pre[k]);
             c[i] = ldg_nc(src + j[i]);
         }
