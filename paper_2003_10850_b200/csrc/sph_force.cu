@@ -182,7 +182,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
 }
 
 template <int KERNEL>
-__global__ void __launch_bounds__(SPH_THREADS, 4) k_force(ForceArgs a)
+__global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

@@ -21,12 +21,19 @@
 #define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)
 #define SPH_WARPS 4         // warps per CTA of the gather kernels (warps are independent)
 #define SPH_THREADS (32 * SPH_WARPS)
+#ifndef SPH_CTAS
+#define SPH_CTAS 5          // resident CTAs per SM the gather kernels are compiled for (register budget)
+#endif
 #define SPH_SMAX 128        // candidate segments per walk batch (per warp)
 #define SPH_STK 192         // walk stack entries (blocks of 8 sibling nodes, per warp)
 #define SPH_STK4 48         // 4-block pops only while the stack is at most this deep
 #define SPH_CH 120          // candidates per chunk (60 pairs: divisible by 1..6, 10, 12, 15, 20, 30)
-#define SPH_QCAP 48         // per-lane hit-queue entries
+#ifndef SPH_QCAP
+#define SPH_QCAP 32         // per-lane hit-queue entries (>= 2 * SPH_QSTEP)
+#endif
+#ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
+#endif
 #define SPH_GBLOCK 4         // consecutive groups a warp takes per work-counter increment
 
 // octree node, 32 bytes, read as two 16-byte loads
