@@ -97,8 +97,8 @@ struct DensLane {
     float h2, ih2;       // H^2 (-1 in dead lanes: never hit), 1 / H^2
     uint32_t q0, qw;     // hit queue of this lane: base and write cursor (shared-memory addresses, stride 128 B)
     uint32_t mofs;       // offset from a queue entry to its mass entry
-    uint32_t ca;         // shared-memory address of this stream's first pair record of the chunk
-    uint32_t cstride;    // bytes between consecutive pair records of this stream (32 f)
+    const float4 *cp;    // this stream's first pair record of the chunk
+    int cstride;         // float4 elements between consecutive pair records of this stream (2 f)
     int steps;           // pair records per chunk for this stream (SPH_CH / 2 / f)
     int cn;              // hits evaluated so far
 };
@@ -140,19 +140,15 @@ __device__ __forceinline__ void drain(DensLane &A, int n)
     }
 }
 
-__device__ __forceinline__ void lds_pair(uint32_t addr, float4 &c0, float2 &c1, float2 &m)
-{
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(c0.x), "=f"(c0.y), "=f"(c0.z), "=f"(c0.w) : "r"(addr) : "memory");
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4+16];" : "=f"(c1.x), "=f"(c1.y), "=f"(m.x), "=f"(m.y) : "r"(addr) : "memory");
-}
-
 // Test the candidates of the gathered chunk against this lane's active: lane (a, s) takes the pair
 // records s, s + f, s + 2f, ...; both distances of a pair come out of one packed f32x2 chain; a hit
 // pushes r^2 (and the mass) onto the lane's queue.
 template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
 {
-    uint32_t ca = A.ca;
+    const float4 *cp = A.cp;
+    float4 n0 = cp[0], n1 = cp[1];
+    cp += A.cstride;
     for (int t0 = 0; t0 < A.steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, A.steps - t0);
         // queue capacity: room for 2 nt more hits in every lane, else evaluate queued hits first
@@ -165,10 +161,12 @@ __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
         uint32_t qw = A.qw;
 #pragma unroll 3
         for (int t = 0; t < nt; t++) {
-            float4 c0; // (x0,x1,y0,y1)
-            float2 c1, cm; // (z0,z1) (w0,w1)
-            lds_pair(ca, c0, c1, cm);
-            ca += A.cstride;
+            const float4 c0 = n0, cz = n1; // (x0,x1,y0,y1) (z0,z1,w0,w1)
+            const float2 c1 = f2(cz.x, cz.y), cm = f2(cz.z, cz.w);
+            // software pipeline: the next pair record is in flight while this one is tested (past the
+            // chunk's last record this reads on inside the warp's own shared memory; the value is unused)
+            n0 = cp[0]; n1 = cp[1];
+            cp += A.cstride;
             float2 r2;
             if (PAIRWRAP) {
                 const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);
@@ -226,8 +224,8 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     A.ih2 = 1.f / (H * H);
     A.q0 = A.qw = smem_u32(W.q + lane);
     A.mofs = HAS_MASS ? smem_u32(W.qm + lane) - A.q0 : 0u;
-    A.ca = smem_u32(W.slot) + 32u * (uint32_t)s;
-    A.cstride = 32u * (uint32_t)f;
+    A.cp = W.slot + 2 * s;
+    A.cstride = 2 * f;
     A.steps = (SPH_CH / 2) / f;
     WalkCtl ctl;
     ctl.sp = -1;

@@ -49,13 +49,17 @@ __device__ __forceinline__ float warp_min(float v)
 // shared-memory primitives
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// Hit-queue stores.  The queue of a lane is written and read by that lane only, through these asm
+// statements and the (volatile, memory-clobbering) queue loads of the drain loops, which stay ordered
+// after them; leaving the clobber off here lets the compiler hoist the next candidates' shared-memory
+// loads above the pushes of the previous test, so that the unrolled tests overlap.
 __device__ __forceinline__ void sts_f32(uint32_t addr, float v)
 {
-    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+    asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v)); // no memory clobber: see hit-queue note
 }
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v));
 }
 
 __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
@@ -235,10 +239,20 @@ struct GatherCtl { // warp-uniform registers
     int kseg; // first segment that overlaps the next chunk to gather
 };
 
+#ifndef SPH_LDG_MODE
+#define SPH_LDG_MODE 0
+#endif
+#if SPH_LDG_MODE == 0
+#define SPH_LDG_OP "ld.global.nc.v4.f32"
+#elif SPH_LDG_MODE == 1
+#define SPH_LDG_OP "ld.global.ca.v4.f32"
+#else
+#define SPH_LDG_OP "ld.global.cg.v4.f32"
+#endif
 __device__ __forceinline__ float4 ldg_nc(const float4 *p)
 {
     float4 v;
-    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    asm volatile(SPH_LDG_OP " {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
 }
 
