@@ -98,7 +98,7 @@ struct DensLane {
     uint32_t q0, qw;     // hit queue of this lane: base and write cursor (shared-memory addresses, stride 128 B)
     uint32_t mofs;       // offset from a queue entry to its mass entry
     const float4 *cp;    // this stream's first pair record of the chunk
-    int cstride;         // float4 elements between consecutive pair records of this stream (2 f)
+    int cstride;         // float4 elements between consecutive pair records of this stream (f)
     int steps;           // pair records per chunk for this stream (SPH_CH / 2 / f)
     int cn;              // hits evaluated so far
 };
@@ -147,7 +147,7 @@ template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
 {
     const float4 *cp = A.cp;
-    float4 n0 = cp[0], n1 = cp[1];
+    float4 n0 = cp[0], n1 = cp[SPH_CH / 2];
     cp += A.cstride;
     for (int t0 = 0; t0 < A.steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, A.steps - t0);
@@ -165,7 +165,7 @@ __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
             const float2 c1 = f2(cz.x, cz.y), cm = f2(cz.z, cz.w);
             // software pipeline: the next pair record is in flight while this one is tested (past the
             // chunk's last record this reads on inside the warp's own shared memory; the value is unused)
-            n0 = cp[0]; n1 = cp[1];
+            n0 = cp[0]; n1 = cp[SPH_CH / 2];
             cp += A.cstride;
             float2 r2;
             if (PAIRWRAP) {
@@ -224,8 +224,8 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     A.ih2 = 1.f / (H * H);
     A.q0 = A.qw = smem_u32(W.q + lane);
     A.mofs = HAS_MASS ? smem_u32(W.qm + lane) - A.q0 : 0u;
-    A.cp = W.slot + 2 * s;
-    A.cstride = 2 * f;
+    A.cp = W.slot + s;
+    A.cstride = f;
     A.steps = (SPH_CH / 2) / f;
     WalkCtl ctl;
     ctl.sp = -1;

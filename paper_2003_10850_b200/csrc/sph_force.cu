@@ -135,7 +135,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
                                               int s, int f, bool live, const Frame &fr)
 {
     const int steps = (SPH_CH / 2) / f;
-    const float4 *cp = slotp + 2 * s;
+    const float4 *cp = slotp + s;
     uint32_t ga = smem_u32(gp + 2 * s);
     const float L = a.L;
     const float xf = PAIRWRAP ? A.xi : recentre(A.xi, fr.thx, L);
@@ -153,8 +153,8 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
 #pragma unroll 2
         for (int t = 0; t < nt; t++) {
-            const float4 c0 = cp[0], c1 = cp[1]; // (x0,x1,y0,y1) (z0,z1,h0,h1)
-            cp += 2 * f;
+            const float4 c0 = cp[0], c1 = cp[SPH_CH / 2]; // (x0,x1,y0,y1) (z0,z1,h0,h1)
+            cp += f;
             float2 r2;
             if (PAIRWRAP) {
                 const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);

@@ -225,8 +225,8 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
 // shared-memory slot itself: lane l takes the four consecutive entries 4l..4l+3, finds their segments
 // (segment heads become bits of a warp-uniform mask; the rank of a position is a population count), loads the
 // four float4 records (one 64-byte run per lane unless a segment boundary intervenes), moves the
-// coordinates into the batch's frame (recentre) and writes them as PAIR records
-//   (x0,x1,y0,y1) (z0,z1,w0,w1)
+// coordinates into the batch's frame (recentre) and writes them as PAIR records, pair p of the chunk =
+//   slot[p] = (x0,x1,y0,y1)   slot[SPH_CH/2 + p] = (z0,z1,w0,w1)
 // so that the test loops load register pairs ready for packed f32x2 arithmetic.  Entries beyond the
 // ragged tail become NaN (every comparison with NaN is false).
 //
@@ -287,43 +287,33 @@ __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &
     }
     gc.kseg = k0;
     __syncwarp(); // every lane is done reading the slot's previous contents
-    if (lane < SPH_CH / 4) {
-        // this lane's entries 4 lane .. 4 lane + 3 lie in one mask word
-        const int wl = lane >> 3, sh = (4 * lane) & 31;
-        const uint32_t wmine = wl == 0 ? w0 : wl == 1 ? w1 : wl == 2 ? w2 : w3;
-        const int below = (wl > 0 ? __popc(w0) : 0) + (wl > 1 ? __popc(w1) : 0) + (wl > 2 ? __popc(w2) : 0);
-        float4 c[4];
-        uint32_t j[4];
-        const uint32_t p0 = lo + 4u * lane;
+    const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // warp-uniform
+    // lane l takes the candidate pairs l and l + 32 (entries 2p, 2p + 1): 32 contiguous bytes per lane
+    // from global memory, 16 contiguous bytes per lane into each half of the slot (no bank conflicts)
 #pragma unroll
-        for (int i = 0; i < 4; i++) {
+    for (int r = 0; r < 2; r++) {
+        const int pr = lane + 32 * r;
+        if (pr < SPH_CH / 2) {
+            const int e0 = 2 * pr, wl = e0 >> 5, sh = e0 & 31; // both entries lie in mask word wl
+            const uint32_t wmine = wl == 0 ? w0 : wl == 1 ? w1 : wl == 2 ? w2 : w3;
+            const int below = kfirst - 1 + (wl > 0 ? __popc(w0) : 0) + (wl > 1 ? __popc(w1) : 0) + (wl > 2 ? __popc(w2) : 0);
+            const int ka = below + __popc(wmine & (0xffffffffu >> (31 - sh)));
+            const int kb = below + __popc(wmine & (0xffffffffu >> (30 - sh)));
+            SPH_ASSERT(ka >= kfirst && kb < ctl.n_seg);
             // entries beyond the ragged tail re-read the last valid one and are turned into NaN below
-            const uint32_t p = min(p0 + i, hi - 1u);
-            const int k = kfirst + below + __popc(wmine & (0xffffffffu >> (31 - sh - i))) - 1;
-            SPH_ASSERT(k >= kfirst && k < ctl.n_seg);
-            j[i] = ws.seg_start[k] + (p - ws.seg_pre[k]);
-            c[i] = ldg_nc(src + j[i]);
-        }
-        if (p0 + 3u >= hi) {
-#pragma unroll
-            for (int i = 0; i < 4; i++)
-                if (p0 + i >= hi) c[i].x = SPH_NANF;
-        }
-        const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // warp-uniform
-        if (rec) {
-#pragma unroll
-            for (int i = 0; i < 4; i++) {
-                c[i].x = recentre(c[i].x, ctl.thx, L);
-                c[i].y = recentre(c[i].y, ctl.thy, L);
-                c[i].z = recentre(c[i].z, ctl.thz, L);
+            const uint32_t pa = min(lo + e0, hi - 1u), pb = min(lo + e0 + 1u, hi - 1u);
+            const uint32_t ja = ws.seg_start[ka] + (pa - ws.seg_pre[ka]), jb = ws.seg_start[kb] + (pb - ws.seg_pre[kb]);
+            float4 ca = ldg_nc(src + ja), cb = ldg_nc(src + jb);
+            if (lo + e0 >= hi) ca.x = SPH_NANF;
+            if (lo + e0 + 1u >= hi) cb.x = SPH_NANF;
+            if (rec) {
+                ca.x = recentre(ca.x, ctl.thx, L); ca.y = recentre(ca.y, ctl.thy, L); ca.z = recentre(ca.z, ctl.thz, L);
+                cb.x = recentre(cb.x, ctl.thx, L); cb.y = recentre(cb.y, ctl.thy, L); cb.z = recentre(cb.z, ctl.thz, L);
             }
+            slotp[pr] = make_float4(ca.x, cb.x, ca.y, cb.y);
+            slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, ca.w, cb.w);
+            if (gidx) reinterpret_cast<uint2 *>(gidx)[pr] = make_uint2(ja, jb);
         }
-#pragma unroll
-        for (int i = 0; i < 4; i += 2) {
-            slotp[4 * lane + i] = make_float4(c[i].x, c[i + 1].x, c[i].y, c[i + 1].y);
-            slotp[4 * lane + i + 1] = make_float4(c[i].z, c[i + 1].z, c[i].w, c[i + 1].w);
-        }
-        if (gidx) reinterpret_cast<uint4 *>(gidx)[lane] = make_uint4(j[0], j[1], j[2], j[3]);
     }
     __syncwarp();
 }
