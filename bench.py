@@ -183,6 +183,23 @@ def workload_config(args, ps, active):
     }
 
 
+def max_over_ranks(x: float, world: int, device: str) -> float:
+    """Timing rule: every multi-rank number is the MAX over ranks (replicas: the slowest GPU sets the time)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, n_active: int, steps: int, ms: float) -> float:
+    """Whole-job throughput: every rank runs one replica of the workload (weak scaling, no exchange step)."""
+    return world * n_active * steps / (ms * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -282,11 +299,8 @@ def main():
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1) - t_flush
     launches = per[-1]["launches"] - l0
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * n_active * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, "cuda")
+    value = whole_job_value(world, n_active, args.steps, ms)
 
     # e2e: the same step through sph_step_host, pinned host buffers, copies inside the timed region
     e2e = None
@@ -309,10 +323,7 @@ def main():
             sph2.sph_step_host(hp, hv, hu, ps.mass, hh, hrho, hom, hngb, hacc, hdu, hvs, ps.n_ngb, ps.n_tol, active=hact)
             tt.append(time.perf_counter() - t0)
         t_e2e = sum(tt[1:])  # first call (allocations) is warm-up
-        if world > 1:
-            t = torch.tensor([t_e2e], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = max_over_ranks(t_e2e, world, "cuda")
         h2d = n * 32 + (0 if hact is None else 4 * len(active_np) + 8 * n)
         d2h = n * 44
         e2e = {"value": world * n_active * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
