@@ -32,7 +32,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
-    for d in os.environ.get("SPH_DEFS", "").split():  # development: e.g. SPH_DEFS="-DSPH_CTAS=4 -DSPH_QCAP=48"
+    for d in os.environ.get("SPH_DEFS", "").split():  # development: e.g. SPH_DEFS="-DSPH_CTAS=4 -DSPH_QCAP=48 -DSPH_LEAF=24 -DSPH_GBLOCK=2"
         cmd.insert(1, d)
     if os.environ.get("SPH_DEBUG"):  # device-side bounds asserts (development only)
         cmd.insert(1, "-DSPH_DEBUG=1")

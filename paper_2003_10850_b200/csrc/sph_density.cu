@@ -193,10 +193,18 @@ __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
     }
 }
 
+// what evaluate() keeps from one evaluation of a group to the next (warp-uniform registers)
+struct WalkCache {
+    WalkCtl ctl;
+    float hg;    // reach the list was walked with
+    bool valid;  // the list in shared memory is complete and reusable
+    bool multi;  // scratch: a batch of the current walk has already been seen
+};
+
 // One evaluation of the group's iterating actives at their current H: walk, stream, test, evaluate.
 // Returns the cross-stream totals in the lanes of stream 0 (lane a < g).
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, int g, double &S,
+__device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, int g, WalkCache &wc, double &S,
                                          double &D, double &R, double &DR, int &nint, unsigned long long &cands)
 {
     const int lane = threadIdx.x & 31;
@@ -227,10 +235,14 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     A.cp = W.slot + s;
     A.cstride = f;
     A.steps = (SPH_CH / 2) / f;
-    WalkCtl ctl;
-    ctl.sp = -1;
+    // The segment list of the group's previous evaluation is still in shared memory.  It stays valid if
+    // it was complete (one batch) and the reach has not grown: the actives still iterating are a subset
+    // (their bounding box lies inside the old one), so the old list and its frame cover this evaluation.
+    const bool reuse = wc.valid && hg <= wc.hg;
+    WalkCtl ctl = wc.ctl;
+    if (!reuse) ctl.sp = -1;
     do {
-        walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
+        if (!reuse) walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
         cands += ctl.total;
         // this lane's active in the batch's frame
         A.nx = f2(-(ctl.pairwrap ? xi : recentre(xi, ctl.thx, L)));
@@ -243,6 +255,12 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
             gather_chunk(W.ws, ctl, gc, c, W.slot, nullptr, a.xyzm, L);
             if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(A, live, L);
             else consume_chunk<KERNEL, HAS_MASS, false>(A, live, L);
+        }
+        if (!reuse) {
+            wc.valid = !wc.multi && ctl.sp <= 0; // complete in its first batch
+            wc.multi = true;
+            wc.hg = hg;
+            wc.ctl = ctl;
         }
     } while (ctl.sp > 0);
     drain<KERNEL, HAS_MASS>(A, __reduce_max_sync(FULLMASK, (int)((A.qw - A.q0) >> 7)));
@@ -302,11 +320,14 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
         }
         __syncwarp();
         int n_u = na;
+        WalkCache wc;
+        wc.valid = false;
         while (n_u > 0) {
+            wc.multi = false;
             double S, D, R, DR;
             int nint;
             unsigned long long cands = 0;
-            evaluate<KERNEL, HAS_MASS>(W, a, n_u, S, D, R, DR, nint, cands);
+            evaluate<KERNEL, HAS_MASS>(W, a, n_u, wc, S, D, R, DR, nint, cands);
 
             // a8: safeguarded Newton update (R7), one lane per particle, fp64 scalars
             bool more = false, bad = false;

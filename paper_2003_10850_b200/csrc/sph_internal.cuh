@@ -16,7 +16,9 @@
 
 #define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
 #define SPH_KEY_BITS (3 * SPH_LMAX)
+#ifndef SPH_LEAF
 #define SPH_LEAF 32         // octree leaf capacity = largest candidate segment (one bulk copy)
+#endif
 #define SPH_MAXB 32         // max actives per group (a warp: one lane per active and stream)
 #define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)
 #define SPH_WARPS 4         // warps per CTA of the gather kernels (warps are independent)
@@ -34,7 +36,9 @@
 #ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #endif
-#define SPH_GBLOCK 4         // consecutive groups a warp takes per work-counter increment
+#ifndef SPH_GBLOCK
+#define SPH_GBLOCK 1         // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
+#endif
 
 // octree node, 32 bytes, read as two 16-byte loads
 struct __align__(16) SphNode {
