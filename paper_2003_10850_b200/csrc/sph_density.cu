@@ -80,8 +80,8 @@ template <bool HAS_MASS>
 struct DensWarp {
     float4 slot[SPH_CH];                     // one chunk of candidates as pair records
     WarpWalk ws;
-    float q[SPH_QCAP * 32];                  // hit queue: entry k of lane l at [k * 32 + l] (r^2)
-    float qm[HAS_MASS ? SPH_QCAP * 32 : 32]; // mass of the hit
+    float q[SPH_NA * SPH_QCAP * 32];         // hit queues: entry k of lane l, active q of the lane, at [(q * QCAP + k) * 32 + l] (r^2)
+    float qm[HAS_MASS ? SPH_NA * SPH_QCAP * 32 : 32]; // mass of the hit
     double lo[SPH_MAXB], hi[SPH_MAXB];       // bracket of the h iteration (R7)
     float ax[SPH_MAXB], ay[SPH_MAXB], az[SPH_MAXB], aH[SPH_MAXB];
     uint32_t aid[SPH_MAXB];
@@ -89,18 +89,23 @@ struct DensWarp {
     int ulist[SPH_MAXB];                     // actives still iterating
 };
 
-// per-lane state of one evaluation: lane (a, s) = active a, candidate stream s
-struct DensLane {
+// Per-lane state of one evaluation.  A lane is (active slot ap, candidate stream s) and holds SPH_NA
+// actives (2 ap, 2 ap + 1): every pair record loaded from shared memory is tested against all of them,
+// which halves the shared-memory reads and the loop overhead per test.
+struct DensAct {         // one active of the lane
     float2 s, ds, r, dr; // packed partial sums: sum w, sum d, sum m w, sum m d
     float2 nx, ny, nz;   // minus the active's position in the batch's frame, duplicated for f32x2
     float xi, yi, zi;    // raw position (per-pair image path)
-    float h2, ih2;       // H^2 (-1 in dead lanes: never hit), 1 / H^2
-    uint32_t q0, qw;     // hit queue of this lane: base and write cursor (shared-memory addresses, stride 128 B)
+    float h2, ih2;       // H^2 (-1 for a missing active: never hits), 1 / H^2
+    uint32_t q0, qw;     // this active's hit queue in this lane: base and write cursor (shared-memory addresses, stride 128 B)
+    int cn;              // hits evaluated so far
+};
+struct DensLane {
+    DensAct act[SPH_NA];
     uint32_t mofs;       // offset from a queue entry to its mass entry
     const float4 *cp;    // this stream's first pair record of the chunk
     int cstride;         // float4 elements between consecutive pair records of this stream (f)
     int steps;           // pair records per chunk for this stream (SPH_CH / 2 / f)
-    int cn;              // hits evaluated so far
 };
 
 __device__ __forceinline__ float lds_f32(uint32_t addr)
@@ -110,10 +115,10 @@ __device__ __forceinline__ float lds_f32(uint32_t addr)
     return v;
 }
 
-// Evaluate the newest min(n, queued) hits of every lane, two per step, without branches: a lane that
-// runs out of entries evaluates u = 1, where w = d = 0 exactly (n is warp-uniform).
+// Evaluate the newest min(n, queued) hits of one active of every lane, two per step, without branches:
+// a lane that runs out of entries evaluates u = 1, where w = d = 0 exactly (n is warp-uniform).
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void drain(DensLane &A, int n)
+__device__ __forceinline__ void drain(DensAct &A, uint32_t mofs, int n)
 {
     const int m = min(n, (int)((A.qw - A.q0) >> 7));
     const uint32_t end = A.qw;
@@ -133,16 +138,28 @@ __device__ __forceinline__ void drain(DensLane &A, int n)
         A.s = __fadd2_rn(A.s, w);
         A.ds = __fadd2_rn(A.ds, d);
         if (HAS_MASS) {
-            const float2 mj = f2(v0 ? lds_f32(ra + A.mofs) : 0.f, v1 ? lds_f32(ra + 128u + A.mofs) : 0.f);
+            const float2 mj = f2(v0 ? lds_f32(ra + mofs) : 0.f, v1 ? lds_f32(ra + 128u + mofs) : 0.f);
             A.r = __ffma2_rn(mj, w, A.r);
             A.dr = __ffma2_rn(mj, d, A.dr);
         }
     }
 }
 
-// Test the candidates of the gathered chunk against this lane's active: lane (a, s) takes the pair
+// queue capacity: room for `need` more hits of this active in every lane, else evaluate queued hits first
+template <int KERNEL, bool HAS_MASS>
+__device__ __forceinline__ void make_room(DensAct &A, uint32_t mofs, bool live, int need)
+{
+    const int cnt = (int)((A.qw - A.q0) >> 7);
+    const int mx = __reduce_max_sync(FULLMASK, cnt);
+    if (mx + need > SPH_QCAP) {
+        const int mn = __reduce_min_sync(FULLMASK, live ? cnt : 0x7fffffff);
+        drain<KERNEL, HAS_MASS>(A, mofs, max(mn, mx + need - SPH_QCAP));
+    }
+}
+
+// Test the candidates of the gathered chunk against this lane's actives: lane (ap, s) takes the pair
 // records s, s + f, s + 2f, ...; both distances of a pair come out of one packed f32x2 chain; a hit
-// pushes r^2 (and the mass) onto the lane's queue.
+// pushes r^2 (and the mass) onto the queue of the active it belongs to.
 template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
 {
@@ -151,14 +168,11 @@ __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
     cp += A.cstride;
     for (int t0 = 0; t0 < A.steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, A.steps - t0);
-        // queue capacity: room for 2 nt more hits in every lane, else evaluate queued hits first
-        const int cnt = (int)((A.qw - A.q0) >> 7);
-        const int mx = __reduce_max_sync(FULLMASK, cnt);
-        if (mx + 2 * nt > SPH_QCAP) {
-            const int mn = __reduce_min_sync(FULLMASK, live ? cnt : 0x7fffffff);
-            drain<KERNEL, HAS_MASS>(A, max(mn, mx + 2 * nt - SPH_QCAP));
-        }
-        uint32_t qw = A.qw;
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) make_room<KERNEL, HAS_MASS>(A.act[a], A.mofs, live, 2 * nt);
+        uint32_t qw[SPH_NA];
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) qw[a] = A.act[a].qw;
 #pragma unroll 3
         for (int t = 0; t < nt; t++) {
             const float4 c0 = n0, cz = n1; // (x0,x1,y0,y1) (z0,z1,w0,w1)
@@ -167,29 +181,34 @@ __device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
             // chunk's last record this reads on inside the warp's own shared memory; the value is unused)
             n0 = cp[0]; n1 = cp[SPH_CH / 2];
             cp += A.cstride;
-            float2 r2;
-            if (PAIRWRAP) {
-                const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);
-                const float dy0 = image_diff(A.yi, c0.z, L), dy1 = image_diff(A.yi, c0.w, L);
-                const float dz0 = image_diff(A.zi, c1.x, L), dz1 = image_diff(A.zi, c1.y, L);
-                r2 = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
-            } else {
-                const float2 dx = __fadd2_rn(f2(c0.x, c0.y), A.nx), dy = __fadd2_rn(f2(c0.z, c0.w), A.ny);
-                const float2 dz = __fadd2_rn(c1, A.nz);
-                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-            }
-            if (r2.x < A.h2) {
-                sts_f32(qw, r2.x);
-                if (HAS_MASS) sts_f32(qw + A.mofs, cm.x);
-                qw += 128u;
-            }
-            if (r2.y < A.h2) {
-                sts_f32(qw, r2.y);
-                if (HAS_MASS) sts_f32(qw + A.mofs, cm.y);
-                qw += 128u;
+#pragma unroll
+            for (int a = 0; a < SPH_NA; a++) {
+                const DensAct &P = A.act[a];
+                float2 r2;
+                if (PAIRWRAP) {
+                    const float dx0 = image_diff(P.xi, c0.x, L), dx1 = image_diff(P.xi, c0.y, L);
+                    const float dy0 = image_diff(P.yi, c0.z, L), dy1 = image_diff(P.yi, c0.w, L);
+                    const float dz0 = image_diff(P.zi, c1.x, L), dz1 = image_diff(P.zi, c1.y, L);
+                    r2 = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
+                } else {
+                    const float2 dx = __fadd2_rn(f2(c0.x, c0.y), P.nx), dy = __fadd2_rn(f2(c0.z, c0.w), P.ny);
+                    const float2 dz = __fadd2_rn(c1, P.nz);
+                    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                }
+                if (r2.x < P.h2) {
+                    sts_f32(qw[a], r2.x);
+                    if (HAS_MASS) sts_f32(qw[a] + A.mofs, cm.x);
+                    qw[a] += 128u;
+                }
+                if (r2.y < P.h2) {
+                    sts_f32(qw[a], r2.y);
+                    if (HAS_MASS) sts_f32(qw[a] + A.mofs, cm.y);
+                    qw[a] += 128u;
+                }
             }
         }
-        A.qw = qw;
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) A.act[a].qw = qw[a];
     }
 }
 
@@ -201,40 +220,55 @@ struct WalkCache {
     bool multi;  // scratch: a batch of the current walk has already been seen
 };
 
-// One evaluation of the group's iterating actives at their current H: walk, stream, test, evaluate.
-// Returns the cross-stream totals in the lanes of stream 0 (lane a < g).
+// One evaluation of the group's g iterating actives at their current H: walk, gather, test, evaluate.
+// Returns the totals of the i-th iterating active in lane i (i < g).
 template <int KERNEL, bool HAS_MASS>
 __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, int g, WalkCache &wc, double &S,
                                          double &D, double &R, double &DR, int &nint, unsigned long long &cands)
 {
     const int lane = threadIdx.x & 31;
     const float L = a.L;
-    const int f = streams_for(g);
-    const bool live = lane < g * f;
-    const int ai = live ? lane % g : 0, s = live ? lane / g : 0;
-    const int k = W.ulist[ai];
-    const float xi = W.ax[k], yi = W.ay[k], zi = W.az[k], H = W.aH[k];
-    // bounding box and reach of the actives still iterating
+    const int gp = (g + SPH_NA - 1) / SPH_NA; // active slots: lane = ap + gp * s
+    const int f = streams_for(gp);
+    const bool live = lane < gp * f;
+    const int ap = live ? lane % gp : 0, s = live ? lane / gp : 0;
     const float inf = __int_as_float(0x7f800000);
-    float x0 = warp_min(live ? xi : inf), x1 = warp_max(live ? xi : -inf);
-    float y0 = warp_min(live ? yi : inf), y1 = warp_max(live ? yi : -inf);
-    float z0 = warp_min(live ? zi : inf), z1 = warp_max(live ? zi : -inf);
-    const float hg = warp_max(live ? H : 0.f);
+
+    DensLane A;
+    A.mofs = HAS_MASS ? smem_u32(W.qm) - smem_u32(W.q) : 0u;
+    A.cp = W.slot + s;
+    A.cstride = f;
+    A.steps = (SPH_CH / 2) / f;
+    // bounding box and reach of the actives still iterating
+    float x0 = inf, x1 = -inf, y0 = inf, y1 = -inf, z0 = inf, z1 = -inf, hg = 0.f;
+#pragma unroll
+    for (int q = 0; q < SPH_NA; q++) {
+        DensAct &P = A.act[q];
+        const int i = ap * SPH_NA + q;
+        const bool has = live && i < g;
+        const int k = W.ulist[has ? i : 0];
+        const float H = W.aH[k];
+        P.xi = W.ax[k]; P.yi = W.ay[k]; P.zi = W.az[k];
+        P.h2 = has ? H * H : -1.f; // a missing active never hits
+        P.ih2 = 1.f / (H * H);
+        P.s = P.ds = P.r = P.dr = f2(0.f);
+        P.cn = 0;
+        P.q0 = P.qw = smem_u32(W.q + q * SPH_QCAP * 32 + lane);
+        if (has) {
+            x0 = fminf(x0, P.xi); x1 = fmaxf(x1, P.xi);
+            y0 = fminf(y0, P.yi); y1 = fmaxf(y1, P.yi);
+            z0 = fminf(z0, P.zi); z1 = fmaxf(z1, P.zi);
+            hg = fmaxf(hg, H);
+        }
+    }
+    x0 = warp_min(x0); x1 = warp_max(x1);
+    y0 = warp_min(y0); y1 = warp_max(y1);
+    z0 = warp_min(z0); z1 = warp_max(z1);
+    hg = warp_max(hg);
     const float gcx = 0.5f * (x0 + x1), ghx = 0.5f * (x1 - x0) * (1.f + 1e-6f);
     const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
     const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
 
-    DensLane A;
-    A.s = A.ds = A.r = A.dr = f2(0.f);
-    A.cn = 0;
-    A.xi = xi; A.yi = yi; A.zi = zi;
-    A.h2 = live ? H * H : -1.f; // dead lanes never hit
-    A.ih2 = 1.f / (H * H);
-    A.q0 = A.qw = smem_u32(W.q + lane);
-    A.mofs = HAS_MASS ? smem_u32(W.qm + lane) - A.q0 : 0u;
-    A.cp = W.slot + s;
-    A.cstride = f;
-    A.steps = (SPH_CH / 2) / f;
     // The segment list of the group's previous evaluation is still in shared memory.  It stays valid if
     // it was complete (one batch) and the reach has not grown: the actives still iterating are a subset
     // (their bounding box lies inside the old one), so the old list and its frame cover this evaluation.
@@ -244,10 +278,14 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
     do {
         if (!reuse) walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
         cands += ctl.total;
-        // this lane's active in the batch's frame
-        A.nx = f2(-(ctl.pairwrap ? xi : recentre(xi, ctl.thx, L)));
-        A.ny = f2(-(ctl.pairwrap ? yi : recentre(yi, ctl.thy, L)));
-        A.nz = f2(-(ctl.pairwrap ? zi : recentre(zi, ctl.thz, L)));
+        // this lane's actives in the batch's frame
+#pragma unroll
+        for (int q = 0; q < SPH_NA; q++) {
+            DensAct &P = A.act[q];
+            P.nx = f2(-(ctl.pairwrap ? P.xi : recentre(P.xi, ctl.thx, L)));
+            P.ny = f2(-(ctl.pairwrap ? P.yi : recentre(P.yi, ctl.thy, L)));
+            P.nz = f2(-(ctl.pairwrap ? P.zi : recentre(P.zi, ctl.thz, L)));
+        }
         const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
         GatherCtl gc;
         gc.kseg = 0;
@@ -263,21 +301,37 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
             wc.ctl = ctl;
         }
     } while (ctl.sp > 0);
-    drain<KERNEL, HAS_MASS>(A, __reduce_max_sync(FULLMASK, (int)((A.qw - A.q0) >> 7)));
 
-    // cross-stream totals: lane a + g*s adds lane a + g*(s+d) for d = 1, 2, 4, ...
-    S = (double)A.s.x + (double)A.s.y; D = (double)A.ds.x + (double)A.ds.y;
-    R = (double)A.r.x + (double)A.r.y; DR = (double)A.dr.x + (double)A.dr.y;
-    nint = A.cn;
-    for (int d = 1; d < f; d <<= 1) {
-        const bool take = live && s + d < f;
-        const int from = take ? lane + g * d : lane;
-        double tS = __shfl_sync(FULLMASK, S, from), tD = __shfl_sync(FULLMASK, D, from);
-        int tn = __shfl_sync(FULLMASK, nint, from);
-        if (take) { S += tS; D += tD; nint += tn; }
+    S = D = R = DR = 0.0;
+    nint = 0;
+#pragma unroll
+    for (int q = 0; q < SPH_NA; q++) {
+        DensAct &P = A.act[q];
+        drain<KERNEL, HAS_MASS>(P, A.mofs, __reduce_max_sync(FULLMASK, (int)((P.qw - P.q0) >> 7)));
+        // cross-stream totals: lane ap + gp*s adds lane ap + gp*(s+d) for d = 1, 2, 4, ...
+        double tS = (double)P.s.x + (double)P.s.y, tD = (double)P.ds.x + (double)P.ds.y;
+        double tR = (double)P.r.x + (double)P.r.y, tDR = (double)P.dr.x + (double)P.dr.y;
+        int tn = P.cn;
+        for (int d = 1; d < f; d <<= 1) {
+            const bool take = live && s + d < f;
+            const int from = take ? lane + gp * d : lane;
+            const double uS = __shfl_sync(FULLMASK, tS, from), uD = __shfl_sync(FULLMASK, tD, from);
+            const int un = __shfl_sync(FULLMASK, tn, from);
+            if (take) { tS += uS; tD += uD; tn += un; }
+            if (HAS_MASS) {
+                const double uR = __shfl_sync(FULLMASK, tR, from), uDR = __shfl_sync(FULLMASK, tDR, from);
+                if (take) { tR += uR; tDR += uDR; }
+            }
+        }
+        // active i = ap * SPH_NA + q sits in lane ap (stream 0): hand it to lane i
+        const int src = lane / SPH_NA;
+        const double oS = __shfl_sync(FULLMASK, tS, src), oD = __shfl_sync(FULLMASK, tD, src);
+        const int on = __shfl_sync(FULLMASK, tn, src);
+        const bool mine = lane % SPH_NA == q;
+        if (mine) { S = oS; D = oD; nint = on; }
         if (HAS_MASS) {
-            double tR = __shfl_sync(FULLMASK, R, from), tDR = __shfl_sync(FULLMASK, DR, from);
-            if (take) { R += tR; DR += tDR; }
+            const double oR = __shfl_sync(FULLMASK, tR, src), oDR = __shfl_sync(FULLMASK, tDR, src);
+            if (mine) { R = oR; DR = oDR; }
         }
     }
 }

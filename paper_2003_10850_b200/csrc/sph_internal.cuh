@@ -36,6 +36,9 @@
 #ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #endif
+#ifndef SPH_NA
+#define SPH_NA 1            // actives per lane of the density gather (1 or 2)
+#endif
 #ifndef SPH_GBLOCK
 #define SPH_GBLOCK 1         // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
 #endif
