@@ -7,11 +7,12 @@
 // formulas: DESIGN.md readings R1-R7.
 //
 // Mapping: one warp per group of g <= 32 active particles.  Lane = (active a,
-// stream s): the f = 32/g streams split every chunk of candidates, lanes of one stream read the same
-// candidate (shared-memory broadcast).  The candidate segments found by the walk are streamed into the
-// warp's ring by bulk copies; each lane tests its candidate against its own active and pushes r^2 of a
-// hit onto its private queue; queued hits are evaluated in bulk so the kernel polynomial runs on
-// converged warps.  No block-level barrier, no atomics on the pair path.
+// stream s): the f ~ 32/g streams split every chunk of candidate pairs, lanes of one stream read the
+// same pair record (shared-memory broadcast).  The warp gathers the candidate segments found by the
+// walk, chunk by chunk, into its shared-memory slot (sph_warp.cuh); each lane tests two candidates per
+// step in packed f32x2 against its own active and pushes r^2 of a hit onto its private queue; queued
+// hits are evaluated in bulk so the kernel polynomial runs on converged warps.  No block-level
+// barrier, no atomics on the pair path.
 #include "sph_warp.cuh"
 
 namespace {

@@ -7,7 +7,7 @@
 // the group's reach and the largest support radius inside the node.
 //
 // Same warp-per-group mapping as sph_density.cu: lane = (active, stream); candidates' (x,y,z,H) are
-// streamed through the warp's ring by bulk copies and tested; a hit pushes the candidate's sorted slot
+// gathered chunk by chunk into the warp's shared-memory slot and tested; a hit pushes the candidate's sorted slot
 // onto the lane's queue; queued hits are evaluated in bulk, fetching the pair's remaining state
 // (velocity, sound speed, rho, A, m) from the sorted arrays through L1.
 #include "sph_warp.cuh"
@@ -127,7 +127,7 @@ __device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__
     else drain<KERNEL, false>(a, qp, A, n, fr);
 }
 
-// Test the candidate pairs of one prepared ring slot against this lane's active (symmetric set, R10):
+// Test the candidate pairs of the gathered chunk against this lane's active (symmetric set, R10):
 // hit if r^2 < max(H_i, H_j)^2; a hit pushes the candidate's sorted slot onto the lane's queue.
 template <int KERNEL, bool PAIRWRAP>
 __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,

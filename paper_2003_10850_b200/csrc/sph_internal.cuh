@@ -17,7 +17,7 @@
 #define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
 #define SPH_KEY_BITS (3 * SPH_LMAX)
 #ifndef SPH_LEAF
-#define SPH_LEAF 32         // octree leaf capacity = largest candidate segment (one bulk copy)
+#define SPH_LEAF 32         // octree leaf capacity (a candidate segment is a run of sibling leaves)
 #endif
 #define SPH_MAXB 32         // max actives per group (a warp: one lane per active and stream)
 #define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)

@@ -230,7 +230,7 @@ __device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const Sph
 // so that the test loops load register pairs ready for packed f32x2 arithmetic.  Entries beyond the
 // ragged tail become NaN (every comparison with NaN is false).
 //
-// Why not TMA bulk copies here (they were the first design, profiles/r1c): octree leaves hold ~8
+// Why not TMA bulk copies here (they were the first design, profiles/r1c_packed_tma.md): octree leaves hold ~8
 // particles on average, so a chunk is ~10 pieces of ~100 bytes at arbitrary 16-byte offsets; every
 // piece is one UBLKCP issued through uniform registers, which the compiler serialises lane by lane
 // (ELECT / R2UR / UBLKCP, ~10 issue slots and a long-scoreboard wait per piece): 30 % of the kernel's

@@ -1,0 +1,89 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (library
+defaults): the whole set goes through sph_build_index -> sph_density -> sph_hydro_force on the GPU, and
+a seeded sample of particles is recomputed one by one by the fp64 oracle.
+Density: end to end from the same guess.  Force: stage-isolated, the GPU's own converged (H, rho, Omega)
+of ALL particles are the inputs of both sides (the sampled particles' neighbours need them)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sph_oracle as O
+from paper_2003_10850_b200 import binding as B
+from paper_2003_10850_b200 import inputs as I
+from parity_util import GpuRun, check_density_e2e, check_force
+
+pytestmark = pytest.mark.gpu
+
+SAMPLE = 192
+_cache = {}
+
+
+def _set(name):
+    if name not in _cache:
+        _cache.clear()  # one full-size set at a time in host memory
+        _cache[name] = {"C2": I.config2, "C3": I.config3, "C4": I.config4}[name]()
+    return _cache[name]
+
+
+def _sampled_parity(ps, active_all, label):
+    rng = np.random.default_rng(I.SEED_BASE + 77)
+    pool = np.arange(ps.n, dtype=np.int32) if active_all is None else active_all
+    sample = np.sort(rng.choice(pool, SAMPLE, replace=False)).astype(np.int32)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    gd = g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=active_all)
+    assert gd["unconv"] == 0
+    st = g.sph.stats()
+    n_act = ps.n if active_all is None else len(active_all)
+    assert st["dens_evals"] >= n_act and st["dens_pairs"] > 30 * n_act
+    # density end to end on the sample (oracle: same guess, same rule)
+    o = O.density(ps.pos, ps.h_guess, kernel=ps.kernel, n_target=ps.n_ngb, n_tol=ps.n_tol, mass_scalar=ps.mass,
+                  active=sample)
+    rep = check_density_e2e(gd, o, ps.pos, ps.h_guess, ps.kernel, ps.mass, ps.n_ngb, ps.n_tol, sel=sample, label=label)
+    # properties that hold at any size: every active converged inside the band; inactive entries untouched
+    conv = (gd["status"] & B.ST_CONVERGED) != 0
+    if active_all is None:
+        assert conv.all() and np.all(gd["rho"] > 0) and np.all(gd["Nint"] >= 1)
+    else:
+        assert conv[active_all].all()
+        inact = np.ones(ps.n, bool); inact[active_all] = False
+        assert np.all(gd["rho"][inact] == -1)
+    return g, gd, sample, rep
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
+def test_fullsize_all_active(name):
+    ps = _set(name)
+    g, gd, sample, rep = _sampled_parity(ps, None, name + " full e2e")
+    H, rho, om = gd["H"], gd["rho"], gd["omega"]
+    gf = g.force(ps.vel, ps.u, H, rho, om)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, H, rho, om, kernel=ps.kernel, mass_scalar=ps.mass, active=sample)
+    repf = check_force(gf, of, sel=sample, label=name + " full force")
+    # momentum: all particles active => sum m a = 0 to rounding (pair terms antisymmetric)
+    a = gf["acc"].astype(np.float64)
+    assert np.all(np.abs(a.sum(0)) <= 1e-5 * np.abs(a).sum(0))
+    print(name, "full", rep, repf, g.sph.stats())
+    g.close()
+
+
+def test_fullsize_config5_active_subset():
+    """configs[4]: the 10^7 set with 1% active by time bin; state = the converged set, actives' h perturbed."""
+    ps = _set("C4")
+    act = I.config5_active(ps)
+    g0 = GpuRun(ps.pos, ps.kernel, ps.mass)
+    full = g0.density(ps.h_guess, ps.n_ngb, ps.n_tol)
+    g0.close()
+    assert full["unconv"] == 0
+    hg = I.perturb_h(full["H"], act, I.SEED_BASE + 5)
+    ps5 = I.ParticleSet("C5", ps.pos, ps.vel, ps.u, hg, ps.mass, ps.kernel, ps.n_ngb, ps.n_tol)
+    g, gd, sample, rep = _sampled_parity(ps5, act, "C5 full e2e")
+    H = hg.copy(); H[act] = gd["H"][act]
+    rho = full["rho"].copy(); rho[act] = gd["rho"][act]
+    om = full["omega"].copy(); om[act] = gd["omega"][act]
+    gf = g.force(ps.vel, ps.u, H, rho, om, active=act)
+    of = O.hydro_force(ps.pos, ps.vel, ps.u, H, rho, om, kernel=ps.kernel, mass_scalar=ps.mass, active=sample)
+    repf = check_force(gf, of, sel=sample, label="C5 full force")
+    inact = np.ones(ps.n, bool); inact[act] = False
+    assert np.all(gf["acc"][inact] == 7.0)
+    print("C5 full", rep, repf, g.sph.stats())
+    g.close()
+    _cache.clear()
