@@ -74,40 +74,48 @@ __global__ void k_tree_init(SphCounters *cnt, SphNode *nodes, uint32_t n, float 
 
 // a4: split every node of `level` that holds more than leaf_cap particles into its 8 octants.
 // The octant of a particle at this level is a 3-bit digit of its key; the sorted order makes each
-// child a contiguous run found by binary search.
+// child a contiguous run found by binary search.  Eight lanes share a node: lane k finds the start of
+// octant k, so the seven dependent-load chains of a node run side by side (the kernel is bound by
+// that latency at the top levels, where a run holds millions of keys).
 __global__ void k_tree_split(SphCounters *cnt, SphNode *nodes, const uint64_t *__restrict__ keys, int level,
                              uint32_t leaf_cap, uint32_t node_cap)
 {
-    uint32_t beg = cnt->lvl_begin[level], end = cnt->lvl_begin[level + 1];
-    int shift = 3 * (SPH_LMAX - 1 - level);
-    for (uint32_t nd = beg + blockIdx.x * blockDim.x + threadIdx.x; nd < end; nd += gridDim.x * blockDim.x) {
-        SphNode p = nodes[nd];
-        if (p.count <= leaf_cap) continue;
-        uint32_t c0 = atomicAdd(&cnt->n_nodes, 8u);
-        if (c0 + 8u > node_cap) { atomicExch(&cnt->overflow, 1u); continue; } // stays an oversize leaf
-        uint32_t b[9];
-        b[0] = p.start;
-        b[8] = p.start + p.count;
-        for (int k = 1; k < 8; k++) { // first slot in [b[k-1], b[8]) whose digit >= k
-            uint32_t lo = b[k - 1], hi = b[8];
-            while (lo < hi) {
-                uint32_t mid = lo + ((hi - lo) >> 1);
-                uint32_t dig = (uint32_t)(keys[mid] >> shift) & 7u;
-                if (dig < (uint32_t)k) lo = mid + 1; else hi = mid;
-            }
-            b[k] = lo;
+    const uint32_t beg = cnt->lvl_begin[level], end = cnt->lvl_begin[level + 1];
+    const int shift = 3 * (SPH_LMAX - 1 - level);
+    const uint32_t k = threadIdx.x & 7u;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x, nthr = gridDim.x * blockDim.x;
+    // warp-uniform trip count: a warp covers 4 consecutive nodes per step
+    for (uint32_t base = beg + ((tid & ~31u) >> 3); base < end; base += nthr >> 3) {
+        const uint32_t nd = base + ((threadIdx.x & 31u) >> 3);
+        const bool valid = nd < end;
+        SphNode p = nodes[valid ? nd : beg];
+        const bool split = valid && p.count > leaf_cap;
+        uint32_t c0 = 0;
+        if (split && k == 0) c0 = atomicAdd(&cnt->n_nodes, 8u);
+        c0 = __shfl_sync(0xffffffffu, c0, threadIdx.x & 24u);
+        const bool ok = split && c0 + 8u <= node_cap;
+        if (split && !ok && k == 0) atomicExch(&cnt->overflow, 1u); // stays an oversize leaf
+        // first slot in [start, start + count) whose digit >= k
+        uint32_t lo = p.start, hi = p.start + p.count;
+        if (!ok || k == 0) hi = lo;
+        while (lo < hi) {
+            const uint32_t mid = lo + ((hi - lo) >> 1);
+            const uint32_t dig = (uint32_t)(keys[mid] >> shift) & 7u;
+            if (dig < k) lo = mid + 1; else hi = mid;
         }
-        float q = 0.5f * p.half;
-        for (int k = 0; k < 8; k++) {
+        uint32_t nxt = __shfl_down_sync(0xffffffffu, lo, 1);
+        if (k == 7u) nxt = p.start + p.count;
+        if (ok) {
+            const float q = 0.5f * p.half;
             SphNode c;
-            c.start = b[k]; c.count = b[k + 1] - b[k]; c.child = 0; c.parent = nd;
+            c.start = lo; c.count = nxt - lo; c.child = 0; c.parent = nd;
             c.cx = p.cx + ((k & 1) ? q : -q);
             c.cy = p.cy + ((k & 2) ? q : -q);
             c.cz = p.cz + ((k & 4) ? q : -q);
             c.half = q;
             nodes[c0 + k] = c;
+            if (k == 0) nodes[nd].child = c0;
         }
-        nodes[nd].child = c0;
     }
     // last block to finish publishes the end of the next level
     __syncthreads();
