@@ -92,7 +92,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
             const float r = r2 * rinv;
-            const float hinv_j = __fdividef(1.f, P0.w);
+            const float hinv_j = __frcp_rn(P0.w); // correctly rounded: H^-4 carries four times its error
             const float hj2 = hinv_j * hinv_j;
             const float Fi = A.f4 * kern_dw<KERNEL>(r * A.hinv);
             const float Fj = kern_sigma<KERNEL>() * hj2 * hj2 * kern_dw<KERNEL>(r * hinv_j);
@@ -100,7 +100,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             const float vr = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx)) * rinv;
             const float mu = fminf(vr, 0.f);
             const float vs = A.c + P1.w - 3.f * mu;
-            const float Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
+            const float Pi = -alpha * vs * mu * __frcp_rn(A.rho + P2.x);
             const float Fbar = 0.5f * (Fi + Fj);
             const float AiFi = A.A * Fi;
             const float pv = Pi * Fbar;

@@ -71,8 +71,11 @@ def check_density_stage(g, o, sel=None, label=""):
     rel = np.abs(grho - o["rho"]) / o["rho"]
     assert rel.max() <= RTOL_RHO, f"{label}: rho rel err {rel.max():.3e}"
     om_o = o["omega"]
-    relo = np.abs(gom - om_o) / np.where(om_o != 0, np.abs(om_o), 1.0)  # a lone particle has Omega = 0 exactly
-    assert relo.max() <= RTOL_RHO, f"{label}: omega rel err {relo.max():.3e}"
+    # Omega = 1 - D/(3S) cancels (exactly to 0 for a lone particle): its error is measured against the
+    # magnitude of the terms that cancel, 1 + |1 - Omega| (R15); for converged sets Omega ~ 1 and
+    # this is the plain 1e-5 relative bound
+    relo = np.abs(gom - om_o) / (1.0 + np.abs(1.0 - om_o))
+    assert relo.max() <= RTOL_RHO, f"{label}: omega err {relo.max():.3e}"
     return dict(n_edge=int(edge.sum()), n_mismatch=int(mism.sum()), rho_err=float(rel.max()), omega_err=float(relo.max()))
 
 
