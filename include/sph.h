@@ -94,9 +94,10 @@ int sph_destroy(sph_ctx *ctx);
 /*
  * Build the spatial index over n particles (steps a1-a5 of DESIGN.md): 48-bit Morton keys
  * (16 bits per axis), radix sort of (key, id), sorted float4 copy (x,y,z,m), inverse permutation,
- * an octree over the sorted order whose leaves hold <= 32 particles, and the group list (every leaf
- * cut into balanced runs of <= group_cap consecutive particles).  Replaces the paper's Hilbert keys + domain decomposition + tree build (§1,
- * :194-196 §4).
+ * an octree over the sorted order whose leaves hold <= 32 particles, and the group list: the highest
+ * octree nodes holding <= group_node particles, each cut into balanced runs of <= group_cap consecutive
+ * sorted particles (one warp per group).  Replaces the paper's Hilbert keys + domain decomposition +
+ * tree build (PAPER.md:25, :41 §1, :194-196 §4).
  *   pos   [n*3] device, x,y,z per particle, 0 <= x < box (values outside are clamped into the
  *         boundary cells for the search and otherwise used as given);
  *   mass  [n] device or NULL; if NULL every particle has mass_scalar.
@@ -121,6 +122,7 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
  *   n_unconverged_host  HOST pointer (may be NULL): number of active particles that stopped
  *                 without SPH_ST_CONVERGED.
  * Returns SPH_OK, or SPH_W_NOCONV if *n_unconverged_host would be > 0.  Synchronises once.
+ * An active id outside [0, n) makes the call compute and write nothing and return SPH_E_ARG.
  */
 int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol,
                 float *h, float *rho, float *omega, int32_t *ngb_count, int32_t *status,
@@ -135,7 +137,8 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
  * with A = (gamma-1) u / (omega rho), F_ij(H) = dW/dr(r_ij, H), Pi_ij the signal-velocity viscosity.
  *   vel [n*3], u [n], h [n], rho [n], omega [n]: device, valid for ALL n particles (inactive
  *   neighbours contribute with their current values, R12); acc [n*3], dudt [n], vsig_max [n]: device,
- *   written for active particles only.  Asynchronous.
+ *   written for active particles only.  Asynchronous: an active id outside [0, n) makes the call compute
+ *   and write nothing, and the next synchronising call (sph_density, sph_get_stats) returns SPH_E_ARG.
  */
 int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
                     const float *h, const float *rho, const float *omega, float *acc, float *dudt,

@@ -134,12 +134,13 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
     if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
     if ((rc = sph_density_launch(ctx, active != nullptr, items, n_ngb_target, n_ngb_tol, h, rho, omega, ngb_count, status)))
         return rc;
-    unsigned int unconv = 0;
-    SPH_CUDA(ctx, cudaMemcpyAsync(&unconv, &ctx->cnt->n_unconv, sizeof(unconv), cudaMemcpyDeviceToHost, ctx->stream));
+    unsigned int res[2] = {0, 0}; // n_unconv, bad_ids (adjacent counters)
+    SPH_CUDA(ctx, cudaMemcpyAsync(res, &ctx->cnt->n_unconv, sizeof(res), cudaMemcpyDeviceToHost, ctx->stream));
     SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     SPH_CUDA(ctx, cudaGetLastError());
-    if (n_unconverged_host) *n_unconverged_host = unconv;
-    return unconv ? SPH_W_NOCONV : SPH_OK;
+    if (res[1]) return sph_fail(ctx, SPH_E_ARG, "sph_density: %u active ids outside [0, n): nothing was computed", res[1]);
+    if (n_unconverged_host) *n_unconverged_host = res[0];
+    return res[0] ? SPH_W_NOCONV : SPH_OK;
 }
 
 int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
@@ -233,6 +234,8 @@ int sph_get_stats(sph_ctx *ctx, sph_stats *out)
     SphCounters h;
     SPH_CUDA(ctx, cudaMemcpyAsync(&h, ctx->cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
     SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (h.bad_ids)
+        return sph_fail(ctx, SPH_E_ARG, "%u active ids outside [0, n) in the last call: nothing was computed", h.bad_ids);
     out->dens_evals = (int64_t)h.dens_evals;
     out->dens_candidates = (int64_t)h.dens_cands;
     out->dens_pairs = (int64_t)h.dens_pairs;

@@ -343,6 +343,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     DensWarp<HAS_MASS> &W = reinterpret_cast<DensWarp<HAS_MASS> *>(smem_raw)[warp];
+    if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_evals = 0, st_cands = 0, st_pairs = 0; // meaningful in lane 0 only
     unsigned int st_unconv = 0;
@@ -468,9 +469,10 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
     }
 }
 
-__global__ void k_reset_counters(SphCounters *c, int which)
+__global__ void k_reset_counters(SphCounters *c, int which, bool subset)
 {
     c->work = 0;
+    if (!subset) c->bad_ids = 0; // no active list in this call
     if (which == 0) { c->n_unconv = 0; c->dens_evals = 0; c->dens_cands = 0; c->dens_pairs = 0; }
     else { c->force_cands = 0; c->force_pairs = 0; }
 }
@@ -495,9 +497,9 @@ int launch(sph_ctx *ctx, const DensArgs &a, int64_t est_groups)
 
 } // namespace
 
-void sph_reset_counters(sph_ctx *ctx, int which)
+void sph_reset_counters(sph_ctx *ctx, int which, bool subset)
 {
-    k_reset_counters<<<1, 1, 0, ctx->stream>>>(ctx->cnt, which);
+    k_reset_counters<<<1, 1, 0, ctx->stream>>>(ctx->cnt, which, subset);
     ctx->launches++;
 }
 
@@ -521,7 +523,7 @@ int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_targe
     a.max_iter = ctx->prm.max_iter;
     a.mass_scalar = ctx->mass_scalar;
     a.h = h; a.rho = rho; a.omega = omega; a.ngb = ngb; a.status = status;
-    sph_reset_counters(ctx, 0);
+    sph_reset_counters(ctx, 0, subset);
     int64_t est_groups = subset ? n_items : ctx->n_groups;
     int rc;
     cudaEventRecord(ctx->ev[2], ctx->stream);

@@ -188,6 +188,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ForceWarp &W = reinterpret_cast<ForceWarp *>(smem_raw)[warp];
     const float L = a.L;
+    if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_cands = 0, st_pairs = 0;
     uint32_t *qp = W.q + lane;
@@ -360,7 +361,7 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
                                                        ctx->f_xyzh, ctx->f_vc, ctx->f_raf);
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->node_hmax, 0, sizeof(float) * ctx->n_nodes, st));
     k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
-    sph_reset_counters(ctx, 1);
+    sph_reset_counters(ctx, 1, subset);
     ctx->launches += 3;
     cudaEventRecord(ctx->ev[5], st);
     ctx->ev_set[2] = true;

@@ -148,11 +148,15 @@ __global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict_
     }
 }
 
-__global__ void k_act_slots(int64_t na, const int32_t *__restrict__ active, const uint32_t *__restrict__ inv,
-                            uint32_t *__restrict__ slot)
+__global__ void k_act_slots(int64_t na, int64_t n, const int32_t *__restrict__ active, const uint32_t *__restrict__ inv,
+                            uint32_t *__restrict__ slot, SphCounters *cnt)
 {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < na) slot[k] = inv[active[k]];
+    if (k >= na) return;
+    const int32_t id = active[k];
+    const bool ok = id >= 0 && (int64_t)id < n;
+    if (!ok) atomicAdd(&cnt->bad_ids, 1u); // the gather kernels then return at once; reported as SPH_E_ARG
+    slot[k] = ok ? inv[id] : 0u;
 }
 
 __global__ void k_act_flags(int64_t na, const uint32_t *__restrict__ slot, const uint32_t *__restrict__ gid,
@@ -296,7 +300,8 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
         ctx->cap_act = cap;
     }
     const int T = 256;
-    k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, active, ctx->inv, ctx->act_slot_alt);
+    SPH_CUDA(ctx, cudaMemsetAsync(&ctx->cnt->bad_ids, 0, sizeof(unsigned int), st));
+    k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, ctx->n, active, ctx->inv, ctx->act_slot_alt, ctx->cnt);
     int bits = 1;
     while (bits < 32 && ((int64_t)1 << bits) < ctx->n) bits++;
     size_t tb = 0, tb2 = 0;

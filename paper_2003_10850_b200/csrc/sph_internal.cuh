@@ -61,6 +61,7 @@ struct SphCounters {
     unsigned int overflow;     // node pool exhausted (graceful: oversize leaves)
     unsigned int work;         // persistent-kernel group counter
     unsigned int n_unconv;     // density: particles stopped without convergence
+    unsigned int bad_ids;      // active ids outside [0, n) in the current active list (the call computes nothing)
     unsigned int lvl_begin[SPH_LMAX + 3];
     unsigned int lvl_done[SPH_LMAX + 3];
     unsigned long long dens_evals, dens_cands, dens_pairs, force_cands, force_pairs;
@@ -123,7 +124,7 @@ int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
 
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
-void sph_reset_counters(sph_ctx *ctx, int which); // 0: density, 1: force
+void sph_reset_counters(sph_ctx *ctx, int which, bool subset); // 0: density, 1: force
 int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t n_active);
 int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_target, float n_tol, float *h,
                        float *rho, float *omega, int32_t *ngb, int32_t *status);

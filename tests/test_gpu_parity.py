@@ -323,3 +323,25 @@ def test_errors_are_return_codes():
     sph.close()
     with pytest.raises(B.SphError):
         B.Sph(kernel=7)
+
+
+def test_active_ids_out_of_range_are_reported_and_nothing_is_written():
+    """Precondition check of the boundary: an id outside [0, n) makes the call compute nothing; sph_density
+    (which synchronises) returns SPH_E_ARG, after the asynchronous sph_hydro_force the next synchronising
+    call does.  A later valid call works again."""
+    ps = I.config1(8)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    bad = np.array([3, ps.n, 7], np.int32)
+    with pytest.raises(B.SphError) as e:
+        g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=bad)
+    assert e.value.code == B.SPH_E_ARG
+    neg = np.array([-1], np.int32)
+    gf = g.force(ps.vel, ps.u, ps.h_guess, np.ones(ps.n, np.float32), np.ones(ps.n, np.float32), active=neg)
+    assert np.all(gf["acc"] == 7.0) and np.all(gf["dudt"] == 7.0)  # nothing written
+    with pytest.raises(B.SphError) as e:
+        g.sph.stats()
+    assert e.value.code == B.SPH_E_ARG
+    ok = g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=np.array([3, 7], np.int32))
+    assert ok["unconv"] == 0 and ok["rho"][3] > 0 and ok["rho"][4] == -1
+    g.sph.stats()
+    g.close()
