@@ -133,9 +133,9 @@ def oracle_sample_run(ps, active_all, sample: int, seed: int):
 
 
 def default_sample(ps) -> int:
-    # sized for roughly 10-30 s of oracle work on the box's host cores (measured on 16 cores: ~6.5e3 updates/s
+    # sized for roughly 10-30 s of oracle work on the box's host cores (measured on 16 cores: ~1.8e4 updates/s
     # at C4; the 64-neighbour configs are several times faster per update)
-    return 131072 if ps.kernel == 1 else 524288
+    return 262144 if ps.kernel == 1 else 1048576
 
 
 def run_reference(args, rank: int):
