@@ -299,6 +299,15 @@ def main():
         dist.barrier()
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1) - t_flush
+    # evaluation histogram of the h iteration (outside the timed region): one more density pass with status
+    stt = torch.zeros(n, device="cuda", dtype=torch.int32)
+    if active is None:
+        h.copy_(h_guess)
+    else:
+        h.index_copy_(0, active.long(), h_guess.index_select(0, active.long()))
+    sph.sph_density(h, rho, om, ngb, ps.n_ngb, ps.n_tol, active=active, status=stt)
+    its = (stt & 0xff) if active is None else (stt.index_select(0, active.long()) & 0xff)
+    eval_hist = torch.bincount(its.long(), minlength=2).cpu().tolist()
     launches = per[-1]["launches"] - l0
     ms = max_over_ranks(ms, world, "cuda")
     value = whole_job_value(world, n_active, args.steps, ms)
@@ -370,7 +379,9 @@ def main():
                       "density_true_pairs": st["dens_pairs"], "density_candidates": st["dens_candidates"],
                       "force_true_pairs": st["force_pairs"], "force_candidates": st["force_candidates"],
                       "pair_interactions_per_s": (st["dens_pairs"] + st["force_pairs"]) * world / (ms / args.steps * 1e-3),
-                      "unconverged": per[-1]["unconv"]},
+                      "unconverged": per[-1]["unconv"],
+                      "density_eval_histogram": {str(k): int(v) for k, v in enumerate(eval_hist) if v},
+                      "updates_per_s_without_index": world * n_active / ((ms / args.steps - ti) * 1e-3)},
         }
         if world == 1 and not args.no_cpu_baseline:
             sample = args.cpu_sample or default_sample(ps)

@@ -49,7 +49,7 @@ __device__ __forceinline__ float kern_sigma()
 struct ForceWarp {
     float4 slot[SPH_CH];                // one chunk of candidates as pair records (x,y,z,H)
     WarpWalk ws;
-    uint32_t q[SPH_QCAP * 32];          // hit queue: sorted slot of the neighbour
+    uint32_t q[SPH_QCAP_FORCE * 32];          // hit queue: sorted slot of the neighbour
     alignas(16) uint32_t gidx[SPH_CH];              // sorted slot of every candidate of the chunk
 };
 
@@ -145,9 +145,9 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
     for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
         const int nt = min(SPH_QSTEP, steps - t0);
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
-        if (mx + 2 * nt > SPH_QCAP) {
+        if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP), fr);
+            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
         }
         const uint32_t q0 = smem_u32(qp);
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;

@@ -33,6 +33,9 @@
 #ifndef SPH_QCAP
 #define SPH_QCAP 32         // per-lane hit-queue entries (>= 2 * SPH_QSTEP)
 #endif
+#ifndef SPH_QCAP_FORCE
+#define SPH_QCAP_FORCE 32   // the same for the force kernel (a hit costs ~95 instructions there: fuller drains pay)
+#endif
 #ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #endif
