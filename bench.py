@@ -352,13 +352,14 @@ def main():
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         peak = sm_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
+        # DRAM bytes per launch of the dominant kernel, from the committed ncu capture (profiles/traffic.csv)
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(w, {}).get("density_kernel_dram_bytes_per_launch")
-            except Exception:
-                traffic = None
+            import csv
+            for row in csv.DictReader(open(tpath)):
+                if row["workload"] == w and row["kernel"] == "k_density":
+                    traffic = int(row["dram_bytes_per_launch"])
         roof = {"bound": "alu", "kernel": "k_density (a6-a9)", "achieved": fl_d / (tk * 1e-3) * 1e-12, "peak": peak,
                 "unit": "TFLOP/s", "frac": fl_d / (tk * 1e-3) * 1e-12 / peak, "traffic": traffic,
                 "peak_source": f"derived: {sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md); "
