@@ -66,28 +66,32 @@ struct ForceLane {
 struct Frame {
     float thx, thy, thz;
     bool pairwrap;
+    bool rec; // some axis is recentred (thr finite); false: raw coordinates are already the frame
 };
 
 // evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
-template <int KERNEL, bool PAIRWRAP>
+// WRAP: 0 raw coordinate differences, 1 recentred frame, 2 per-pair nearest image
+template <int KERNEL, int WRAP>
 __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
                                       const Frame &fr)
 {
     const int m = min(n, A.cnt), base = A.cnt - m;
     const float L = a.L, alpha = a.alpha;
-    const float xf = PAIRWRAP ? A.xi : recentre(A.xi, fr.thx, L);
-    const float yf = PAIRWRAP ? A.yi : recentre(A.yi, fr.thy, L);
-    const float zf = PAIRWRAP ? A.zi : recentre(A.zi, fr.thz, L);
+    const float xf = WRAP == 1 ? recentre(A.xi, fr.thx, L) : A.xi;
+    const float yf = WRAP == 1 ? recentre(A.yi, fr.thy, L) : A.yi;
+    const float zf = WRAP == 1 ? recentre(A.zi, fr.thz, L) : A.zi;
 #pragma unroll 2
     for (int k = 0; k < n; k++) {
         if (k < m) {
             const uint32_t j = qp[(base + k) * 32];
             const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + j), P2 = __ldg(a.raf + j);
             float dx, dy, dz;
-            if (PAIRWRAP) {
+            if (WRAP == 2) {
                 dx = image_diff(A.xi, P0.x, L); dy = image_diff(A.yi, P0.y, L); dz = image_diff(A.zi, P0.z, L);
-            } else {
+            } else if (WRAP == 1) {
                 dx = xf - recentre(P0.x, fr.thx, L); dy = yf - recentre(P0.y, fr.thy, L); dz = zf - recentre(P0.z, fr.thz, L);
+            } else {
+                dx = xf - P0.x; dy = yf - P0.y; dz = zf - P0.z;
             }
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
@@ -123,8 +127,9 @@ template <int KERNEL>
 __device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
                                           const Frame &fr)
 {
-    if (fr.pairwrap) drain<KERNEL, true>(a, qp, A, n, fr);
-    else drain<KERNEL, false>(a, qp, A, n, fr);
+    if (fr.pairwrap) drain<KERNEL, 2>(a, qp, A, n, fr);
+    else if (fr.rec) drain<KERNEL, 1>(a, qp, A, n, fr);
+    else drain<KERNEL, 0>(a, qp, A, n, fr);
 }
 
 // Test the candidate pairs of the gathered chunk against this lane's active (symmetric set, R10):
@@ -147,7 +152,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
         if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, PAIRWRAP>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
+            drain_any<KERNEL>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
         }
         const uint32_t q0 = smem_u32(qp);
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
@@ -239,6 +244,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
             Frame fr;
             fr.thx = fr.thy = fr.thz = __int_as_float(0x7f800000);
             fr.pairwrap = false;
+            fr.rec = false;
             do {
                 walk_batch<true>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
                 cands += ctl.total;
@@ -246,6 +252,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
                 if (ctl.pairwrap != fr.pairwrap || ctl.thx != fr.thx || ctl.thy != fr.thy || ctl.thz != fr.thz) {
                     drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
                     fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
+                    fr.rec = ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f;
                 }
                 const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
                 GatherCtl gc;
