@@ -17,7 +17,7 @@ namespace {
 struct ForceArgs {
     const SphNode *nodes;
     const float *node_hmax;
-    const float4 *xyzh, *vc, *raf; // sorted: (x,y,z,H) (vx,vy,vz,c) (rho, A, m, slot)
+    const float4 *xyzh, *vc, *raf; // sorted: (x,y,z,H) (vx,vy,vz,c) (rho, A, m, 1/H)
     const uint32_t *perm;
     const uint32_t *gstart;
     const unsigned int *n_groups;
@@ -38,6 +38,24 @@ __device__ __forceinline__ float kern_dw(float q) // w'(q), 0 for q >= 1 (R1)
     } else {
         float t2 = t * t, t4 = t2 * t2, t7 = t4 * t2 * t;
         return -22.f * q * t7 * fmaf(q, fmaf(16.f, q, 7.f), 1.f);
+    }
+}
+// w'(q) for the two arguments of a pair, (r / H_i, r / H_j), in one packed f32x2 chain
+template <int KERNEL>
+__device__ __forceinline__ float2 kern_dw2(float2 q)
+{
+    const float2 one = make_float2(1.f, 1.f);
+    float2 t = __ffma2_rn(q, make_float2(-1.f, -1.f), one);
+    t = make_float2(fmaxf(t.x, 0.f), fmaxf(t.y, 0.f));
+    const float2 t2 = __fmul2_rn(t, t);
+    if (KERNEL == SPH_KERNEL_CUBIC) {
+        const float2 a = __fmul2_rn(q, __ffma2_rn(make_float2(18.f, 18.f), q, make_float2(-12.f, -12.f)));
+        const float2 b = __fmul2_rn(make_float2(-6.f, -6.f), t2);
+        return make_float2(q.x <= 0.5f ? a.x : b.x, q.y <= 0.5f ? a.y : b.y);
+    } else {
+        const float2 t4 = __fmul2_rn(t2, t2), t7 = __fmul2_rn(__fmul2_rn(t4, t2), t);
+        const float2 p = __ffma2_rn(q, __ffma2_rn(make_float2(16.f, 16.f), q, make_float2(7.f, 7.f)), one);
+        return __fmul2_rn(__fmul2_rn(__fmul2_rn(make_float2(-22.f, -22.f), q), t7), p);
     }
 }
 template <int KERNEL>
@@ -96,15 +114,16 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
             const float r = r2 * rinv;
-            const float hinv_j = __frcp_rn(P0.w); // correctly rounded: H^-4 carries four times its error
+            const float hinv_j = P2.w; // 1 / H_j, correctly rounded once per particle (k_force_prep)
             const float hj2 = hinv_j * hinv_j;
-            const float Fi = A.f4 * kern_dw<KERNEL>(r * A.hinv);
-            const float Fj = kern_sigma<KERNEL>() * hj2 * hj2 * kern_dw<KERNEL>(r * hinv_j);
+            const float2 dw = kern_dw2<KERNEL>(__fmul2_rn(make_float2(r, r), make_float2(A.hinv, hinv_j)));
+            const float Fi = A.f4 * dw.x;
+            const float Fj = kern_sigma<KERNEL>() * hj2 * hj2 * dw.y;
             const float dvx = A.vx - P1.x, dvy = A.vy - P1.y, dvz = A.vz - P1.z;
             const float vr = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx)) * rinv;
             const float mu = fminf(vr, 0.f);
             const float vs = A.c + P1.w - 3.f * mu;
-            const float Pi = -alpha * vs * mu * __frcp_rn(A.rho + P2.x);
+            const float Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
             const float Fbar = 0.5f * (Fi + Fj);
             const float AiFi = A.A * Fi;
             const float pv = Pi * Fbar;
@@ -314,7 +333,7 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
     float A = (gamma - 1.f) * ui / (omega[id] * ri); // P/(Omega rho^2), P = (gamma-1) rho u
     xyzh[i] = make_float4(p.x, p.y, p.z, h[id]);
     vc[i] = make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c);
-    raf[i] = make_float4(ri, A, p.w, __uint_as_float((uint32_t)i));
+    raf[i] = make_float4(ri, A, p.w, 1.f / h[id]);
 }
 
 // largest support radius inside every octree node: leaves scan their particles, then push the value
