@@ -291,7 +291,7 @@ __device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &
         GatherCtl gc;
         gc.kseg = 0;
         for (uint32_t c = 0; c < nch; c++) {
-            gather_chunk(W.ws, ctl, gc, c, W.slot, nullptr, a.xyzm, L);
+            gather_chunk<false>(W.ws, ctl, gc, c, W.slot, nullptr, a.xyzm, L);
             if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(A, live, L);
             else consume_chunk<KERNEL, HAS_MASS, false>(A, live, L);
         }

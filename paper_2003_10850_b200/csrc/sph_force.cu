@@ -177,7 +177,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
 #pragma unroll 2
         for (int t = 0; t < nt; t++) {
-            const float4 c0 = cp[0], c1 = cp[SPH_CH / 2]; // (x0,x1,y0,y1) (z0,z1,h0,h1)
+            const float4 c0 = cp[0], c1 = cp[SPH_CH / 2]; // (x0,x1,y0,y1) (z0,z1,H0^2,H1^2)
             cp += f;
             float2 r2;
             if (PAIRWRAP) {
@@ -190,7 +190,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
                 const float2 dz = __fadd2_rn(make_float2(c1.x, c1.y), nz);
                 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
-            const float2 hj2 = __fmul2_rn(make_float2(c1.z, c1.w), make_float2(c1.z, c1.w));
+            const float2 hj2 = make_float2(c1.z, c1.w); // H_j^2 (squared once per candidate by the gather)
             if (r2.x < fmaxf(A.h2, hj2.x)) {
                 sts_u32(qw, lds_u32(ga));
                 qw += 128u;
@@ -277,7 +277,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
                 GatherCtl gc;
                 gc.kseg = 0;
                 for (uint32_t c = 0; c < nch; c++) {
-                    gather_chunk(W.ws, ctl, gc, c, W.slot, W.gidx, a.xyzh, L);
+                    gather_chunk<true>(W.ws, ctl, gc, c, W.slot, W.gidx, a.xyzh, L);
                     if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                     else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                 }

@@ -257,6 +257,7 @@ __device__ __forceinline__ float4 ldg_nc(const float4 *p)
 }
 
 // slotp: [SPH_CH] float4; gidx: [SPH_CH] sorted slot of every entry or NULL
+template <bool SQUARE_W>
 __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &ctl, GatherCtl &gc, uint32_t chunk,
                                              float4 *slotp, uint32_t *gidx, const float4 *__restrict__ src, float L)
 {
@@ -310,6 +311,7 @@ __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &
                 ca.x = recentre(ca.x, ctl.thx, L); ca.y = recentre(ca.y, ctl.thy, L); ca.z = recentre(ca.z, ctl.thz, L);
                 cb.x = recentre(cb.x, ctl.thx, L); cb.y = recentre(cb.y, ctl.thy, L); cb.z = recentre(cb.z, ctl.thz, L);
             }
+            if (SQUARE_W) { ca.w *= ca.w; cb.w *= cb.w; } // force pass: the test compares r^2 with H_j^2
             slotp[pr] = make_float4(ca.x, cb.x, ca.y, cb.y);
             slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, ca.w, cb.w);
             if (gidx) reinterpret_cast<uint2 *>(gidx)[pr] = make_uint2(ja, jb);
