@@ -320,6 +320,87 @@ __device__ __forceinline__ void gather_chunk(const WarpWalk &ws, const WalkCtl &
     __syncwarp();
 }
 
+// ---- the same gather split in two, so that the loads of chunk c + 1 are in flight while chunk c is
+// tested: gather_load computes the addresses and issues the 16-byte loads into registers, gather_store
+// (after the consumer is done with the slot) fixes up and writes the pair records.
+struct GatherRegs {
+    float4 c[4];   // entries 2 l, 2 l + 1, 2 (l + 32), 2 (l + 32) + 1 of the chunk
+    uint32_t j[4]; // their sorted slots
+    uint32_t lo, hi;
+};
+
+__device__ __forceinline__ void gather_load(const WarpWalk &ws, const WalkCtl &ctl, GatherCtl &gc, uint32_t chunk,
+                                            GatherRegs &G, const float4 *__restrict__ src)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t lo = chunk * SPH_CH, hi = min(lo + SPH_CH, ctl.total);
+    G.lo = lo; G.hi = hi;
+    const int kfirst = gc.kseg;
+    uint32_t w0 = 0u, w1 = 0u, w2 = 0u, w3 = 0u;
+    int k0 = kfirst;
+    for (;;) {
+        const int k = k0 + lane;
+        const bool in = k < ctl.n_seg;
+        const uint32_t p0 = in ? ws.seg_pre[k] : 0xffffffffu, p1 = in ? ws.seg_pre[k + 1] : 0xffffffffu;
+        const bool ov = in && p0 < hi && p1 > lo;
+        const uint32_t pos = max(p0, lo) - lo, bit = ov ? 1u << (pos & 31u) : 0u, wd = pos >> 5;
+        w0 |= __reduce_or_sync(FULLMASK, wd == 0u ? bit : 0u);
+        w1 |= __reduce_or_sync(FULLMASK, wd == 1u ? bit : 0u);
+        w2 |= __reduce_or_sync(FULLMASK, wd == 2u ? bit : 0u);
+        w3 |= __reduce_or_sync(FULLMASK, wd == 3u ? bit : 0u);
+        const unsigned m = __ballot_sync(FULLMASK, in && p1 > hi);
+        if (m) { k0 += __ffs(m) - 1; break; }
+        k0 += 32;
+        if (k0 >= ctl.n_seg) { k0 = ctl.n_seg; break; }
+    }
+    gc.kseg = k0;
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+        const int pr = lane + 32 * r;
+        if (pr < SPH_CH / 2) {
+            const int e0 = 2 * pr, wl = e0 >> 5, sh = e0 & 31;
+            const uint32_t wmine = wl == 0 ? w0 : wl == 1 ? w1 : wl == 2 ? w2 : w3;
+            const int below = kfirst - 1 + (wl > 0 ? __popc(w0) : 0) + (wl > 1 ? __popc(w1) : 0) + (wl > 2 ? __popc(w2) : 0);
+            const int ka = below + __popc(wmine & (0xffffffffu >> (31 - sh)));
+            const int kb = below + __popc(wmine & (0xffffffffu >> (30 - sh)));
+            SPH_ASSERT(ka >= kfirst && kb < ctl.n_seg);
+            const uint32_t pa = min(lo + e0, hi - 1u), pb = min(lo + e0 + 1u, hi - 1u);
+            G.j[2 * r] = ws.seg_start[ka] + (pa - ws.seg_pre[ka]);
+            G.j[2 * r + 1] = ws.seg_start[kb] + (pb - ws.seg_pre[kb]);
+            G.c[2 * r] = ldg_nc(src + G.j[2 * r]);
+            G.c[2 * r + 1] = ldg_nc(src + G.j[2 * r + 1]);
+        }
+    }
+}
+
+template <bool SQUARE_W, bool NEED_W>
+__device__ __forceinline__ void gather_store(const WalkCtl &ctl, GatherRegs &G, float4 *slotp, uint32_t *gidx, float L)
+{
+    const int lane = threadIdx.x & 31;
+    __syncwarp(); // every lane is done reading the slot's previous contents
+    const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // warp-uniform
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+        const int pr = lane + 32 * r;
+        if (pr < SPH_CH / 2) {
+            float4 ca = G.c[2 * r], cb = G.c[2 * r + 1];
+            const uint32_t e0 = 2u * pr;
+            if (G.lo + e0 >= G.hi) ca.x = SPH_NANF;
+            if (G.lo + e0 + 1u >= G.hi) cb.x = SPH_NANF;
+            if (rec) {
+                ca.x = recentre(ca.x, ctl.thx, L); ca.y = recentre(ca.y, ctl.thy, L); ca.z = recentre(ca.z, ctl.thz, L);
+                cb.x = recentre(cb.x, ctl.thx, L); cb.y = recentre(cb.y, ctl.thy, L); cb.z = recentre(cb.z, ctl.thz, L);
+            }
+            if (SQUARE_W) { ca.w *= ca.w; cb.w *= cb.w; }
+            slotp[pr] = make_float4(ca.x, cb.x, ca.y, cb.y);
+            if (NEED_W) slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, ca.w, cb.w);
+            else slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, 0.f, 0.f); // w is never read: its registers are free during the tests
+            if (gidx) reinterpret_cast<uint2 *>(gidx)[pr] = make_uint2(G.j[2 * r], G.j[2 * r + 1]);
+        }
+    }
+    __syncwarp();
+}
+
 // Lane layout of a group of g actives: lane = a + g * s with a < g the active and s < f the candidate
 // stream; f is the largest divisor of SPH_CH / 2 (candidate pairs per chunk) with g * f <= 32, so that
 // every chunk splits evenly over the streams.
