@@ -206,7 +206,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
 }
 
 template <int KERNEL>
-__global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
+__global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -276,12 +276,23 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_force(ForceArgs a)
                 const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
                 GatherCtl gc;
                 gc.kseg = 0;
+#ifdef SPH_GATHER_PIPE_FORCE
+                GatherRegs G;
+                if (nch) gather_load(W.ws, ctl, gc, 0, G, a.xyzh);
+                for (uint32_t c = 0; c < nch; c++) {
+                    gather_store<true, true>(ctl, G, W.slot, W.gidx, L);
+                    if (c + 1 < nch) gather_load(W.ws, ctl, gc, c + 1, G, a.xyzh);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                }
+#else
                 // (the register-staged gather pipeline of the density kernel measured slower here: 85.8 vs 76.3 ms)
                 for (uint32_t c = 0; c < nch; c++) {
                     gather_chunk<true>(W.ws, ctl, gc, c, W.slot, W.gidx, a.xyzh, L);
                     if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                     else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                 }
+#endif
             } while (ctl.sp > 0);
             drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
             // cross-stream totals

@@ -21,7 +21,9 @@
 #endif
 #define SPH_MAXB 32         // max actives per group (a warp: one lane per active and stream)
 #define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)
+#ifndef SPH_WARPS
 #define SPH_WARPS 4         // warps per CTA of the gather kernels (warps are independent)
+#endif
 #define SPH_THREADS (32 * SPH_WARPS)
 #ifndef SPH_CTAS
 #define SPH_CTAS 5          // resident CTAs per SM the gather kernels are compiled for (register budget)
@@ -30,6 +32,9 @@
 #define SPH_STK 192         // walk stack entries (blocks of 8 sibling nodes, per warp)
 #define SPH_STK4 48         // 4-block pops only while the stack is at most this deep
 #define SPH_CH 120          // candidates per chunk (60 pairs: divisible by 1..6, 10, 12, 15, 20, 30)
+#ifndef SPH_CTAS_FORCE
+#define SPH_CTAS_FORCE SPH_CTAS
+#endif
 #ifndef SPH_QCAP
 #define SPH_QCAP 32         // per-lane hit-queue entries (>= 2 * SPH_QSTEP)
 #endif
