@@ -17,7 +17,7 @@ namespace {
 struct ForceArgs {
     const SphNode *nodes;
     const float *node_hmax;
-    const float4 *xyzh, *vc, *raf; // sorted: (x,y,z,H) (vx,vy,vz,c) (rho, A, m, 1/H)
+    const float4 *xyzh, *vc; // sorted: (x,y,z,H); 32-byte records (vx,vy,vz,c | rho, A, m, 1/H) at vc[2j], vc[2j+1]
     const uint32_t *perm;
     const uint32_t *gstart;
     const unsigned int *n_groups;
@@ -102,7 +102,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
     for (int k = 0; k < n; k++) {
         if (k < m) {
             const uint32_t j = qp[(base + k) * 32];
-            const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + j), P2 = __ldg(a.raf + j);
+            const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + 2 * (size_t)j), P2 = __ldg(a.vc + 2 * (size_t)j + 1);
             float dx, dy, dz;
             if (WRAP == 2) {
                 dx = image_diff(A.xi, P0.x, L); dy = image_diff(A.yi, P0.y, L); dz = image_diff(A.zi, P0.z, L);
@@ -235,7 +235,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
         ForceLane A;
         {
             const uint32_t slot = a.item_slot ? a.item_slot[i0 + ai] : i0 + ai;
-            const float4 p0 = a.xyzh[slot], p1 = a.vc[slot], p2 = a.raf[slot];
+            const float4 p0 = a.xyzh[slot], p1 = a.vc[2 * (size_t)slot], p2 = a.vc[2 * (size_t)slot + 1];
             A.slot = slot;
             A.xi = live ? p0.x : SPH_NANF; // dead lanes never hit
             A.yi = p0.y; A.zi = p0.z;
@@ -334,7 +334,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
 __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const float4 *__restrict__ xyzm,
                              const float *__restrict__ vel, const float *__restrict__ u, const float *__restrict__ h,
                              const float *__restrict__ rho, const float *__restrict__ omega, float gamma,
-                             float4 *__restrict__ xyzh, float4 *__restrict__ vc, float4 *__restrict__ raf)
+                             float4 *__restrict__ xyzh, float4 *__restrict__ vc)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -344,8 +344,8 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
     float c = sqrtf(gamma * (gamma - 1.f) * ui);
     float A = (gamma - 1.f) * ui / (omega[id] * ri); // P/(Omega rho^2), P = (gamma-1) rho u
     xyzh[i] = make_float4(p.x, p.y, p.z, h[id]);
-    vc[i] = make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c);
-    raf[i] = make_float4(ri, A, p.w, 1.f / h[id]);
+    vc[2 * i] = make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c);
+    vc[2 * i + 1] = make_float4(ri, A, p.w, 1.f / h[id]);
 }
 
 // largest support radius inside every octree node: leaves scan their particles, then push the value
@@ -396,7 +396,7 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     const int T = 256;
     cudaEventRecord(ctx->ev[4], st);
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
-                                                       ctx->f_xyzh, ctx->f_vc, ctx->f_raf);
+                                                       ctx->f_xyzh, ctx->f_vc);
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->node_hmax, 0, sizeof(float) * ctx->n_nodes, st));
     k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
     sph_reset_counters(ctx, 1, subset);
@@ -407,7 +407,7 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     ForceArgs a;
     a.nodes = ctx->nodes;
     a.node_hmax = ctx->node_hmax;
-    a.xyzh = ctx->f_xyzh; a.vc = ctx->f_vc; a.raf = ctx->f_raf;
+    a.xyzh = ctx->f_xyzh; a.vc = ctx->f_vc;
     a.perm = ctx->perm;
     a.gstart = subset ? ctx->agrp_start : ctx->grp_start;
     a.n_groups = subset ? &ctx->cnt->n_agroups : &ctx->cnt->n_groups;
