@@ -416,7 +416,8 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
                         double gs = 1.0 / (1.0 - D / (3.0 * S));
                         if (!(gs > 0.0 && gs < 4.0) || N == 0.0) gs = 1.0;
                         const double smin = 0.79370052598409973738, smax = 1.25992104989487316476;
-                        double sc = (N == 0.0) ? smax : 1.0 - (N - nt) / (3.0 * N) * gs;
+                        // Newton step on ln N(ln H): d ln N / d ln H = 3 / gs  (R7)
+                        double sc = (N == 0.0) ? smax : pow(nt / N, gs / 3.0);
                         sc = fmin(fmax(sc, smin), smax);
                         Hn = H * sc;
                         if (br && !(lo < Hn && Hn < hi)) Hn = cbrt(0.5 * (lo * lo * lo + hi * hi * hi));
