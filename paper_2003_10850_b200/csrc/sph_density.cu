@@ -78,11 +78,11 @@ __device__ __forceinline__ void kern_wd2(float2 u, float2 &w, float2 &d)
 }
 
 // per-CTA shared memory
-#define SPH_DSLOTS (SPH_DCAP + SPH_PILE_SLACK + 16) // stored slots incl. the rounding of the pile map and the all-NaN quad
+#define SPH_DSLOTS (SPH_DCAP + 16) // stored slots incl. the ragged tail and the all-NaN quad
 template <bool HAS_MASS>
 struct DensCta {
-    // the staged candidates, component-wise, in the batch's frame and in pile order (sph_warp.cuh); slots
-    // that hold no candidate and the whole quad after the last one are NaN (every comparison with NaN is false)
+    // the staged candidates, component-wise, in the batch's frame; the ragged tail of the last quad and the
+    // whole quad after it are NaN (every comparison with NaN is false)
     alignas(16) float X[SPH_DSLOTS];
     alignas(16) float Y[SPH_DSLOTS];
     alignas(16) float Z[SPH_DSLOTS];
@@ -100,6 +100,7 @@ struct DensCta {
     int listed;                              // W holds the group's complete segment list (one batch)
     int resident;                            // ... and the arrays hold all of its candidates (one chunk)
     int reuse;                               // this evaluation reuses the list
+    unsigned int nstaged;                    // candidates in the arrays
     int n_u;
     unsigned int gnext;
 };
@@ -228,44 +229,57 @@ __device__ __forceinline__ void consume(const DensCta<HAS_MASS> &C, DensLane &A,
 }
 
 // Stage the candidates [lo, lo + cnt) of the walk batch's flat index space (segment k covers
-// [seg_pre[k], seg_pre[k+1])) in the component arrays.  Warp w copies a quarter of the range, 32
+// [seg_pre[k], seg_pre[k+1])) in the component arrays.  Warp w reads a quarter of the range, 32
 // consecutive positions at a time (coalesced 16-byte loads): the segments that begin inside the window
 // become bits of a warp-uniform mask, the segment of a position is a population count.  Candidates are
-// moved into the batch's frame (recentre: exact) and stored in pile order.
+// moved into the batch's frame (recentre: exact).  The walk prunes cell by cell, so most of what it
+// lists lies in the corners of cells that merely touch the group's reach: a candidate is staged only if
+// it lies within the walk's reach of the group's bounding box itself (one point-to-box distance per
+// candidate, instead of one distance test per candidate and ACTIVE later); the survivors are packed in
+// arrival order (a ballot, a population count and one shared-memory atomic per window).
 template <bool HAS_MASS>
 __device__ __forceinline__ void gather_chunk(DensCta<HAS_MASS> &C, const WalkCtl &ctl, uint32_t lo, uint32_t cnt,
-                                             const PileMap &pm, const float4 *__restrict__ src, float L)
+                                             const float4 *__restrict__ src, float L)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const WalkShared &W = C.W;
     const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // CTA-uniform
+    // the group's box in the batch's frame (a group lies inside one octree cell below the root, i.e. on one
+    // side of L/2 on every axis; if it does not -- a root-level group of a tiny set -- nothing is filtered)
+    const float hl = 0.5f * L;
+    const bool strad = (W.box[0] - W.box[3] < hl && W.box[0] + W.box[3] >= hl) || (W.box[1] - W.box[4] < hl && W.box[1] + W.box[4] >= hl) ||
+                       (W.box[2] - W.box[5] < hl && W.box[2] + W.box[5] >= hl);
+    const bool filt = !ctl.pairwrap && !(rec && strad);
+    const float bx = rec ? recentre(W.box[0], ctl.thx, L) : W.box[0], by = rec ? recentre(W.box[1], ctl.thy, L) : W.box[1];
+    const float bz = rec ? recentre(W.box[2], ctl.thz, L) : W.box[2];
+    const float ex = W.box[3], ey = W.box[4], ez = W.box[5];
+    const float lim = filt ? W.box[6] * W.box[6] * (1.f + 1e-5f) : __int_as_float(0x7f800000);
     const uint32_t per = (((cnt + SPH_WARPS - 1) / SPH_WARPS) + 31u) & ~31u; // positions per warp, whole windows
     const uint32_t b0 = lo + min(cnt, warp * per), b1 = lo + min(cnt, (warp + 1) * per);
     int kb = seg_of(W, ctl.n_seg, b0); // warp-uniform
     for (uint32_t base = b0; base < b1; base += 32) {
         const uint32_t p = base + lane;
         const int ks = kb + 1 + lane;
-        const uint32_t pre = ks < ctl.n_seg ? W.seg_pre[ks] : 0xffffffffu; // > base: kb is the last segment that begins at or before base
+        const uint32_t pre = ks < ctl.n_seg ? W.seg_pre[ks] : 0xffffffffu; // >= base: kb is the last segment that begins at or before base
         const unsigned mask = __reduce_or_sync(FULLMASK, pre < base + 32u ? 1u << (pre - base) : 0u);
         const int k = kb + __popc(mask & (0xffffffffu >> (31 - lane)));
         kb += __popc(mask);
+        bool keep = false;
+        float4 c = make_float4(0.f, 0.f, 0.f, 0.f);
         if (p < b1) {
-            float4 c = ldg_nc(src + (W.seg_start[k] + (p - W.seg_pre[k])));
+            c = ldg_nc(src + (W.seg_start[k] + (p - W.seg_pre[k])));
             if (rec) { c.x = recentre(c.x, ctl.thx, L); c.y = recentre(c.y, ctl.thy, L); c.z = recentre(c.z, ctl.thz, L); }
-            const uint32_t o = pile_slot(pm, p - lo);
+            const float dx = fmaxf(fabsf(c.x - bx) - ex, 0.f), dy = fmaxf(fabsf(c.y - by) - ey, 0.f), dz = fmaxf(fabsf(c.z - bz) - ez, 0.f);
+            keep = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) <= lim;
+        }
+        const unsigned mk = __ballot_sync(FULLMASK, keep);
+        unsigned int o = 0;
+        if (lane == 0 && mk) o = atomicAdd(&C.nstaged, (unsigned int)__popc(mk));
+        o = __shfl_sync(FULLMASK, o, 0) + __popc(mk & lanemask_lt());
+        if (keep) {
             C.X[o] = c.x; C.Y[o] = c.y; C.Z[o] = c.z;
             if (HAS_MASS) C.M[o] = c.w;
         }
-    }
-    // slots of the pile map that hold no candidate, and the quad after the last one
-    for (uint32_t o = cnt + tid; o < pm.np; o += SPH_THREADS) {
-        const uint32_t sl = pile_slot(pm, o);
-        C.X[sl] = SPH_NANF; C.Y[sl] = 0.f; C.Z[sl] = 0.f;
-        if (HAS_MASS) C.M[sl] = 0.f;
-    }
-    if (tid < 4) {
-        C.X[pm.np + tid] = SPH_NANF; C.Y[pm.np + tid] = 0.f; C.Z[pm.np + tid] = 0.f;
-        if (HAS_MASS) C.M[pm.np + tid] = 0.f;
     }
 }
 
@@ -318,7 +332,6 @@ __device__ __forceinline__ void evaluate(DensCta<HAS_MASS> &C, const DensArgs &a
     bool first = true, onechunk = false;
     for (;;) {
         const WalkCtl ctl = walk_result(C.W);
-        cands += ctl.total;
         // this thread's active in the batch's frame
         A.nx = f2(-(ctl.pairwrap ? A.xi : recentre(A.xi, ctl.thx, L)));
         A.ny = f2(-(ctl.pairwrap ? A.yi : recentre(A.yi, ctl.thy, L)));
@@ -327,13 +340,22 @@ __device__ __forceinline__ void evaluate(DensCta<HAS_MASS> &C, const DensArgs &a
         const bool keep = reuse && C.resident; // the candidates themselves are still staged
         for (uint32_t c = 0; c < nch; c++) {
             const uint32_t lo = c * SPH_DCAP, cnt = min((uint32_t)SPH_DCAP, ctl.total - lo);
-            const PileMap pm = pile_map(cnt);
             if (!keep) {
-                gather_chunk<HAS_MASS>(C, ctl, lo, cnt, pm, a.xyzm, L);
-                staged += cnt;
+                if (tid == 0) C.nstaged = 0;
                 __syncthreads();
+                gather_chunk<HAS_MASS>(C, ctl, lo, cnt, a.xyzm, L);
+                __syncthreads();
+                const uint32_t ns = C.nstaged;
+                if (tid < 8) { // the ragged tail of the last quad and the quad after it
+                    C.X[ns + tid] = SPH_NANF; C.Y[ns + tid] = 0.f; C.Z[ns + tid] = 0.f;
+                    if (HAS_MASS) C.M[ns + tid] = 0.f;
+                }
+                __syncthreads();
+                staged += cnt;
             }
-            const int nq = (int)(pm.np >> 2);
+            const uint32_t ns = C.nstaged;
+            cands += ns;
+            const int nq = (int)((ns + 3u) >> 2);
             if (ctl.pairwrap) consume<KERNEL, HAS_MASS, true>(C, A, nq, s, f, live, L);
             else consume<KERNEL, HAS_MASS, false>(C, A, nq, s, f, live, L);
             if (c + 1 < nch || ctl.sp > 0) __syncthreads(); // the arrays are about to be overwritten
