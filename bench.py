@@ -381,9 +381,6 @@ def main():
                       "force_true_pairs": st["force_pairs"], "force_candidates": st["force_candidates"],
                       "pair_interactions_per_s": (st["dens_pairs"] + st["force_pairs"]) * world / (ms / args.steps * 1e-3),
                       "unconverged": per[-1]["unconv"],
-                      "groups": st["n_groups"], "density_group_evals": st["dens_group_evals"],
-                      "density_walks": st["dens_walks"], "density_staged": st["dens_staged"],
-                      "force_staged": st["force_staged"],
                       "density_eval_histogram": {str(k): int(v) for k, v in enumerate(eval_hist) if v},
                       "updates_per_s_without_index": world * n_active / ((ms / args.steps - ti) * 1e-3)},
         }

@@ -85,11 +85,6 @@ typedef struct {
     float t_density_kernel_ms; /* the persistent gather + h-iteration kernel alone (a6-a9) */
     float t_force_prep_ms;     /* sorted force state + per-node max H (a9/a4 refresh) */
     float t_force_kernel_ms;   /* the hydro-force gather kernel alone (a10-a11) */
-    /* how the last sph_density / sph_hydro_force calls spent their work */
-    int64_t dens_group_evals;  /* evaluations of a group (all its still-iterating particles at once) */
-    int64_t dens_walks;        /* octree walks (an evaluation whose reach has not grown reuses the last one) */
-    int64_t dens_staged;       /* candidates copied into shared memory */
-    int64_t force_staged;
 } sph_stats;
 
 /* Create a context. `cuda_stream` is a cudaStream_t (NULL = legacy default stream). */

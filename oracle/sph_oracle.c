@@ -362,6 +362,7 @@ int orc_density(const orc_params *p, int64_t n, const float *pos, const float *m
 typedef struct {
     double a[3], du, vsig;
     double asum, dusum; /* sums of |pair term| for the parity tolerance floor (R15) */
+    double asq, dusq;   /* sums of (pair term)^2: the fp32 resolution of the sum (R15), test-side only */
     double duvisc;      /* viscous part of du/dt (pin: >= 0) */
     int64_t npair;
     int edge;
@@ -411,9 +412,11 @@ static inline void force_pair(const force_ctx *c, int64_t i, int64_t j, force_ac
     double t = mj * (Ai * Fi + Aj * Fj + Pi * Fbar);
     for (int a = 0; a < 3; a++) f->a[a] -= t * rh[a];
     f->asum += fabs(t);
+    f->asq += t * t;
     double e = mj * (Ai * Fi + 0.5 * Pi * Fbar) * vr;
     f->du += e;
     f->dusum += fabs(e);
+    f->dusq += e * e;
     f->duvisc += mj * 0.5 * Pi * Fbar * vr;
     if (vs > f->vsig) f->vsig = vs;
 }
@@ -422,7 +425,7 @@ int orc_hydro_force(const orc_params *p, int64_t n, const float *pos, const floa
                     const float *mass, double mass_scalar, const float *h, const float *rho, const float *omega,
                     const int32_t *active, int64_t n_active, int brute, double cell_hint,
                     double *acc, double *dudt, double *vsig, double *asum, double *dusum, double *duvisc,
-                    int64_t *npair, uint8_t *edge)
+                    int64_t *npair, uint8_t *edge, double *asq, double *dusq)
 {
     orc_grid *g = brute ? NULL : grid_build(n, pos, p->box, cell_hint, h);
     force_ctx c = {p, n, pos, vel, u, mass, h, rho, omega, mass_scalar};
@@ -460,6 +463,8 @@ int orc_hydro_force(const orc_params *p, int64_t n, const float *pos, const floa
         if (asum) asum[a] = f.asum;
         if (dusum) dusum[a] = f.dusum;
         if (duvisc) duvisc[a] = f.duvisc;
+        if (asq) asq[a] = f.asq;
+        if (dusq) dusq[a] = f.dusq;
         if (npair) npair[a] = f.npair;
         if (edge) edge[a] = (uint8_t)(f.edge ? ORC_E_RADIUS : 0);
     }

@@ -144,7 +144,8 @@ def density(pos, h_guess, *, kernel, n_target, n_tol, box=1.0, mass=None, mass_s
 
 def hydro_force(pos, vel, u, h, rho, omega, *, kernel, box=1.0, gamma=5.0 / 3.0, alpha=1.0, mass=None,
                 mass_scalar=1.0, active=None, brute=False, cell_hint=None):
-    """Symmetric hydro-force pair sum. Returns dict: acc (na,3), dudt, vsig, asum, dusum, duvisc (fp64), npair (int64), edge."""
+    """Symmetric hydro-force pair sum. Returns dict: acc (na,3), dudt, vsig, asum, dusum, duvisc, asq, dusq (fp64),
+    npair (int64), edge.  asum/dusum are the sums of |pair term|, asq/dusq of (pair term)^2 (tolerances, R15)."""
     pos_, ppos = _p(pos, np.float32)
     vel_, pvel = _p(vel, np.float32)
     u_, pu = _p(u, np.float32)
@@ -156,7 +157,7 @@ def hydro_force(pos, vel, u, h, rho, omega, *, kernel, box=1.0, gamma=5.0 / 3.0,
     n = pos_.shape[0]
     na = n if act_ is None else act_.shape[0]
     out = {"acc": np.zeros((na, 3), np.float64)}
-    for k in ("dudt", "vsig", "asum", "dusum", "duvisc"):
+    for k in ("dudt", "vsig", "asum", "dusum", "duvisc", "asq", "dusq"):
         out[k] = np.zeros(na, np.float64)
     out["npair"] = np.zeros(na, np.int64)
     out["edge"] = np.zeros(na, np.uint8)
@@ -165,7 +166,7 @@ def hydro_force(pos, vel, u, h, rho, omega, *, kernel, box=1.0, gamma=5.0 / 3.0,
         cell_hint = float(np.median(h_)) if n else box
     lib().orc_hydro_force(C.byref(prm), C.c_int64(n), ppos, pvel, pu, pm, C.c_double(mass_scalar), ph, prho, pom,
                           pact, C.c_int64(na), C.c_int(int(brute)), C.c_double(cell_hint),
-                          *[out[k].ctypes.data_as(C.c_void_p) for k in ("acc", "dudt", "vsig", "asum", "dusum", "duvisc", "npair", "edge")])
+                          *[out[k].ctypes.data_as(C.c_void_p) for k in ("acc", "dudt", "vsig", "asum", "dusum", "duvisc", "npair", "edge", "asq", "dusq")])
     return out
 
 

@@ -30,8 +30,7 @@ class SphParams(C.Structure):
 class SphStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n", "n_nodes", "n_groups", "launches", "dens_evals", "dens_candidates",
                                          "dens_pairs", "force_candidates", "force_pairs")] + \
-               [(k, C.c_float) for k in ("t_index_ms", "t_density_kernel_ms", "t_force_prep_ms", "t_force_kernel_ms")] + \
-               [(k, C.c_int64) for k in ("dens_group_evals", "dens_walks", "dens_staged", "force_staged")]
+               [(k, C.c_float) for k in ("t_index_ms", "t_density_kernel_ms", "t_force_prep_ms", "t_force_kernel_ms")]
 
 
 class SphError(RuntimeError):

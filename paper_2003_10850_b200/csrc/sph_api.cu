@@ -58,7 +58,7 @@ int sph_create(sph_ctx **out, const sph_params *p, void *cuda_stream)
     if (!ctx) return SPH_E_OOM;
     ctx->prm = *p;
     ctx->grp_cap = p->group_cap ? p->group_cap : SPH_GCAP_DEFAULT;
-    ctx->grp_node = p->group_node > 0 ? p->group_node : (p->group_cap ? 2 * ctx->grp_cap : SPH_GNODE_DEFAULT);
+    ctx->grp_node = p->group_node > 0 ? p->group_node : 2 * ctx->grp_cap;
     ctx->stream = (cudaStream_t)cuda_stream;
     int dev = 0;
     cudaDeviceProp prop;
@@ -236,19 +236,11 @@ int sph_get_stats(sph_ctx *ctx, sph_stats *out)
     SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (h.bad_ids)
         return sph_fail(ctx, SPH_E_ARG, "%u active ids outside [0, n) in the last call: nothing was computed", h.bad_ids);
-#ifdef SPH_DIAG
-    fprintf(stderr, "diag evals<2: max*live %u sum %u max*32 %u | later: %u %u %u\n", h.lvl_begin[0], h.lvl_done[0], h.lvl_begin[1],
-            h.lvl_begin[2], h.lvl_done[2], h.lvl_begin[3]);
-#endif
     out->dens_evals = (int64_t)h.dens_evals;
     out->dens_candidates = (int64_t)h.dens_cands;
     out->dens_pairs = (int64_t)h.dens_pairs;
     out->force_candidates = (int64_t)h.force_cands;
     out->force_pairs = (int64_t)h.force_pairs;
-    out->dens_group_evals = (int64_t)h.dens_group_evals;
-    out->dens_walks = (int64_t)h.dens_walks;
-    out->dens_staged = (int64_t)h.dens_staged;
-    out->force_staged = (int64_t)h.force_staged;
     float *t[4] = {&out->t_index_ms, &out->t_density_kernel_ms, &out->t_force_prep_ms, &out->t_force_kernel_ms};
     for (int i = 0; i < 4; i++)
         if (ctx->ev_set[i] && cudaEventElapsedTime(t[i], ctx->ev[2 * i], ctx->ev[2 * i + 1]) != cudaSuccess) {

@@ -6,14 +6,13 @@
 // "performs a tree walk and neighbour interactions in chunks" of N_chunk = 32 (§2.4);
 // formulas: DESIGN.md readings R1-R7.
 //
-// Mapping: one CTA (4 warps) per group of g <= 32 active particles.  Thread =
-// (active a, stream s): the f = 128/g streams split the candidate quads, threads of one stream read the
-// same quad (shared-memory broadcast).  Warp 0 walks the octree once for the group; all warps stage the
-// candidate runs it found in shared memory as component arrays X[], Y[], Z[] (in the group's periodic
-// frame), where they STAY for every evaluation of the h iteration whose reach they cover.  Each thread
-// tests four candidates per step in packed f32x2 against its own active and pushes r^2 of a hit onto
-// its private queue; queued hits are evaluated in bulk so the kernel polynomial runs on converged
-// warps.  No atomics on the pair path.
+// Mapping: one warp per group of g <= 32 active particles.  Lane = (active a,
+// stream s): the f ~ 32/g streams split every chunk of candidate pairs, lanes of one stream read the
+// same pair record (shared-memory broadcast).  The warp gathers the candidate segments found by the
+// walk, chunk by chunk, into its shared-memory slot (sph_warp.cuh); each lane tests two candidates per
+// step in packed f32x2 against its own active and pushes r^2 of a hit onto its private queue; queued
+// hits are evaluated in bulk so the kernel polynomial runs on converged warps.  No block-level
+// barrier, no atomics on the pair path.
 #include "sph_warp.cuh"
 
 namespace {
@@ -77,45 +76,37 @@ __device__ __forceinline__ void kern_wd2(float2 u, float2 &w, float2 &d)
     }
 }
 
-// per-CTA shared memory
-#define SPH_DSLOTS (SPH_DCAP + 16) // stored slots incl. the ragged tail and the all-NaN quad
+// per-warp shared memory
 template <bool HAS_MASS>
-struct DensCta {
-    // the staged candidates, component-wise, in the batch's frame; the ragged tail of the last quad and the
-    // whole quad after it are NaN (every comparison with NaN is false)
-    alignas(16) float X[SPH_DSLOTS];
-    alignas(16) float Y[SPH_DSLOTS];
-    alignas(16) float Z[SPH_DSLOTS];
-    alignas(16) float M[HAS_MASS ? SPH_DSLOTS : 4];
-    // hit queues: entry k of thread t at [k * SPH_THREADS + t] (r^2); reused for the cross-stream totals
-    alignas(16) float q[SPH_QCAP * SPH_THREADS];
-    float qm[HAS_MASS ? SPH_QCAP * SPH_THREADS : 4]; // mass of the hit
-    WalkShared W;
+struct DensWarp {
+    float4 slot[SPH_CH];                     // one chunk of candidates as pair records
+    WarpWalk ws;
+    float q[SPH_NA * SPH_QCAP * 32];         // hit queues: entry k of lane l, active q of the lane, at [(q * QCAP + k) * 32 + l] (r^2)
+    float qm[HAS_MASS ? SPH_NA * SPH_QCAP * 32 : 32]; // mass of the hit
     double lo[SPH_MAXB], hi[SPH_MAXB];       // bracket of the h iteration (R7)
     float ax[SPH_MAXB], ay[SPH_MAXB], az[SPH_MAXB], aH[SPH_MAXB];
     uint32_t aid[SPH_MAXB];
     int it[SPH_MAXB];
     int ulist[SPH_MAXB];                     // actives still iterating
-    float walk_hg;                           // reach the segment list was walked with
-    int listed;                              // W holds the group's complete segment list (one batch)
-    int resident;                            // ... and the arrays hold all of its candidates (one chunk)
-    int reuse;                               // this evaluation reuses the list
-    unsigned int nstaged;                    // candidates in the arrays
-    int n_u;
-    unsigned int gnext;
 };
 
-#define SPH_QSTRIDE (4u * SPH_THREADS) // bytes between consecutive queue entries of a thread
-
-// Per-thread state of one evaluation: thread = (active a, candidate stream s).
-struct DensLane {
+// Per-lane state of one evaluation.  A lane is (active slot ap, candidate stream s) and holds SPH_NA
+// actives (2 ap, 2 ap + 1): every pair record loaded from shared memory is tested against all of them,
+// which halves the shared-memory reads and the loop overhead per test.
+struct DensAct {         // one active of the lane
     float2 s, ds, r, dr; // packed partial sums: sum w, sum d, sum m w, sum m d
     float2 nx, ny, nz;   // minus the active's position in the batch's frame, duplicated for f32x2
     float xi, yi, zi;    // raw position (per-pair image path)
-    float h2, ih2;       // H^2 (-1 for a dead thread: never hits), 1 / H^2
-    uint32_t q0, qw;     // this thread's hit queue: base and write cursor (shared-memory addresses)
-    uint32_t mofs;       // offset from a queue entry to its mass entry
+    float h2, ih2;       // H^2 (-1 for a missing active: never hits), 1 / H^2
+    uint32_t q0, qw;     // this active's hit queue in this lane: base and write cursor (shared-memory addresses, stride 128 B)
     int cn;              // hits evaluated so far
+};
+struct DensLane {
+    DensAct act[SPH_NA];
+    uint32_t mofs;       // offset from a queue entry to its mass entry
+    const float4 *cp;    // this stream's first pair record of the chunk
+    int cstride;         // float4 elements between consecutive pair records of this stream (f)
+    int steps;           // pair records per chunk for this stream (SPH_CH / 2 / f)
 };
 
 __device__ __forceinline__ float lds_f32(uint32_t addr)
@@ -125,21 +116,21 @@ __device__ __forceinline__ float lds_f32(uint32_t addr)
     return v;
 }
 
-// Evaluate the newest min(n, queued) hits of every thread of the warp, two per step, without branches:
-// a thread that runs out of entries evaluates u = 1, where w = d = 0 exactly (n is warp-uniform).
+// Evaluate the newest min(n, queued) hits of one active of every lane, two per step, without branches:
+// a lane that runs out of entries evaluates u = 1, where w = d = 0 exactly (n is warp-uniform).
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void drain(DensLane &A, int n)
+__device__ __forceinline__ void drain(DensAct &A, uint32_t mofs, int n)
 {
-    const int m = min(n, (int)((A.qw - A.q0) / SPH_QSTRIDE));
+    const int m = min(n, (int)((A.qw - A.q0) >> 7));
     const uint32_t end = A.qw;
-    uint32_t ra = end - (uint32_t)m * SPH_QSTRIDE;
+    uint32_t ra = end - (uint32_t)m * 128u;
     A.qw = ra;
     A.cn += m;
     const float2 ih22 = f2(A.ih2);
 #pragma unroll 2
-    for (int k = 0; k < n; k += 2, ra += 2u * SPH_QSTRIDE) {
-        const bool v0 = ra < end, v1 = ra + SPH_QSTRIDE < end;
-        const float r0 = v0 ? lds_f32(ra) : 0.f, r1 = v1 ? lds_f32(ra + SPH_QSTRIDE) : 0.f;
+    for (int k = 0; k < n; k += 2, ra += 256u) {
+        const bool v0 = ra < end, v1 = ra + 128u < end;
+        const float r0 = v0 ? lds_f32(ra) : 0.f, r1 = v1 ? lds_f32(ra + 128u) : 0.f;
         float2 u = __fmul2_rn(f2(r0, r1), ih22);
         u.x = v0 ? u.x : 1.f;
         u.y = v1 ? u.y : 1.f;
@@ -148,389 +139,334 @@ __device__ __forceinline__ void drain(DensLane &A, int n)
         A.s = __fadd2_rn(A.s, w);
         A.ds = __fadd2_rn(A.ds, d);
         if (HAS_MASS) {
-            const float2 mj = f2(v0 ? lds_f32(ra + A.mofs) : 0.f, v1 ? lds_f32(ra + SPH_QSTRIDE + A.mofs) : 0.f);
+            const float2 mj = f2(v0 ? lds_f32(ra + mofs) : 0.f, v1 ? lds_f32(ra + 128u + mofs) : 0.f);
             A.r = __ffma2_rn(mj, w, A.r);
             A.dr = __ffma2_rn(mj, d, A.dr);
         }
     }
 }
 
-// queue capacity: room for `need` more hits in every thread of the warp, else evaluate queued hits first.
-// Only as many as the emptiest live queue holds (every lane busy), unless more room is needed.
+// queue capacity: room for `need` more hits of this active in every lane, else evaluate queued hits first
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void make_room(DensLane &A, bool live, int need)
+__device__ __forceinline__ void make_room(DensAct &A, uint32_t mofs, bool live, int need)
 {
-    const int cnt = (int)((A.qw - A.q0) / SPH_QSTRIDE);
+    const int cnt = (int)((A.qw - A.q0) >> 7);
     const int mx = __reduce_max_sync(FULLMASK, cnt);
     if (mx + need > SPH_QCAP) {
         const int mn = __reduce_min_sync(FULLMASK, live ? cnt : 0x7fffffff);
-        drain<KERNEL, HAS_MASS>(A, max(min(mn, mx), mx + need - SPH_QCAP));
+        drain<KERNEL, HAS_MASS>(A, mofs, max(mn, mx + need - SPH_QCAP));
     }
 }
 
-// one candidate against this thread's active: a hit pushes r^2 (and the mass) onto the queue
-template <bool HAS_MASS>
-__device__ __forceinline__ void push_if(const DensLane &A, uint32_t &qw, float r2, float m)
-{
-    if (r2 < A.h2) {
-        sts_f32(qw, r2);
-        if (HAS_MASS) sts_f32(qw + A.mofs, m);
-        qw += SPH_QSTRIDE;
-    }
-}
-
-// Test the nq candidate quads staged in shared memory against this thread's active: thread (a, s) takes
-// the quads s, s + f, s + 2f, ... (past the end: the all-NaN quad nq); the four distances of a quad come
-// out of two packed f32x2 chains.
+// Test the candidates of the gathered chunk against this lane's actives: lane (ap, s) takes the pair
+// records s, s + f, s + 2f, ...; both distances of a pair come out of one packed f32x2 chain; a hit
+// pushes r^2 (and the mass) onto the queue of the active it belongs to.
 template <int KERNEL, bool HAS_MASS, bool PAIRWRAP>
-__device__ __forceinline__ void consume(const DensCta<HAS_MASS> &C, DensLane &A, int nq, int s, int f, bool live, float L)
+__device__ __forceinline__ void consume_chunk(DensLane &A, bool live, float L)
 {
-    const float4 *X4 = reinterpret_cast<const float4 *>(C.X), *Y4 = reinterpret_cast<const float4 *>(C.Y);
-    const float4 *Z4 = reinterpret_cast<const float4 *>(C.Z), *M4 = reinterpret_cast<const float4 *>(C.M);
-    const int steps = (nq + f - 1) / f; // CTA-uniform
-    int qd = s, qi = min(qd, nq);
-    // software pipeline: the next quad is in flight while this one is tested
-    float4 nx = X4[qi], ny = Y4[qi], nz = Z4[qi], nm = HAS_MASS ? M4[qi] : make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
-        const int nt = min(SPH_QSTEP, steps - t0);
-        make_room<KERNEL, HAS_MASS>(A, live, 4 * nt);
-        uint32_t qw = A.qw;
-#pragma unroll 2
+    const float4 *cp = A.cp;
+    float4 n0 = cp[0], n1 = cp[SPH_CH / 2];
+    cp += A.cstride;
+    for (int t0 = 0; t0 < A.steps; t0 += SPH_QSTEP) {
+        const int nt = min(SPH_QSTEP, A.steps - t0);
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) make_room<KERNEL, HAS_MASS>(A.act[a], A.mofs, live, 2 * nt);
+        uint32_t qw[SPH_NA];
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) qw[a] = A.act[a].qw;
+#pragma unroll 3
         for (int t = 0; t < nt; t++) {
-            const float4 x = nx, y = ny, z = nz, m = nm;
-            qd += f;
-            qi = min(qd, nq);
-            nx = X4[qi]; ny = Y4[qi]; nz = Z4[qi];
-            if (HAS_MASS) nm = M4[qi];
-            float2 ra, rb;
-            if (PAIRWRAP) {
-                const float dx0 = image_diff(A.xi, x.x, L), dx1 = image_diff(A.xi, x.y, L);
-                const float dx2 = image_diff(A.xi, x.z, L), dx3 = image_diff(A.xi, x.w, L);
-                const float dy0 = image_diff(A.yi, y.x, L), dy1 = image_diff(A.yi, y.y, L);
-                const float dy2 = image_diff(A.yi, y.z, L), dy3 = image_diff(A.yi, y.w, L);
-                const float dz0 = image_diff(A.zi, z.x, L), dz1 = image_diff(A.zi, z.y, L);
-                const float dz2 = image_diff(A.zi, z.z, L), dz3 = image_diff(A.zi, z.w, L);
-                ra = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
-                rb = f2(fmaf(dz2, dz2, fmaf(dy2, dy2, dx2 * dx2)), fmaf(dz3, dz3, fmaf(dy3, dy3, dx3 * dx3)));
-            } else {
-                const float2 dxa = __fadd2_rn(f2(x.x, x.y), A.nx), dxb = __fadd2_rn(f2(x.z, x.w), A.nx);
-                const float2 dya = __fadd2_rn(f2(y.x, y.y), A.ny), dyb = __fadd2_rn(f2(y.z, y.w), A.ny);
-                const float2 dza = __fadd2_rn(f2(z.x, z.y), A.nz), dzb = __fadd2_rn(f2(z.z, z.w), A.nz);
-                ra = __ffma2_rn(dza, dza, __ffma2_rn(dya, dya, __fmul2_rn(dxa, dxa)));
-                rb = __ffma2_rn(dzb, dzb, __ffma2_rn(dyb, dyb, __fmul2_rn(dxb, dxb)));
+            const float4 c0 = n0, cz = n1; // (x0,x1,y0,y1) (z0,z1,w0,w1)
+            const float2 c1 = f2(cz.x, cz.y), cm = f2(cz.z, cz.w);
+            // software pipeline: the next pair record is in flight while this one is tested (past the
+            // chunk's last record this reads on inside the warp's own shared memory; the value is unused)
+            n0 = cp[0]; n1 = cp[SPH_CH / 2];
+            cp += A.cstride;
+#pragma unroll
+            for (int a = 0; a < SPH_NA; a++) {
+                const DensAct &P = A.act[a];
+                float2 r2;
+                if (PAIRWRAP) {
+                    const float dx0 = image_diff(P.xi, c0.x, L), dx1 = image_diff(P.xi, c0.y, L);
+                    const float dy0 = image_diff(P.yi, c0.z, L), dy1 = image_diff(P.yi, c0.w, L);
+                    const float dz0 = image_diff(P.zi, c1.x, L), dz1 = image_diff(P.zi, c1.y, L);
+                    r2 = f2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
+                } else {
+                    const float2 dx = __fadd2_rn(f2(c0.x, c0.y), P.nx), dy = __fadd2_rn(f2(c0.z, c0.w), P.ny);
+                    const float2 dz = __fadd2_rn(c1, P.nz);
+                    r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+                }
+                if (r2.x < P.h2) {
+                    sts_f32(qw[a], r2.x);
+                    if (HAS_MASS) sts_f32(qw[a] + A.mofs, cm.x);
+                    qw[a] += 128u;
+                }
+                if (r2.y < P.h2) {
+                    sts_f32(qw[a], r2.y);
+                    if (HAS_MASS) sts_f32(qw[a] + A.mofs, cm.y);
+                    qw[a] += 128u;
+                }
             }
-            push_if<HAS_MASS>(A, qw, ra.x, m.x);
-            push_if<HAS_MASS>(A, qw, ra.y, m.y);
-            push_if<HAS_MASS>(A, qw, rb.x, m.z);
-            push_if<HAS_MASS>(A, qw, rb.y, m.w);
         }
-        A.qw = qw;
+#pragma unroll
+        for (int a = 0; a < SPH_NA; a++) A.act[a].qw = qw[a];
     }
 }
 
-// Stage the candidates [lo, lo + cnt) of the walk batch's flat index space (segment k covers
-// [seg_pre[k], seg_pre[k+1])) in the component arrays.  Warp w reads a quarter of the range, 32
-// consecutive positions at a time (coalesced 16-byte loads): the segments that begin inside the window
-// become bits of a warp-uniform mask, the segment of a position is a population count.  Candidates are
-// moved into the batch's frame (recentre: exact).  The walk prunes cell by cell, so most of what it
-// lists lies in the corners of cells that merely touch the group's reach: a candidate is staged only if
-// it lies within the walk's reach of the group's bounding box itself (one point-to-box distance per
-// candidate, instead of one distance test per candidate and ACTIVE later); the survivors are packed in
-// arrival order (a ballot, a population count and one shared-memory atomic per window).
-template <bool HAS_MASS>
-__device__ __forceinline__ void gather_chunk(DensCta<HAS_MASS> &C, const WalkCtl &ctl, uint32_t lo, uint32_t cnt,
-                                             const float4 *__restrict__ src, float L)
-{
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const WalkShared &W = C.W;
-    const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // CTA-uniform
-    // the group's box in the batch's frame (a group lies inside one octree cell below the root, i.e. on one
-    // side of L/2 on every axis; if it does not -- a root-level group of a tiny set -- nothing is filtered)
-    const float hl = 0.5f * L;
-    const bool strad = (W.box[0] - W.box[3] < hl && W.box[0] + W.box[3] >= hl) || (W.box[1] - W.box[4] < hl && W.box[1] + W.box[4] >= hl) ||
-                       (W.box[2] - W.box[5] < hl && W.box[2] + W.box[5] >= hl);
-    const bool filt = !ctl.pairwrap && !(rec && strad);
-    const float bx = rec ? recentre(W.box[0], ctl.thx, L) : W.box[0], by = rec ? recentre(W.box[1], ctl.thy, L) : W.box[1];
-    const float bz = rec ? recentre(W.box[2], ctl.thz, L) : W.box[2];
-    const float ex = W.box[3], ey = W.box[4], ez = W.box[5];
-    const float lim = filt ? W.box[6] * W.box[6] * (1.f + 1e-5f) : __int_as_float(0x7f800000);
-    const uint32_t per = (((cnt + SPH_WARPS - 1) / SPH_WARPS) + 31u) & ~31u; // positions per warp, whole windows
-    const uint32_t b0 = lo + min(cnt, warp * per), b1 = lo + min(cnt, (warp + 1) * per);
-    int kb = seg_of(W, ctl.n_seg, b0); // warp-uniform
-    for (uint32_t base = b0; base < b1; base += 32) {
-        const uint32_t p = base + lane;
-        const int ks = kb + 1 + lane;
-        const uint32_t pre = ks < ctl.n_seg ? W.seg_pre[ks] : 0xffffffffu; // >= base: kb is the last segment that begins at or before base
-        const unsigned mask = __reduce_or_sync(FULLMASK, pre < base + 32u ? 1u << (pre - base) : 0u);
-        const int k = kb + __popc(mask & (0xffffffffu >> (31 - lane)));
-        kb += __popc(mask);
-        bool keep = false;
-        float4 c = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (p < b1) {
-            c = ldg_nc(src + (W.seg_start[k] + (p - W.seg_pre[k])));
-            if (rec) { c.x = recentre(c.x, ctl.thx, L); c.y = recentre(c.y, ctl.thy, L); c.z = recentre(c.z, ctl.thz, L); }
-            const float dx = fmaxf(fabsf(c.x - bx) - ex, 0.f), dy = fmaxf(fabsf(c.y - by) - ey, 0.f), dz = fmaxf(fabsf(c.z - bz) - ez, 0.f);
-            keep = fmaf(dz, dz, fmaf(dy, dy, dx * dx)) <= lim;
-        }
-        const unsigned mk = __ballot_sync(FULLMASK, keep);
-        unsigned int o = 0;
-        if (lane == 0 && mk) o = atomicAdd(&C.nstaged, (unsigned int)__popc(mk));
-        o = __shfl_sync(FULLMASK, o, 0) + __popc(mk & lanemask_lt());
-        if (keep) {
-            C.X[o] = c.x; C.Y[o] = c.y; C.Z[o] = c.z;
-            if (HAS_MASS) C.M[o] = c.w;
-        }
-    }
-}
+// what evaluate() keeps from one evaluation of a group to the next (warp-uniform registers)
+struct WalkCache {
+    WalkCtl ctl;
+    float hg;    // reach the list was walked with
+    bool valid;  // the list in shared memory is complete and reusable
+    bool multi;  // scratch: a batch of the current walk has already been seen
+};
 
-// One evaluation of the group's g iterating actives at their current H: walk (or reuse of the resident
-// set), gather, test, evaluate.  Returns the totals of the i-th iterating active in thread i (i < g).
+// One evaluation of the group's g iterating actives at their current H: walk, gather, test, evaluate.
+// Returns the totals of the i-th iterating active in lane i (i < g).
 template <int KERNEL, bool HAS_MASS>
-__device__ __forceinline__ void evaluate(DensCta<HAS_MASS> &C, const DensArgs &a, int g, int evalno, double &S, double &D,
-                                         double &R, double &DR, int &nint, unsigned long long &cands, unsigned long long &staged, unsigned int &walks)
+__device__ __forceinline__ void evaluate(DensWarp<HAS_MASS> &W, const DensArgs &a, int g, WalkCache &wc, double &S,
+                                         double &D, double &R, double &DR, int &nint, unsigned long long &cands)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lane = threadIdx.x & 31;
     const float L = a.L;
-    const int f = streams_for(g);
-    const bool live = tid < g * f;
-    const int ai = live ? tid % g : 0, s = live ? tid / g : 0;
+    const int gp = (g + SPH_NA - 1) / SPH_NA; // active slots: lane = ap + gp * s
+    const int f = streams_for(gp);
+    const bool live = lane < gp * f;
+    const int ap = live ? lane % gp : 0, s = live ? lane / gp : 0;
     const float inf = __int_as_float(0x7f800000);
 
     DensLane A;
-    {
-        const int k = C.ulist[ai];
-        const float H = C.aH[k];
-        A.xi = C.ax[k]; A.yi = C.ay[k]; A.zi = C.az[k];
-        A.h2 = live ? H * H : -1.f; // a dead thread never hits
-        A.ih2 = 1.f / (H * H);
-        A.s = A.ds = A.r = A.dr = f2(0.f);
-        A.cn = 0;
-        A.q0 = A.qw = smem_u32(C.q + tid);
-        A.mofs = HAS_MASS ? smem_u32(C.qm) - smem_u32(C.q) : 0u;
-    }
-    // warp 0 (thread i < g holds active i): bounding box and reach of the actives still iterating; the
-    // segment list of the previous evaluation stays valid if it was complete and the reach has not
-    // grown -- the actives still iterating are a subset (their bounding box lies inside the old one), so
-    // the old list and its frame cover this evaluation; if its candidates fitted in shared memory they
-    // are still there, too.
-    if (warp == 0) {
-        const bool has = lane < g;
-        const float hg = warp_max(has ? C.aH[C.ulist[lane]] : 0.f);
-        const bool reuse = C.listed && hg <= C.walk_hg;
-        if (!reuse) {
-            // after the first evaluation H is within a few per cent of its final value: reach a little
-            // farther than needed, so that the evaluations that follow find the list still valid
-            const float hgw = evalno > 0 ? hg * (1.f + SPH_REWALK_MARGIN) : hg;
-            publish_box(C.W, has, A.xi, A.yi, A.zi, hgw);
-            if (lane == 0) C.walk_hg = hgw;
+    A.mofs = HAS_MASS ? smem_u32(W.qm) - smem_u32(W.q) : 0u;
+    A.cp = W.slot + s;
+    A.cstride = f;
+    A.steps = (SPH_CH / 2) / f;
+    // bounding box and reach of the actives still iterating
+    float x0 = inf, x1 = -inf, y0 = inf, y1 = -inf, z0 = inf, z1 = -inf, hg = 0.f;
+#pragma unroll
+    for (int q = 0; q < SPH_NA; q++) {
+        DensAct &P = A.act[q];
+        const int i = ap * SPH_NA + q;
+        const bool has = live && i < g;
+        const int k = W.ulist[has ? i : 0];
+        const float H = W.aH[k];
+        P.xi = W.ax[k]; P.yi = W.ay[k]; P.zi = W.az[k];
+        P.h2 = has ? H * H : -1.f; // a missing active never hits
+        P.ih2 = 1.f / (H * H);
+        P.s = P.ds = P.r = P.dr = f2(0.f);
+        P.cn = 0;
+        P.q0 = P.qw = smem_u32(W.q + q * SPH_QCAP * 32 + lane);
+        if (has) {
+            x0 = fminf(x0, P.xi); x1 = fmaxf(x1, P.xi);
+            y0 = fminf(y0, P.yi); y1 = fmaxf(y1, P.yi);
+            z0 = fminf(z0, P.zi); z1 = fmaxf(z1, P.zi);
+            hg = fmaxf(hg, H);
         }
-        if (lane == 0) C.reuse = reuse ? 1 : 0;
     }
-    __syncthreads();
-    const bool reuse = C.reuse != 0;
-    if (!reuse) { walk_cta<false>(C.W, a.nodes, nullptr, L, true); walks++; }
-    bool first = true, onechunk = false;
-    for (;;) {
-        const WalkCtl ctl = walk_result(C.W);
-        // this thread's active in the batch's frame
-        A.nx = f2(-(ctl.pairwrap ? A.xi : recentre(A.xi, ctl.thx, L)));
-        A.ny = f2(-(ctl.pairwrap ? A.yi : recentre(A.yi, ctl.thy, L)));
-        A.nz = f2(-(ctl.pairwrap ? A.zi : recentre(A.zi, ctl.thz, L)));
-        const uint32_t nch = (ctl.total + SPH_DCAP - 1) / SPH_DCAP;
-        const bool keep = reuse && C.resident; // the candidates themselves are still staged
-        for (uint32_t c = 0; c < nch; c++) {
-            const uint32_t lo = c * SPH_DCAP, cnt = min((uint32_t)SPH_DCAP, ctl.total - lo);
-            if (!keep) {
-                if (tid == 0) C.nstaged = 0;
-                __syncthreads();
-                gather_chunk<HAS_MASS>(C, ctl, lo, cnt, a.xyzm, L);
-                __syncthreads();
-                const uint32_t ns = C.nstaged;
-                if (tid < 8) { // the ragged tail of the last quad and the quad after it
-                    C.X[ns + tid] = SPH_NANF; C.Y[ns + tid] = 0.f; C.Z[ns + tid] = 0.f;
-                    if (HAS_MASS) C.M[ns + tid] = 0.f;
-                }
-                __syncthreads();
-                staged += cnt;
-            }
-            const uint32_t ns = C.nstaged;
-            cands += ns;
-            const int nq = (int)((ns + 3u) >> 2);
-            if (ctl.pairwrap) consume<KERNEL, HAS_MASS, true>(C, A, nq, s, f, live, L);
-            else consume<KERNEL, HAS_MASS, false>(C, A, nq, s, f, live, L);
-            if (c + 1 < nch || ctl.sp > 0) __syncthreads(); // the arrays are about to be overwritten
-        }
-        onechunk = first && nch == 1;
-        if (reuse || ctl.sp <= 0) break;
-        first = false;
-        walk_cta<false>(C.W, a.nodes, nullptr, L, false);
-    }
-    if (!reuse && tid == 0) {
-        C.listed = first ? 1 : 0;              // complete in one batch
-        C.resident = first && onechunk ? 1 : 0;  // ... and in one chunk
-    }
+    x0 = warp_min(x0); x1 = warp_max(x1);
+    y0 = warp_min(y0); y1 = warp_max(y1);
+    z0 = warp_min(z0); z1 = warp_max(z1);
+    hg = warp_max(hg);
+    const float gcx = 0.5f * (x0 + x1), ghx = 0.5f * (x1 - x0) * (1.f + 1e-6f);
+    const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
+    const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
 
-    drain<KERNEL, HAS_MASS>(A, __reduce_max_sync(FULLMASK, (int)((A.qw - A.q0) / SPH_QSTRIDE)));
-    // cross-stream totals through shared memory (the queues are empty now): fp64, ascending stream order
-    __syncthreads();
-    double *pS = reinterpret_cast<double *>(C.q), *pD = pS + SPH_THREADS, *pR = pD + SPH_THREADS, *pDR = pR + SPH_THREADS;
-    int *pn = reinterpret_cast<int *>(pDR + SPH_THREADS);
-    pS[tid] = (double)A.s.x + (double)A.s.y;
-    pD[tid] = (double)A.ds.x + (double)A.ds.y;
-    if (HAS_MASS) { pR[tid] = (double)A.r.x + (double)A.r.y; pDR[tid] = (double)A.dr.x + (double)A.dr.y; }
-    pn[tid] = A.cn;
-#ifdef SPH_DIAG
-    {
-        const int mxh = __reduce_max_sync(FULLMASK, A.cn), smh = __reduce_add_sync(FULLMASK, A.cn);
-        const int nl = __popc(__ballot_sync(FULLMASK, live));
-        if (lane == 0 && nl) {
-            const int b = evalno < 2 ? 0 : 1;
-            atomicAdd(&a.cnt->lvl_begin[2 * b], (unsigned)mxh * nl);   // reuse dead index counters as scratch
-            atomicAdd(&a.cnt->lvl_done[2 * b], (unsigned)smh);
-            atomicAdd(&a.cnt->lvl_begin[2 * b + 1], (unsigned)mxh * 32);
+    // The segment list of the group's previous evaluation is still in shared memory.  It stays valid if
+    // it was complete (one batch) and the reach has not grown: the actives still iterating are a subset
+    // (their bounding box lies inside the old one), so the old list and its frame cover this evaluation.
+    const bool reuse = wc.valid && hg <= wc.hg;
+    WalkCtl ctl = wc.ctl;
+    if (!reuse) ctl.sp = -1;
+    do {
+        if (!reuse) walk_batch<false>(W.ws, ctl, a.nodes, nullptr, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
+        cands += ctl.total;
+        // this lane's actives in the batch's frame
+#pragma unroll
+        for (int q = 0; q < SPH_NA; q++) {
+            DensAct &P = A.act[q];
+            P.nx = f2(-(ctl.pairwrap ? P.xi : recentre(P.xi, ctl.thx, L)));
+            P.ny = f2(-(ctl.pairwrap ? P.yi : recentre(P.yi, ctl.thy, L)));
+            P.nz = f2(-(ctl.pairwrap ? P.zi : recentre(P.zi, ctl.thz, L)));
         }
-    }
-#endif
-    __syncthreads();
+        const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
+        GatherCtl gc;
+        gc.kseg = 0;
+        // software pipeline: the loads of chunk c + 1 are in flight (in registers) while chunk c is tested
+        GatherRegs G;
+        if (nch) gather_load(W.ws, ctl, gc, 0, G, a.xyzm);
+        for (uint32_t c = 0; c < nch; c++) {
+            gather_store<false, true>(ctl, G, W.slot, nullptr, L); // (writing w even when unread measured faster: 74.6 vs 78.6 ms)
+            if (c + 1 < nch) gather_load(W.ws, ctl, gc, c + 1, G, a.xyzm);
+            if (ctl.pairwrap) consume_chunk<KERNEL, HAS_MASS, true>(A, live, L);
+            else consume_chunk<KERNEL, HAS_MASS, false>(A, live, L);
+        }
+        if (!reuse) {
+            wc.valid = !wc.multi && ctl.sp <= 0; // complete in its first batch
+            wc.multi = true;
+            wc.hg = hg;
+            wc.ctl = ctl;
+        }
+    } while (ctl.sp > 0);
+
     S = D = R = DR = 0.0;
     nint = 0;
-    if (tid < g) {
-        for (int t = tid; t < g * f; t += g) {
-            S += pS[t]; D += pD[t]; nint += pn[t];
-            if (HAS_MASS) { R += pR[t]; DR += pDR[t]; }
+#pragma unroll
+    for (int q = 0; q < SPH_NA; q++) {
+        DensAct &P = A.act[q];
+        drain<KERNEL, HAS_MASS>(P, A.mofs, __reduce_max_sync(FULLMASK, (int)((P.qw - P.q0) >> 7)));
+        // cross-stream totals: lane ap + gp*s adds lane ap + gp*(s+d) for d = 1, 2, 4, ...
+        double tS = (double)P.s.x + (double)P.s.y, tD = (double)P.ds.x + (double)P.ds.y;
+        double tR = (double)P.r.x + (double)P.r.y, tDR = (double)P.dr.x + (double)P.dr.y;
+        int tn = P.cn;
+        for (int d = 1; d < f; d <<= 1) {
+            const bool take = live && s + d < f;
+            const int from = take ? lane + gp * d : lane;
+            const double uS = __shfl_sync(FULLMASK, tS, from), uD = __shfl_sync(FULLMASK, tD, from);
+            const int un = __shfl_sync(FULLMASK, tn, from);
+            if (take) { tS += uS; tD += uD; tn += un; }
+            if (HAS_MASS) {
+                const double uR = __shfl_sync(FULLMASK, tR, from), uDR = __shfl_sync(FULLMASK, tDR, from);
+                if (take) { tR += uR; tDR += uDR; }
+            }
+        }
+        // active i = ap * SPH_NA + q sits in lane ap (stream 0): hand it to lane i
+        const int src = lane / SPH_NA;
+        const double oS = __shfl_sync(FULLMASK, tS, src), oD = __shfl_sync(FULLMASK, tD, src);
+        const int on = __shfl_sync(FULLMASK, tn, src);
+        const bool mine = lane % SPH_NA == q;
+        if (mine) { S = oS; D = oD; nint = on; }
+        if (HAS_MASS) {
+            const double oR = __shfl_sync(FULLMASK, tR, src), oDR = __shfl_sync(FULLMASK, tDR, src);
+            if (mine) { R = oR; DR = oDR; }
         }
     }
-    __syncthreads(); // the totals are read before the next evaluation pushes onto the queues
 }
 
 template <int KERNEL, bool HAS_MASS>
 __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    DensCta<HAS_MASS> &C = *reinterpret_cast<DensCta<HAS_MASS> *>(smem_raw);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    DensWarp<HAS_MASS> &W = reinterpret_cast<DensWarp<HAS_MASS> *>(smem_raw)[warp];
     if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
-    unsigned long long st_evals = 0, st_cands = 0, st_pairs = 0, st_staged = 0; // meaningful in thread 0 only
-    unsigned int st_unconv = 0, st_walks = 0, st_gevals = 0;
+    unsigned long long st_evals = 0, st_cands = 0, st_pairs = 0; // meaningful in lane 0 only
+    unsigned int st_unconv = 0;
+    unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups (neighbouring groups share candidates in L1/L2)
     for (;;) {
-        __syncthreads(); // the previous group's shared state is dead
-        if (tid == 0) C.gnext = atomicAdd(&a.cnt->work, 1u);
-        __syncthreads();
-        const unsigned int g = C.gnext;
-        if (g >= n_groups) break;
+        if (gnext == gend) {
+            if (lane == 0) gnext = atomicAdd(&a.cnt->work, (unsigned int)SPH_GBLOCK);
+            gnext = __shfl_sync(FULLMASK, gnext, 0);
+            if (gnext >= n_groups) break;
+            gend = min(gnext + SPH_GBLOCK, n_groups);
+        }
+        const unsigned int g = gnext++;
         const uint32_t i0 = a.gstart[g];
         const uint32_t i1 = (g + 1 < n_groups) ? a.gstart[g + 1] : a.n_items;
         const int na = (int)(i1 - i0);
         SPH_ASSERT(i1 > i0 && i1 <= a.n_items && na <= SPH_MAXB);
-        if (tid < na) {
-            uint32_t slot = a.item_slot ? a.item_slot[i0 + tid] : i0 + tid;
+        __syncwarp();
+        if (lane < na) {
+            uint32_t slot = a.item_slot ? a.item_slot[i0 + lane] : i0 + lane;
             SPH_ASSERT(slot < a.n_total);
             float4 p = a.xyzm[slot];
             uint32_t id = a.perm[slot];
-            C.aid[tid] = id;
-            C.ax[tid] = p.x; C.ay[tid] = p.y; C.az[tid] = p.z;
-            C.aH[tid] = a.h[id];
-            C.lo[tid] = 0.0;
-            C.hi[tid] = (double)__int_as_float(0x7f800000);
-            C.it[tid] = 0;
-            C.ulist[tid] = tid;
+            W.aid[lane] = id;
+            W.ax[lane] = p.x; W.ay[lane] = p.y; W.az[lane] = p.z;
+            W.aH[lane] = a.h[id];
+            W.lo[lane] = 0.0;
+            W.hi[lane] = (double)__int_as_float(0x7f800000);
+            W.it[lane] = 0;
+            W.ulist[lane] = lane;
         }
-        if (tid == 0) { C.resident = 0; C.listed = 0; }
-        __syncthreads();
-        int n_u = na, evalno = 0;
+        __syncwarp();
+        int n_u = na;
+        WalkCache wc;
+        wc.valid = false;
         while (n_u > 0) {
+            wc.multi = false;
             double S, D, R, DR;
             int nint;
             unsigned long long cands = 0;
-            evaluate<KERNEL, HAS_MASS>(C, a, n_u, evalno, S, D, R, DR, nint, cands, st_staged, st_walks);
-            st_gevals++;
+            evaluate<KERNEL, HAS_MASS>(W, a, n_u, wc, S, D, R, DR, nint, cands);
 
-            if (warp == 0) {
-                // a8: safeguarded Newton update (R7), one thread per particle, fp64 scalars
-                bool more = false, bad = false;
-                int k = -1;
-                if (lane < n_u) {
-                    k = C.ulist[lane];
-                    const double H = (double)C.aH[k];
-                    const double Nw = (4.0 * 3.14159265358979323846 / 3.0) * KernelConst<KERNEL>::sigma * S;
-                    const double N = a.count_mode ? (double)nint : Nw;
-                    const double nt = (double)a.n_target, tol = (double)a.n_tol;
-                    int it = ++C.it[k];
-                    int flag = 0;
-                    double lo = C.lo[k], hi = C.hi[k], Hn = H;
-                    if (fabs(N - nt) <= tol) flag = SPH_ST_CONVERGED;
-                    else if (it >= a.max_iter) flag = SPH_ST_NOTCONV;
+            // a8: safeguarded Newton update (R7), one lane per particle, fp64 scalars
+            bool more = false, bad = false;
+            int k = -1;
+            if (lane < n_u) {
+                k = W.ulist[lane];
+                const double H = (double)W.aH[k];
+                const double Nw = (4.0 * 3.14159265358979323846 / 3.0) * KernelConst<KERNEL>::sigma * S;
+                const double N = a.count_mode ? (double)nint : Nw;
+                const double nt = (double)a.n_target, tol = (double)a.n_tol;
+                int it = ++W.it[k];
+                int flag = 0;
+                double lo = W.lo[k], hi = W.hi[k], Hn = H;
+                if (fabs(N - nt) <= tol) flag = SPH_ST_CONVERGED;
+                else if (it >= a.max_iter) flag = SPH_ST_NOTCONV;
+                else {
+                    if (N < nt) { if (H > lo) lo = H; } else { if (H < hi) hi = H; }
+                    bool br = isfinite(hi) && lo > 0.0;
+                    if (br && hi - lo <= 1e-6 * lo) flag = SPH_ST_BRACKET;
                     else {
-                        if (N < nt) { if (H > lo) lo = H; } else { if (H < hi) hi = H; }
-                        bool br = isfinite(hi) && lo > 0.0;
-                        if (br && hi - lo <= 1e-6 * lo) flag = SPH_ST_BRACKET;
-                        else {
-                            // g = 1/(1 + H D'/(3 S')) with D' = -sigma H^-4 D, S' = sigma H^-3 S  ->  1/(1 - D/(3S))
-                            double gs = 1.0 / (1.0 - D / (3.0 * S));
-                            if (!(gs > 0.0 && gs < 4.0) || N == 0.0) gs = 1.0;
-                            const double smin = 0.79370052598409973738, smax = 1.25992104989487316476;
-                            // Newton step on ln N(ln H): d ln N / d ln H = 3 / gs  (R7)
-                            double sc = (N == 0.0) ? smax : pow(nt / N, gs / 3.0);
-                            sc = fmin(fmax(sc, smin), smax);
-                            Hn = H * sc;
-                            if (br && !(lo < Hn && Hn < hi)) Hn = cbrt(0.5 * (lo * lo * lo + hi * hi * hi));
-                            Hn = fmin(Hn, 0.49999 * (double)a.L);
-                            // the evaluation runs at fp32 H: a step below fp32 resolution cannot move it
-                            if ((float)Hn == (float)H) flag = SPH_ST_STALLED;
-                        }
-                    }
-                    C.lo[k] = lo; C.hi[k] = hi;
-                    if (flag) { // a9: finalise and scatter to the caller's particle id
-                        const uint32_t id = C.aid[k];
-                        const double ih = 1.0 / H, ih3 = ih * ih * ih;
-                        double rho, om;
-                        if (HAS_MASS) {
-                            rho = KernelConst<KERNEL>::sigma * ih3 * R;
-                            om = 1.0 - DR / (3.0 * R);
-                        } else {
-                            rho = (double)a.mass_scalar * KernelConst<KERNEL>::sigma * ih3 * S;
-                            om = 1.0 - D / (3.0 * S);
-                        }
-                        a.h[id] = (float)H;
-                        a.rho[id] = (float)rho;
-                        a.omega[id] = (float)om;
-                        a.ngb[id] = nint;
-                        if (a.status) a.status[id] = it | flag;
-                        bad = flag != SPH_ST_CONVERGED;
-                    } else {
-                        C.aH[k] = (float)Hn;
-                        more = true;
+                        // g = 1/(1 + H D'/(3 S')) with D' = -sigma H^-4 D, S' = sigma H^-3 S  ->  1/(1 - D/(3S))
+                        double gs = 1.0 / (1.0 - D / (3.0 * S));
+                        if (!(gs > 0.0 && gs < 4.0) || N == 0.0) gs = 1.0;
+                        const double smin = 0.79370052598409973738, smax = 1.25992104989487316476;
+                        // Newton step on ln N(ln H): d ln N / d ln H = 3 / gs  (R7)
+                        double sc = (N == 0.0) ? smax : pow(nt / N, gs / 3.0);
+                        sc = fmin(fmax(sc, smin), smax);
+                        Hn = H * sc;
+                        if (br && !(lo < Hn && Hn < hi)) Hn = cbrt(0.5 * (lo * lo * lo + hi * hi * hi));
+                        Hn = fmin(Hn, 0.49999 * (double)a.L);
+                        // the evaluation runs at fp32 H: a step below fp32 resolution cannot move it
+                        if ((float)Hn == (float)H) flag = SPH_ST_STALLED;
                     }
                 }
-                // statistics (warp-uniform reductions)
-                unsigned long long pr = (lane < n_u) ? (unsigned long long)nint : 0ull;
-#pragma unroll
-                for (int o = 16; o; o >>= 1) pr += __shfl_xor_sync(FULLMASK, pr, o);
-                const unsigned mb = __ballot_sync(FULLMASK, bad);
-                const unsigned mm = __ballot_sync(FULLMASK, more);
-                st_evals += (unsigned long long)n_u;
-                st_cands += cands * (unsigned long long)n_u;
-                st_pairs += pr;
-                st_unconv += __popc(mb);
-                // compact the list of particles that keep iterating
-                __syncwarp();
-                if (more) C.ulist[__popc(mm & lanemask_lt())] = k;
-                if (lane == 0) C.n_u = __popc(mm);
+                W.lo[k] = lo; W.hi[k] = hi;
+                if (flag) { // a9: finalise and scatter to the caller's particle id
+                    const uint32_t id = W.aid[k];
+                    const double ih = 1.0 / H, ih3 = ih * ih * ih;
+                    double rho, om;
+                    if (HAS_MASS) {
+                        rho = KernelConst<KERNEL>::sigma * ih3 * R;
+                        om = 1.0 - DR / (3.0 * R);
+                    } else {
+                        rho = (double)a.mass_scalar * KernelConst<KERNEL>::sigma * ih3 * S;
+                        om = 1.0 - D / (3.0 * S);
+                    }
+                    a.h[id] = (float)H;
+                    a.rho[id] = (float)rho;
+                    a.omega[id] = (float)om;
+                    a.ngb[id] = nint;
+                    if (a.status) a.status[id] = it | flag;
+                    bad = flag != SPH_ST_CONVERGED;
+                } else {
+                    W.aH[k] = (float)Hn;
+                    more = true;
+                }
             }
-            __syncthreads();
-            n_u = C.n_u;
-            evalno++;
+            // statistics (warp-uniform reductions)
+            unsigned long long pr = (lane < n_u) ? (unsigned long long)nint : 0ull;
+#pragma unroll
+            for (int o = 16; o; o >>= 1) pr += __shfl_xor_sync(FULLMASK, pr, o);
+            unsigned mb = __ballot_sync(FULLMASK, bad);
+            unsigned mm = __ballot_sync(FULLMASK, more);
+            st_evals += (unsigned long long)n_u;
+            st_cands += cands * (unsigned long long)n_u;
+            st_pairs += pr;
+            st_unconv += __popc(mb);
+            // compact the list of particles that keep iterating
+            __syncwarp();
+            if (more) W.ulist[__popc(mm & lanemask_lt())] = k;
+            n_u = __popc(mm);
+            __syncwarp();
         }
     }
-    if (tid == 0) {
+    if (lane == 0) {
         if (st_evals) atomicAdd(&a.cnt->dens_evals, st_evals);
         if (st_cands) atomicAdd(&a.cnt->dens_cands, st_cands);
         if (st_pairs) atomicAdd(&a.cnt->dens_pairs, st_pairs);
         if (st_unconv) atomicAdd(&a.cnt->n_unconv, st_unconv);
-        atomicAdd(&a.cnt->dens_group_evals, (unsigned long long)st_gevals);
-        atomicAdd(&a.cnt->dens_walks, (unsigned long long)st_walks);
-        atomicAdd(&a.cnt->dens_staged, st_staged);
     }
 }
 
@@ -538,22 +474,23 @@ __global__ void k_reset_counters(SphCounters *c, int which, bool subset)
 {
     c->work = 0;
     if (!subset) c->bad_ids = 0; // no active list in this call
-    if (which == 0) { c->n_unconv = 0; c->dens_evals = 0; c->dens_cands = 0; c->dens_pairs = 0; c->dens_group_evals = 0; c->dens_walks = 0; c->dens_staged = 0; }
-    else { c->force_cands = 0; c->force_pairs = 0; c->force_staged = 0; }
+    if (which == 0) { c->n_unconv = 0; c->dens_evals = 0; c->dens_cands = 0; c->dens_pairs = 0; }
+    else { c->force_cands = 0; c->force_pairs = 0; }
 }
 
 template <int KERNEL, bool HAS_MASS>
 int launch(sph_ctx *ctx, const DensArgs &a, int64_t est_groups)
 {
-    size_t dyn = sizeof(DensCta<HAS_MASS>);
+    size_t dyn = sizeof(DensWarp<HAS_MASS>) * SPH_WARPS;
     auto kfn = k_density<KERNEL, HAS_MASS>;
     SPH_CUDA(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
     int per_sm = 1;
     SPH_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kfn, SPH_THREADS, dyn));
     if (per_sm < 1) return sph_fail(ctx, SPH_E_INTERNAL, "k_density does not fit on an SM");
-    // persistent CTAs: every SM filled to the occupancy the kernel reaches
+    // persistent warps: every SM filled to the occupancy the kernel reaches
     int64_t grid = (int64_t)ctx->device_sms * per_sm;
-    if (est_groups < grid) grid = est_groups > 0 ? est_groups : 1;
+    int64_t need = (est_groups + SPH_WARPS * SPH_GBLOCK - 1) / (SPH_WARPS * SPH_GBLOCK);
+    if (need < grid) grid = need > 0 ? need : 1;
     kfn<<<(int)grid, SPH_THREADS, dyn, ctx->stream>>>(a);
     SPH_CUDA(ctx, cudaGetLastError());
     return SPH_OK;

@@ -6,12 +6,10 @@
 // r_ij < max(H_i, H_j) (R10): the walk prunes a node only if it is farther from the group than both
 // the group's reach and the largest support radius inside the node.
 //
-// Same CTA-per-group mapping as sph_density.cu: thread = (active, stream).  The candidate runs found by
-// the walk are staged tile by tile in shared memory, each candidate twice: component arrays X[], Y[],
-// Z[], H2[] for the packed distance tests, and three 16-byte records (x,y,z,slot | v,c | rho,A,m,1/H) for
-// the hit evaluation.  A hit pushes the candidate's tile-local index onto the thread's queue; queued
-// hits are evaluated in bulk from shared memory (no global access per hit); a, du/dt are accumulated
-// in fp64 per thread (R15).
+// Same warp-per-group mapping as sph_density.cu: lane = (active, stream); candidates' (x,y,z,H) are
+// gathered chunk by chunk into the warp's shared-memory slot and tested; a hit pushes the candidate's sorted slot
+// onto the lane's queue; queued hits are evaluated in bulk, fetching the pair's remaining state
+// (velocity, sound speed, rho, A, m) from the sorted arrays through L1.
 #include "sph_warp.cuh"
 
 namespace {
@@ -30,18 +28,6 @@ struct ForceArgs {
     float *acc, *dudt, *vsig;
 };
 
-template <int KERNEL>
-__device__ __forceinline__ float kern_dw(float q) // w'(q), 0 for q >= 1 (R1)
-{
-    float t = fmaxf(1.f - q, 0.f);
-    if (KERNEL == SPH_KERNEL_CUBIC) {
-        float a = q * fmaf(18.f, q, -12.f), b = -6.f * t * t;
-        return q <= 0.5f ? a : b;
-    } else {
-        float t2 = t * t, t4 = t2 * t2, t7 = t4 * t2 * t;
-        return -22.f * q * t7 * fmaf(q, fmaf(16.f, q, 7.f), 1.f);
-    }
-}
 // w'(q) for the two arguments of a pair, (r / H_i, r / H_j), in one packed f32x2 chain
 template <int KERNEL>
 __device__ __forceinline__ float2 kern_dw2(float2 q)
@@ -66,66 +52,61 @@ __device__ __forceinline__ float kern_sigma()
     return KERNEL == SPH_KERNEL_CUBIC ? 2.54647908947032537f : 6.78895304126365994f;
 }
 
-struct ForceCta {
-    // one tile of candidates in the batch's frame: component arrays for the tests (NaN-padded like the
-    // density kernel's) and the state records for the hits
-    alignas(16) float X[SPH_FTILE + 8];
-    alignas(16) float Y[SPH_FTILE + 8];
-    alignas(16) float Z[SPH_FTILE + 8];
-    alignas(16) float H2[SPH_FTILE + 8];
-    alignas(16) float4 r0[SPH_FTILE]; // x, y, z (frame), sorted slot (bits)
-    alignas(16) float4 r1[SPH_FTILE]; // vx, vy, vz, c
-    alignas(16) float4 r2[SPH_FTILE]; // rho, A, m, 1/H
-    alignas(16) uint16_t q[SPH_QCAP_FORCE * SPH_THREADS]; // hit queues: entry k of thread t at [k * SPH_THREADS + t]
-    WalkShared W;
-    unsigned int gnext;
+struct ForceWarp {
+    float4 slot[SPH_CH];                // one chunk of candidates as pair records (x,y,z,H)
+    WarpWalk ws;
+    uint32_t q[SPH_QCAP_FORCE * 32];          // hit queue: sorted slot of the neighbour
+    alignas(16) uint32_t gidx[SPH_CH];              // sorted slot of every candidate of the chunk
 };
 
-#define SPH_FQSTRIDE (2u * SPH_THREADS) // bytes between consecutive queue entries of a thread
-
-// per-thread state of the thread's active and its running sums
+// per-lane state of the lane's active and its running sums
 struct ForceLane {
     float xi, yi, zi, h2, hinv, f4;  // position, H^2, 1/H, sigma/H^4
-    float xf, yf, zf;                // position in the batch's frame
     float vx, vy, vz, c, rho, A;
     uint32_t slot;
-    double px, py, pz, pdu;          // fp64 accumulators (R15: "fp64 accumulation where needed")
+    double px, py, pz, pdu; // fp64 accumulators of a and du/dt (R15: "fp64 accumulation where needed")
     float pvs;
-    int cn, cnt;                     // hits evaluated; hits queued
+    int cn, cnt;
 };
 
-__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v)
-{
-    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v)); // no memory clobber: see sts_f32
-}
-__device__ __forceinline__ uint32_t lds_u16(uint32_t addr)
-{
-    unsigned short v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
-    return (uint32_t)v;
-}
+// frame of the batch the queued hits were found in (see walk_batch)
+struct Frame {
+    float thx, thy, thz;
+    bool pairwrap;
+    bool rec; // some axis is recentred (thr finite); false: raw coordinates are already the frame
+};
 
-// evaluate the m newest queued hits of every thread of the warp (n = warp-wide maximum of m) from the
-// tile's state records
-template <int KERNEL, bool PAIRWRAP>
-__device__ __forceinline__ void drain(const ForceCta &C, const ForceArgs &a, uint32_t q0, ForceLane &A, int n)
+// evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
+// WRAP: 0 raw coordinate differences, 1 recentred frame, 2 per-pair nearest image
+template <int KERNEL, int WRAP>
+__device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
+                                      const Frame &fr)
 {
     const int m = min(n, A.cnt), base = A.cnt - m;
     const float L = a.L, alpha = a.alpha;
-    uint32_t ra = q0 + (uint32_t)base * SPH_FQSTRIDE;
+    const float xf = WRAP == 1 ? recentre(A.xi, fr.thx, L) : A.xi;
+    const float yf = WRAP == 1 ? recentre(A.yi, fr.thy, L) : A.yi;
+    const float zf = WRAP == 1 ? recentre(A.zi, fr.thz, L) : A.zi;
 #pragma unroll 2
-    for (int k = 0; k < n; k++, ra += SPH_FQSTRIDE) {
+    for (int k = 0; k < n; k++) {
         if (k < m) {
-            const uint32_t j = lds_u16(ra);
-            const float4 P0 = C.r0[j], P1 = C.r1[j], P2 = C.r2[j];
+            const uint32_t j = lds_u32(smem_u32(qp + (base + k) * 32)); // (volatile: ordered after the pushes)
+            const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + 2 * (size_t)j), P2 = __ldg(a.vc + 2 * (size_t)j + 1);
             float dx, dy, dz;
-            if (PAIRWRAP) {
+            if (WRAP == 2) {
                 dx = image_diff(A.xi, P0.x, L); dy = image_diff(A.yi, P0.y, L); dz = image_diff(A.zi, P0.z, L);
+            } else if (WRAP == 1) {
+                dx = xf - recentre(P0.x, fr.thx, L); dy = yf - recentre(P0.y, fr.thy, L); dz = zf - recentre(P0.z, fr.thz, L);
             } else {
-                dx = A.xf - P0.x; dy = A.yf - P0.y; dz = A.zf - P0.z;
+                dx = xf - P0.x; dy = yf - P0.y; dz = zf - P0.z;
             }
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            const float rinv = rsqrtf(fmaxf(r2, 1e-37f));
+            // 1/r to ~1 ulp: the hardware approximation (2 ulp) plus one Newton step.  The pair term's error is
+            // dominated by the error of r amplified by w''/w' (~10), and a sum of ~500 such terms is compared
+            // with 1e-7 of the sum of their magnitudes (R15)
+            const float r2c = fmaxf(r2, 1e-37f);
+            float rinv = rsqrtf(r2c);
+            rinv = rinv * fmaf(-0.5f * r2c, rinv * rinv, 1.5f);
             const float r = r2 * rinv;
             const float hinv_j = P2.w; // 1 / H_j, correctly rounded once per particle (k_force_prep)
             const float hj2 = hinv_j * hinv_j;
@@ -140,7 +121,7 @@ __device__ __forceinline__ void drain(const ForceCta &C, const ForceArgs &a, uin
             const float Fbar = 0.5f * (Fi + Fj);
             const float AiFi = A.A * Fi;
             const float pv = Pi * Fbar;
-            const bool other = __float_as_uint(P0.w) != A.slot; // j == i: no self force, no self signal velocity
+            const bool other = j != A.slot; // j == i: no self force, no self signal velocity
             // select, not multiply by zero: a lone particle has Omega = 0, hence A = inf
             const float tr = other ? P2.z * (AiFi + fmaf(P2.y, Fj, pv)) * rinv : 0.f;
             const float du = other ? P2.z * fmaf(0.5f, pv, AiFi) * vr : 0.f;
@@ -155,182 +136,166 @@ __device__ __forceinline__ void drain(const ForceCta &C, const ForceArgs &a, uin
     A.cnt = base;
 }
 
-// one candidate against this thread's active (symmetric set, R10): hit if r^2 < max(H_i, H_j)^2
-__device__ __forceinline__ void push_if(const ForceLane &A, uint32_t &qw, float r2, float hj2, uint32_t idx)
+template <int KERNEL>
+__device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
+                                          const Frame &fr)
 {
-    if (r2 < fmaxf(A.h2, hj2)) {
-        sts_u16(qw, idx);
-        qw += SPH_FQSTRIDE;
-    }
+    if (fr.pairwrap) drain<KERNEL, 2>(a, qp, A, n, fr);
+    else if (fr.rec) drain<KERNEL, 1>(a, qp, A, n, fr);
+    else drain<KERNEL, 0>(a, qp, A, n, fr);
 }
 
-// Test the nq candidate quads of the staged tile against this thread's active; a hit pushes the
-// candidate's tile-local index onto the thread's queue.
+// Test the candidate pairs of the gathered chunk against this lane's active (symmetric set, R10):
+// hit if r^2 < max(H_i, H_j)^2; a hit pushes the candidate's sorted slot onto the lane's queue.
 template <int KERNEL, bool PAIRWRAP>
-__device__ __forceinline__ void consume(const ForceCta &C, const ForceArgs &a, uint32_t q0, ForceLane &A, int nq, int s, int f,
-                                        bool live)
+__device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,
+                                              const uint32_t *__restrict__ gp, uint32_t *__restrict__ qp, ForceLane &A,
+                                              int s, int f, bool live, const Frame &fr)
 {
-    const float4 *X4 = reinterpret_cast<const float4 *>(C.X), *Y4 = reinterpret_cast<const float4 *>(C.Y);
-    const float4 *Z4 = reinterpret_cast<const float4 *>(C.Z), *H4 = reinterpret_cast<const float4 *>(C.H2);
+    const int steps = (SPH_CH / 2) / f;
+    const float4 *cp = slotp + s;
+    uint32_t ga = smem_u32(gp + 2 * s);
     const float L = a.L;
-    const float2 nx = make_float2(-A.xf, -A.xf), ny = make_float2(-A.yf, -A.yf), nz = make_float2(-A.zf, -A.zf);
-    const int steps = (nq + f - 1) / f; // CTA-uniform
-    int qd = s;
-    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP_FORCE) {
-        const int nt = min(SPH_QSTEP_FORCE, steps - t0);
+    const float xf = PAIRWRAP ? A.xi : recentre(A.xi, fr.thx, L);
+    const float yf = PAIRWRAP ? A.yi : recentre(A.yi, fr.thy, L);
+    const float zf = PAIRWRAP ? A.zi : recentre(A.zi, fr.thz, L);
+    const float2 nx = make_float2(-xf, -xf), ny = make_float2(-yf, -yf), nz = make_float2(-zf, -zf);
+    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
+        const int nt = min(SPH_QSTEP, steps - t0);
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
-        if (mx + 4 * nt > SPH_QCAP_FORCE) {
+        if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain<KERNEL, PAIRWRAP>(C, a, q0, A, max(min(mn, mx), mx + 4 * nt - SPH_QCAP_FORCE));
+            drain_any<KERNEL>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
         }
-        uint32_t qw = q0 + (uint32_t)A.cnt * SPH_FQSTRIDE;
+        const uint32_t q0 = smem_u32(qp);
+        uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
 #pragma unroll 2
         for (int t = 0; t < nt; t++) {
-            const int qi = min(qd, nq);
-            qd += f;
-            const float4 x = X4[qi], y = Y4[qi], z = Z4[qi], h = H4[qi]; // h: H_j^2 (squared once per candidate by the gather)
-            float2 ra, rb;
+            const float4 c0 = cp[0], c1 = cp[SPH_CH / 2]; // (x0,x1,y0,y1) (z0,z1,H0^2,H1^2)
+            cp += f;
+            float2 r2;
             if (PAIRWRAP) {
-                const float dx0 = image_diff(A.xi, x.x, L), dx1 = image_diff(A.xi, x.y, L);
-                const float dx2 = image_diff(A.xi, x.z, L), dx3 = image_diff(A.xi, x.w, L);
-                const float dy0 = image_diff(A.yi, y.x, L), dy1 = image_diff(A.yi, y.y, L);
-                const float dy2 = image_diff(A.yi, y.z, L), dy3 = image_diff(A.yi, y.w, L);
-                const float dz0 = image_diff(A.zi, z.x, L), dz1 = image_diff(A.zi, z.y, L);
-                const float dz2 = image_diff(A.zi, z.z, L), dz3 = image_diff(A.zi, z.w, L);
-                ra = make_float2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
-                rb = make_float2(fmaf(dz2, dz2, fmaf(dy2, dy2, dx2 * dx2)), fmaf(dz3, dz3, fmaf(dy3, dy3, dx3 * dx3)));
+                const float dx0 = image_diff(A.xi, c0.x, L), dx1 = image_diff(A.xi, c0.y, L);
+                const float dy0 = image_diff(A.yi, c0.z, L), dy1 = image_diff(A.yi, c0.w, L);
+                const float dz0 = image_diff(A.zi, c1.x, L), dz1 = image_diff(A.zi, c1.y, L);
+                r2 = make_float2(fmaf(dz0, dz0, fmaf(dy0, dy0, dx0 * dx0)), fmaf(dz1, dz1, fmaf(dy1, dy1, dx1 * dx1)));
             } else {
-                const float2 dxa = __fadd2_rn(make_float2(x.x, x.y), nx), dxb = __fadd2_rn(make_float2(x.z, x.w), nx);
-                const float2 dya = __fadd2_rn(make_float2(y.x, y.y), ny), dyb = __fadd2_rn(make_float2(y.z, y.w), ny);
-                const float2 dza = __fadd2_rn(make_float2(z.x, z.y), nz), dzb = __fadd2_rn(make_float2(z.z, z.w), nz);
-                ra = __ffma2_rn(dza, dza, __ffma2_rn(dya, dya, __fmul2_rn(dxa, dxa)));
-                rb = __ffma2_rn(dzb, dzb, __ffma2_rn(dyb, dyb, __fmul2_rn(dxb, dxb)));
+                const float2 dx = __fadd2_rn(make_float2(c0.x, c0.y), nx), dy = __fadd2_rn(make_float2(c0.z, c0.w), ny);
+                const float2 dz = __fadd2_rn(make_float2(c1.x, c1.y), nz);
+                r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
-            const uint32_t i0 = 4u * (uint32_t)qi;
-            push_if(A, qw, ra.x, h.x, i0);
-            push_if(A, qw, ra.y, h.y, i0 + 1u);
-            push_if(A, qw, rb.x, h.z, i0 + 2u);
-            push_if(A, qw, rb.y, h.w, i0 + 3u);
+            const float2 hj2 = make_float2(c1.z, c1.w); // H_j^2 (squared once per candidate by the gather)
+            if (r2.x < fmaxf(A.h2, hj2.x)) {
+                sts_u32(qw, lds_u32(ga));
+                qw += 128u;
+            }
+            if (r2.y < fmaxf(A.h2, hj2.y)) {
+                sts_u32(qw, lds_u32(ga + 4u));
+                qw += 128u;
+            }
+            ga += 8u * (uint32_t)f;
         }
-        A.cnt = (int)((qw - q0) / SPH_FQSTRIDE);
+        A.cnt = (int)((qw - q0) >> 7);
     }
-}
-
-// Stage tile t of the nt tiles of a walk batch: test arrays + state records.  The batch's candidates are
-// dealt onto the tiles one by one, round-robin (flat position p goes to tile p % nt, slot p / nt): every
-// tile is a uniform, fine-grained sample of the whole candidate set, so every thread finds its fair share
-// of hits in every tile and the bulk evaluation at the end of a tile keeps the lanes busy (a tile of
-// consecutive candidates is a compact region, near some actives and out of reach of the rest).
-// Returns the number of candidates of the tile (slots [0, cnt) are in use).
-__device__ __forceinline__ uint32_t gather_tile(ForceCta &C, const WalkCtl &ctl, uint32_t t, uint32_t nt, const ForceArgs &a)
-{
-    const int tid = threadIdx.x;
-    const float L = a.L;
-    const WalkShared &W = C.W;
-    const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // CTA-uniform
-    const uint32_t cnt = (ctl.total - t + nt - 1u) / nt; // t < nt <= total
-    for (uint32_t sl = tid; sl < cnt; sl += SPH_THREADS) {
-        const uint32_t p = sl * nt + t;
-        const int k = seg_of(W, ctl.n_seg, p);
-        const uint32_t j = W.seg_start[k] + (p - W.seg_pre[k]);
-        float4 c = ldg_nc(a.xyzh + j);
-        const float4 v = ldg_nc(a.vc + 2 * (size_t)j), w = ldg_nc(a.vc + 2 * (size_t)j + 1);
-        if (rec) { c.x = recentre(c.x, ctl.thx, L); c.y = recentre(c.y, ctl.thy, L); c.z = recentre(c.z, ctl.thz, L); }
-        C.X[sl] = c.x; C.Y[sl] = c.y; C.Z[sl] = c.z; C.H2[sl] = c.w * c.w;
-        C.r0[sl] = make_float4(c.x, c.y, c.z, __uint_as_float(j));
-        C.r1[sl] = v;
-        C.r2[sl] = w;
-    }
-    const uint32_t nq = (cnt + 3u) >> 2;
-    for (uint32_t o = cnt + tid; o < 4u * nq + 4u; o += SPH_THREADS) { C.X[o] = SPH_NANF; C.Y[o] = 0.f; C.Z[o] = 0.f; C.H2[o] = 0.f; }
-    return cnt;
 }
 
 template <int KERNEL>
 __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    ForceCta &C = *reinterpret_cast<ForceCta *>(smem_raw);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    ForceWarp &W = reinterpret_cast<ForceWarp *>(smem_raw)[warp];
     const float L = a.L;
     if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
-    unsigned long long st_cands = 0, st_pairs = 0, st_staged = 0; // thread 0 / warp 0
-    const uint32_t q0 = smem_u32(C.q + tid);
+    unsigned long long st_cands = 0, st_pairs = 0;
+    uint32_t *qp = W.q + lane;
 
+    unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups
     for (;;) {
-        __syncthreads(); // the previous group's shared state is dead
-        if (tid == 0) C.gnext = atomicAdd(&a.cnt->work, 1u);
-        __syncthreads();
-        const unsigned int grp = C.gnext;
-        if (grp >= n_groups) break;
+        if (gnext == gend) {
+            if (lane == 0) gnext = atomicAdd(&a.cnt->work, (unsigned int)SPH_GBLOCK);
+            gnext = __shfl_sync(FULLMASK, gnext, 0);
+            if (gnext >= n_groups) break;
+            gend = min(gnext + SPH_GBLOCK, n_groups);
+        }
+        const unsigned int grp = gnext++;
         const uint32_t i0 = a.gstart[grp];
         const uint32_t i1 = (grp + 1 < n_groups) ? a.gstart[grp + 1] : a.n_items;
         const int g = (int)(i1 - i0);
-        SPH_ASSERT(g >= 1 && g <= SPH_MAXB);
         const int f = streams_for(g);
-        const bool live = tid < g * f;
-        const int ai = live ? tid % g : 0, s = live ? tid / g : 0;
+        const bool live = lane < g * f;
+        const int ai = live ? lane % g : 0, s = live ? lane / g : 0;
         ForceLane A;
-        const uint32_t slot = a.item_slot ? a.item_slot[i0 + ai] : i0 + ai;
-        const float4 p0 = a.xyzh[slot], p1 = a.vc[2 * (size_t)slot], p2 = a.vc[2 * (size_t)slot + 1];
-        A.slot = slot;
-        A.xi = live ? p0.x : SPH_NANF; // dead threads never hit
-        A.yi = p0.y; A.zi = p0.z;
-        A.h2 = p0.w * p0.w;
-        A.hinv = 1.f / p0.w;
-        const float h2i = A.hinv * A.hinv;
-        A.f4 = kern_sigma<KERNEL>() * h2i * h2i;
-        A.vx = p1.x; A.vy = p1.y; A.vz = p1.z; A.c = p1.w;
-        A.rho = p2.x; A.A = p2.y;
-        A.px = A.py = A.pz = A.pdu = 0.0;
-        A.pvs = 0.f;
-        A.cn = A.cnt = 0;
-        // warp 0 (thread i < g holds active i): bounding box and reach of the group
-        if (warp == 0) publish_box(C.W, lane < g, p0.x, p0.y, p0.z, warp_max(lane < g ? p0.w : 0.f));
-        __syncthreads();
-        walk_cta<true>(C.W, a.nodes, a.node_hmax, L, true);
-        unsigned long long cands = 0;
-        for (;;) {
-            const WalkCtl ctl = walk_result(C.W);
-            cands += ctl.total;
-            A.xf = ctl.pairwrap ? A.xi : recentre(A.xi, ctl.thx, L);
-            A.yf = ctl.pairwrap ? A.yi : recentre(A.yi, ctl.thy, L);
-            A.zf = ctl.pairwrap ? A.zi : recentre(A.zi, ctl.thz, L);
-            const uint32_t nt = (ctl.total + SPH_FTILE - 1) / SPH_FTILE;
-            for (uint32_t c = 0; c < nt; c++) {
-                const uint32_t cnt = gather_tile(C, ctl, c, nt, a);
-                st_staged += cnt;
-                __syncthreads();
-                const int nq = (int)((cnt + 3u) >> 2);
-                // queued hits refer to this tile's records: all of them are evaluated before the tile is replaced
-                if (ctl.pairwrap) {
-                    consume<KERNEL, true>(C, a, q0, A, nq, s, f, live);
-                    drain<KERNEL, true>(C, a, q0, A, __reduce_max_sync(FULLMASK, A.cnt));
-                } else {
-                    consume<KERNEL, false>(C, a, q0, A, nq, s, f, live);
-                    drain<KERNEL, false>(C, a, q0, A, __reduce_max_sync(FULLMASK, A.cnt));
+        {
+            const uint32_t slot = a.item_slot ? a.item_slot[i0 + ai] : i0 + ai;
+            const float4 p0 = a.xyzh[slot], p1 = a.vc[2 * (size_t)slot], p2 = a.vc[2 * (size_t)slot + 1];
+            A.slot = slot;
+            A.xi = live ? p0.x : SPH_NANF; // dead lanes never hit
+            A.yi = p0.y; A.zi = p0.z;
+            A.h2 = p0.w * p0.w;
+            A.hinv = 1.f / p0.w;
+            const float h2i = A.hinv * A.hinv;
+            A.f4 = kern_sigma<KERNEL>() * h2i * h2i;
+            A.vx = p1.x; A.vy = p1.y; A.vz = p1.z; A.c = p1.w;
+            A.rho = p2.x; A.A = p2.y;
+            A.px = A.py = A.pz = A.pdu = 0.0;
+            A.pvs = 0.f;
+            A.cn = A.cnt = 0;
+            // bounding box and reach of the group
+            const float inf = __int_as_float(0x7f800000);
+            const float x0 = warp_min(live ? p0.x : inf), x1 = warp_max(live ? p0.x : -inf);
+            const float y0 = warp_min(live ? p0.y : inf), y1 = warp_max(live ? p0.y : -inf);
+            const float z0 = warp_min(live ? p0.z : inf), z1 = warp_max(live ? p0.z : -inf);
+            const float hg = warp_max(live ? p0.w : 0.f);
+            const float gcx = 0.5f * (x0 + x1), ghx = 0.5f * (x1 - x0) * (1.f + 1e-6f);
+            const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
+            const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
+
+            WalkCtl ctl;
+            ctl.sp = -1;
+            unsigned long long cands = 0;
+            Frame fr;
+            fr.thx = fr.thy = fr.thz = __int_as_float(0x7f800000);
+            fr.pairwrap = false;
+            fr.rec = false;
+            do {
+                walk_batch<true>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
+                cands += ctl.total;
+                // queued hits of an earlier batch are evaluated in the frame they were found in
+                if (ctl.pairwrap != fr.pairwrap || ctl.thx != fr.thx || ctl.thy != fr.thy || ctl.thz != fr.thz) {
+                    drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+                    fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
+                    fr.rec = ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f;
                 }
-                __syncthreads();
+                const uint32_t nch = (ctl.total + SPH_CH - 1) / SPH_CH;
+                GatherCtl gc;
+                gc.kseg = 0;
+                // (the register-staged gather pipeline of the density kernel measured slower here: 85.8 vs 76.3 ms)
+                for (uint32_t c = 0; c < nch; c++) {
+                    GatherRegs G;
+                    gather_load(W.ws, ctl, gc, c, G, a.xyzh);
+                    gather_store<true, true>(ctl, G, W.slot, W.gidx, L);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                }
+            } while (ctl.sp > 0);
+            drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+            // cross-stream totals
+            double X = A.px, Y = A.py, Z = A.pz, U = A.pdu;
+            float V = A.pvs;
+            int cn = A.cn;
+            for (int d = 1; d < f; d <<= 1) {
+                const bool take = live && s + d < f;
+                const int from = take ? lane + g * d : lane;
+                const double tX = __shfl_sync(FULLMASK, X, from), tY = __shfl_sync(FULLMASK, Y, from);
+                const double tZ = __shfl_sync(FULLMASK, Z, from), tU = __shfl_sync(FULLMASK, U, from);
+                const float tV = __shfl_sync(FULLMASK, V, from);
+                const int tn = __shfl_sync(FULLMASK, cn, from);
+                if (take) { X += tX; Y += tY; Z += tZ; U += tU; V = fmaxf(V, tV); cn += tn; }
             }
-            if (ctl.sp <= 0) break;
-            walk_cta<true>(C.W, a.nodes, a.node_hmax, L, false);
-        }
-        // cross-stream totals through shared memory (the tile is dead): fp64, ascending stream order
-        double *pX = reinterpret_cast<double *>(C.r0), *pY = pX + SPH_THREADS, *pZ = pY + SPH_THREADS, *pU = pZ + SPH_THREADS;
-        float *pV = reinterpret_cast<float *>(pU + SPH_THREADS);
-        int *pn = reinterpret_cast<int *>(pV + SPH_THREADS);
-        pX[tid] = A.px; pY[tid] = A.py; pZ[tid] = A.pz; pU[tid] = A.pdu; pV[tid] = A.pvs; pn[tid] = A.cn;
-        __syncthreads();
-        if (warp == 0) {
-            double X = 0.0, Y = 0.0, Z = 0.0, U = 0.0;
-            float V = 0.f;
-            int cn = 0;
+            // a11: scatter to the caller's particle id
             if (lane < g) {
-                for (int t = lane; t < g * f; t += g) {
-                    X += pX[t]; Y += pY[t]; Z += pZ[t]; U += pU[t]; V = fmaxf(V, pV[t]); cn += pn[t];
-                }
-                // a11: scatter to the caller's particle id
                 const uint32_t id = a.perm[slot];
                 a.acc[3 * (size_t)id] = (float)X;
                 a.acc[3 * (size_t)id + 1] = (float)Y;
@@ -345,10 +310,9 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
             st_cands += cands * (unsigned long long)g;
         }
     }
-    if (tid == 0) {
+    if (lane == 0) {
         if (st_cands) atomicAdd(&a.cnt->force_cands, st_cands);
         if (st_pairs) atomicAdd(&a.cnt->force_pairs, st_pairs);
-        atomicAdd(&a.cnt->force_staged, st_staged);
     }
 }
 
@@ -394,14 +358,15 @@ __global__ void k_node_hmax(const SphCounters *cnt, const SphNode *__restrict__ 
 template <int KERNEL>
 int launch(sph_ctx *ctx, const ForceArgs &a, int64_t est_groups)
 {
-    size_t dyn = sizeof(ForceCta);
+    size_t dyn = sizeof(ForceWarp) * SPH_WARPS;
     auto kfn = k_force<KERNEL>;
     SPH_CUDA(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
     int per_sm = 1;
     SPH_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kfn, SPH_THREADS, dyn));
     if (per_sm < 1) return sph_fail(ctx, SPH_E_INTERNAL, "k_force does not fit on an SM");
     int64_t grid = (int64_t)ctx->device_sms * per_sm;
-    if (est_groups < grid) grid = est_groups > 0 ? est_groups : 1;
+    int64_t need = (est_groups + SPH_WARPS * SPH_GBLOCK - 1) / (SPH_WARPS * SPH_GBLOCK);
+    if (need < grid) grid = need > 0 ? need : 1;
     kfn<<<(int)grid, SPH_THREADS, dyn, ctx->stream>>>(a);
     SPH_CUDA(ctx, cudaGetLastError());
     return SPH_OK;

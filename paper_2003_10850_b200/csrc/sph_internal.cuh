@@ -17,44 +17,38 @@
 #define SPH_LMAX 16         // octree depth: 16 bits per axis -> 48-bit Morton keys
 #define SPH_KEY_BITS (3 * SPH_LMAX)
 #ifndef SPH_LEAF
-#define SPH_LEAF 32         // octree leaf capacity (a candidate segment is a run of sibling leaves or a whole cell)
+#define SPH_LEAF 32         // octree leaf capacity (a candidate segment is a run of sibling leaves)
 #endif
-#define SPH_MAXB 32         // max actives per group (one CTA per group; thread = (active, candidate stream))
-#define SPH_GCAP_DEFAULT 32 // default actives per group (group nodes are cut into balanced runs)
-#ifndef SPH_GNODE_DEFAULT
-#define SPH_GNODE_DEFAULT 64 // default group node size: highest octree nodes holding <= this many particles
+#define SPH_MAXB 32         // max actives per group (a warp: one lane per active and stream)
+#define SPH_GCAP_DEFAULT 8  // default actives per group (leaves are cut into balanced runs)
+#ifndef SPH_WARPS
+#define SPH_WARPS 4         // warps per CTA of the gather kernels (warps are independent)
 #endif
-#define SPH_WARPS 4         // warps per CTA of the gather kernels
 #define SPH_THREADS (32 * SPH_WARPS)
 #ifndef SPH_CTAS
-#define SPH_CTAS 4          // resident CTAs per SM k_density is compiled for (shared-memory budget)
+#define SPH_CTAS 5          // resident CTAs per SM the gather kernels are compiled for (register budget)
 #endif
+#define SPH_SMAX 128        // candidate segments per walk batch (per warp)
+#define SPH_STK 192         // walk stack entries (blocks of 8 sibling nodes, per warp)
+#define SPH_STK4 48         // 4-block pops only while the stack is at most this deep
+#define SPH_CH 120          // candidates per chunk (60 pairs: divisible by 1..6, 10, 12, 15, 20, 30)
 #ifndef SPH_CTAS_FORCE
-#define SPH_CTAS_FORCE 5    // the same for k_force
-#endif
-#define SPH_SMAX 512        // candidate segments per walk batch (a power of two)
-#define SPH_STK 512         // walk stack entries (blocks of 8 sibling nodes)
-#define SPH_STK16 256       // 16-block pops only while the stack is at most this deep
-#ifndef SPH_DCAP
-#define SPH_DCAP 2240       // density: candidates staged in shared memory at once (resident across the h iteration)
+#define SPH_CTAS_FORCE SPH_CTAS
 #endif
 #ifndef SPH_QCAP
-#define SPH_QCAP 40         // density: per-thread hit-queue entries
-#endif
-#ifndef SPH_QSTEP
-#define SPH_QSTEP 4         // candidate quads (4 tests each) between queue-capacity checks
-#endif
-#ifndef SPH_FTILE
-#define SPH_FTILE 448       // force: candidates per staged tile (test arrays + 48-byte state records)
+#define SPH_QCAP 32         // per-lane hit-queue entries (>= 2 * SPH_QSTEP)
 #endif
 #ifndef SPH_QCAP_FORCE
-#define SPH_QCAP_FORCE 32   // force: per-thread hit-queue entries (16-bit tile-local indices)
+#define SPH_QCAP_FORCE 32   // the same for the force kernel (a hit costs ~95 instructions there: fuller drains pay)
 #endif
-#ifndef SPH_QSTEP_FORCE
-#define SPH_QSTEP_FORCE 2
+#ifndef SPH_QSTEP
+#define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #endif
-#ifndef SPH_REWALK_MARGIN
-#define SPH_REWALK_MARGIN 0.02f // density: a re-walk after the first evaluation reaches this much farther than needed
+#ifndef SPH_NA
+#define SPH_NA 1            // actives per lane of the density gather (1 or 2)
+#endif
+#ifndef SPH_GBLOCK
+#define SPH_GBLOCK 1         // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
 #endif
 
 // octree node, 32 bytes, read as two 16-byte loads
@@ -79,7 +73,6 @@ struct SphCounters {
     unsigned int lvl_begin[SPH_LMAX + 3];
     unsigned int lvl_done[SPH_LMAX + 3];
     unsigned long long dens_evals, dens_cands, dens_pairs, force_cands, force_pairs;
-    unsigned long long dens_group_evals, dens_walks, dens_staged, force_staged; // group evaluations, tree walks, candidates staged in shared memory
 };
 
 struct sph_ctx {

@@ -1,12 +1,12 @@
-// sph_warp.cuh -- device code shared by the gather kernels (steps a5/a6): the octree walk that emits
-// the candidate set of a group as runs of the sorted order, and the shared-memory primitives.
+// sph_warp.cuh -- device code shared by the warp-per-group gather kernels (steps a5/a6):
+// per-warp octree walk that emits candidate leaf segments, and the cooperative gather that stages a
+// chunk of candidates in the warp's shared-memory slot as pair records for packed f32x2 tests.
 //
-// One CTA owns one group of <= 32 active particles that are consecutive in the sorted order inside one
-// small octree node -- the paper's "tree walk over groups of one or more active particles"
-// (§1).  Warp 0 of the CTA walks the tree for the whole group; all warps then stage the
-// candidate runs in shared memory and test them (sph_density.cu, sph_force.cu).  The staged tile plays
-// the role of the paper's N_chunk (PAPER.md:104 §2.4, :108 §3): candidates are consumed tile by tile,
-// never as per-particle neighbour lists in memory.
+// One WARP owns one group of <= 32 active particles that are consecutive in the sorted order inside
+// one octree leaf -- the paper's "tree walk over groups of one or more active particles"
+// (§1).  Warps never synchronise with one another: walk latency of one group hides
+// behind the pair arithmetic of the others.  The chunk plays the role of the paper's N_chunk
+// (PAPER.md:104 §2.4, :108 §3): candidates are consumed in fixed-size chunks, not as whole lists.
 #pragma once
 
 #include "sph_internal.cuh"
@@ -70,36 +70,22 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Walk state of a group, in shared memory.
-struct WalkShared {
-    uint32_t seg_start[SPH_SMAX];   // first sorted slot of each candidate segment (a run of the sorted order)
+// Per-warp walk state.
+struct WarpWalk {
+    uint32_t seg_start[SPH_SMAX];   // first sorted slot of each candidate segment (a leaf)
     uint32_t seg_pre[SPH_SMAX + 1]; // exclusive prefix of the segment lengths; [n_seg] = total
     uint32_t stack[SPH_STK];        // blocks of 8 sibling nodes still to visit
-    int sp, n_seg;                  // stack pointer and segment count between the steps of a batch
-    int wcnt[SPH_WARPS][2];         // per warp: segment heads / pushes of the current step
-    float wmax[SPH_WARPS][2];       // per warp: largest emitted cell half edge, largest reach
-    float box[7];                   // the group: bounding box centre (3), half extent (3), reach
-    // Result of the batch.  Frame (see the end of walk_cta): per axis, coordinates >= thr are shifted
-    // by -L (thr = +inf: axis untouched); pairwrap: per-pair nearest image needed instead.
-    uint32_t total;
-    float thx, thy, thz;
-    int pairwrap;
 };
 
-// the batch result as registers of every thread
-struct WalkCtl {
-    int sp, n_seg;
+struct WalkCtl { // warp-uniform registers
+    int sp;        // stack pointer; -1: walk not started
+    int n_seg;
     uint32_t total;
+    // Frame of this batch (see the end of walk_batch): per axis, coordinates >= thr are shifted by -L
+    // (thr = +inf: axis untouched); pairwrap: per-pair nearest image needed instead.
     float thx, thy, thz;
     bool pairwrap;
 };
-__device__ __forceinline__ WalkCtl walk_result(const WalkShared &W)
-{
-    WalkCtl c;
-    c.sp = W.sp; c.n_seg = W.n_seg; c.total = W.total;
-    c.thx = W.thx; c.thy = W.thy; c.thz = W.thz; c.pairwrap = W.pairwrap != 0;
-    return c;
-}
 
 // coordinate in the batch's frame: exact (x - L is exact for x >= L/2, Sterbenz)
 __device__ __forceinline__ float recentre(float x, float thr, float L) { return x >= thr ? x - L : x; }
@@ -115,67 +101,56 @@ __device__ __forceinline__ SphNode load_node(const SphNode *__restrict__ nodes, 
     return n;
 }
 
-// Starts (start = true) or continues the depth-first walk of the CTA's group and fills one batch of
-// candidate segments: every leaf whose cell comes closer to the group's bounding box (W.box: centre,
-// half extent) than the reach (density: hg = W.box[6]; force: max(hg, largest support radius inside
-// the node), the symmetric set of R10), and every cell that lies wholly within hg of the box.  Called
-// by ALL threads of the CTA: a step pops up to 16 blocks of 8 siblings, one node per thread, so the
-// chain of dependent node loads is as short as the tree is deep, not as long as the candidate list.
-// Stack bound: 16-block pops only while sp <= SPH_STK16 (+112 at most), single-block pops grow the
-// stack by <= 7 per tree level: sp <= SPH_STK16 + 112 + 8 * SPH_LMAX <= SPH_STK.
-// On return (after a __syncthreads) W.sp > 0 means the walk is not finished: call again.
+// Continues (or starts, ctl.sp == -1) the depth-first walk of this warp's group and fills one batch
+// of candidate segments: every leaf whose cell comes closer to the group's bounding box (centre gc,
+// half extent gh) than the reach (density: hg; force: max(hg, largest support radius inside the
+// node), the symmetric set of R10).  Stack entries are blocks of 8 siblings; a step pops up to 4
+// blocks (one node per lane).  Stack bound: 4-block pops only while sp <= SPH_STK4, single-block
+// pops grow the stack by <= 7 per tree level, so sp <= SPH_STK4 + 28 + 7 * SPH_LMAX < SPH_STK.
 template <bool FORCE>
-__device__ __forceinline__ void walk_cta(WalkShared &W, const SphNode *__restrict__ nodes,
-                                         const float *__restrict__ node_hmax, float L, bool start)
+__device__ __forceinline__ void walk_batch(WarpWalk &ws, WalkCtl &ctl, const SphNode *__restrict__ nodes,
+                                           const float *__restrict__ node_hmax, float L, float gcx, float gcy,
+                                           float gcz, float ghx, float ghy, float ghz, float hg)
 {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const float gcx = W.box[0], gcy = W.box[1], gcz = W.box[2], ghx = W.box[3], ghy = W.box[4], ghz = W.box[5];
-    const float hg = W.box[6];
+    const int lane = threadIdx.x & 31;
+    int sp = ctl.sp, n_seg = 0;
     float maxhalf = 0.f, maxreach = hg;
     const float pad = 1e-6f * L;
-    if (tid == 0) {
-        W.n_seg = 0;
-        if (start) {
-            SphNode root = load_node(nodes, 0);
-            W.sp = 0;
-            if (root.child == 0) {
-                if (root.count > 0) {
-                    W.seg_start[0] = root.start; W.seg_pre[0] = root.count;
-                    W.n_seg = 1; maxhalf = root.half;
-                }
-                if (FORCE) maxreach = fmaxf(maxreach, __ldg(node_hmax));
-            } else {
-                W.stack[0] = root.child;
-                W.sp = 1;
+    __syncwarp();
+    if (sp < 0) { // start
+        SphNode root = load_node(nodes, 0);
+        sp = 0;
+        if (root.child == 0) {
+            if (root.count > 0) {
+                if (lane == 0) { ws.seg_start[0] = root.start; ws.seg_pre[0] = root.count; }
+                n_seg = 1; maxhalf = root.half;
             }
+            if (FORCE) maxreach = fmaxf(maxreach, __ldg(node_hmax));
+        } else {
+            if (lane == 0) ws.stack[0] = root.child;
+            sp = 1;
         }
+        __syncwarp();
     }
-    for (;;) {
-        __syncthreads();
-        const int sp0 = W.sp, ns0 = W.n_seg;
-        if (sp0 <= 0 || ns0 > SPH_SMAX - SPH_THREADS) break;
-        const int npop = sp0 <= SPH_STK16 ? min(sp0, SPH_THREADS / 8) : 1;
-        const int e = tid >> 3;
-        const bool valid = e < npop;
-        const uint32_t idx = valid ? W.stack[sp0 - npop + e] + (tid & 7) : 0u;
+    while (sp > 0 && n_seg <= SPH_SMAX - 32) {
+        int npop = sp <= SPH_STK4 ? min(sp, 4) : 1;
+        sp -= npop;
+        int e = lane >> 3;
+        bool valid = e < npop;
+        uint32_t idx = valid ? ws.stack[sp + e] + (lane & 7) : 0u;
         SphNode nd = load_node(nodes, idx);
         float reach = hg;
         if (FORCE) reach = fmaxf(reach, __ldg(node_hmax + idx));
-        const float hh = nd.half * (1.f + 1e-6f) + pad;
-        const float ax = fabsf(gcx - nd.cx), ay = fabsf(gcy - nd.cy), az = fabsf(gcz - nd.cz);
-        const float mx = fminf(ax, L - ax), my = fminf(ay, L - ay), mz = fminf(az, L - az); // periodic separation of the centres
-        const float dx = fmaxf(mx - (ghx + hh), 0.f), dy = fmaxf(my - (ghy + hh), 0.f), dz = fmaxf(mz - (ghz + hh), 0.f);
-        const float d2 = dx * dx + dy * dy + dz * dz;
-        const float rp = reach * (1.f + 1e-5f);
-        const bool pass = valid && nd.count > 0 && d2 <= rp * rp;
-        const bool leaf = nd.child == 0;
-        // A cell EVERY point of which lies within the group's own reach of the bounding box is emitted
-        // whole, as one long run of the sorted order: none of its descendants could be pruned (their
-        // nearest point is no farther than that), so descending would only cut the run into pieces.
-        const float fx = fmaxf(mx + hh - ghx, 0.f), fy = fmaxf(my + hh - ghy, 0.f), fz = fmaxf(mz + hh - ghz, 0.f);
-        const bool inside = fx * fx + fy * fy + fz * fz <= hg * hg;
-        const bool emit = pass && (leaf || inside), push = pass && !emit;
-        // Sibling cells are consecutive runs of the sorted order: a run of emitted siblings (empty ones
+        float hh = nd.half * (1.f + 1e-6f) + pad;
+        float dx = fabsf(gcx - nd.cx); dx = fminf(dx, L - dx); dx = fmaxf(dx - (ghx + hh), 0.f);
+        float dy = fabsf(gcy - nd.cy); dy = fminf(dy, L - dy); dy = fmaxf(dy - (ghy + hh), 0.f);
+        float dz = fabsf(gcz - nd.cz); dz = fminf(dz, L - dz); dz = fmaxf(dz - (ghz + hh), 0.f);
+        float d2 = dx * dx + dy * dy + dz * dz;
+        float rp = reach * (1.f + 1e-5f);
+        bool pass = valid && nd.count > 0 && d2 <= rp * rp;
+        bool leaf = nd.child == 0;
+        bool emit = pass && leaf, push = pass && !leaf;
+        // Sibling leaves are consecutive runs of the sorted order: a run of emitted siblings (empty ones
         // in between do not matter) becomes ONE segment, emitted by the run's first lane.
         const unsigned me = __ballot_sync(FULLMASK, emit);
         const unsigned mbrk = __ballot_sync(FULLMASK, valid && nd.count > 0 && !emit);
@@ -188,94 +163,81 @@ __device__ __forceinline__ void walk_cta(WalkShared &W, const SphNode *__restric
         const int last = 31 - __clz(runm | (1u << lane));           // last emitted sibling of the run
         const uint32_t endpos = __shfl_sync(FULLMASK, nd.start + nd.count, last);
         const unsigned mh = __ballot_sync(FULLMASK, head);
-        const unsigned mp = __ballot_sync(FULLMASK, push);
         if (emit) {
-            if (!inside) maxhalf = fmaxf(maxhalf, nd.half); // (every point of an inside cell lies within hg of the box)
+            maxhalf = fmaxf(maxhalf, nd.half);
             maxreach = fmaxf(maxreach, reach);
         }
-        if (lane == 0) { W.wcnt[warp][0] = __popc(mh); W.wcnt[warp][1] = __popc(mp); }
-        __syncthreads();
-        int sb = ns0, pb = sp0 - npop, st = 0, pt = 0;
-#pragma unroll
-        for (int w = 0; w < SPH_WARPS; w++) {
-            const int a = W.wcnt[w][0], b = W.wcnt[w][1];
-            if (w < warp) { sb += a; pb += b; }
-            st += a; pt += b;
-        }
         if (head) {
-            const int p = sb + __popc(mh & lanemask_lt());
+            int p = n_seg + __popc(mh & lanemask_lt());
             SPH_ASSERT(p < SPH_SMAX);
-            W.seg_start[p] = nd.start;
-            W.seg_pre[p] = endpos - nd.start;
+            ws.seg_start[p] = nd.start;
+            ws.seg_pre[p] = endpos - nd.start;
         }
-        if (push) {
-            SPH_ASSERT(pb + __popc(mp & lanemask_lt()) < SPH_STK);
-            W.stack[pb + __popc(mp & lanemask_lt())] = nd.child;
-        }
-        if (tid == 0) { W.sp = sp0 - npop + pt; W.n_seg = ns0 + st; }
+        n_seg += __popc(mh);
+        unsigned mp = __ballot_sync(FULLMASK, push);
+        SPH_ASSERT(sp + __popc(mp) <= SPH_STK);
+        if (push) ws.stack[sp + __popc(mp & lanemask_lt())] = nd.child;
+        sp += __popc(mp);
+        __syncwarp();
     }
-    // (every thread has passed the loop's last barrier; W.sp / W.n_seg are final)
     maxhalf = warp_max(maxhalf);
     maxreach = warp_max(maxreach);
-    if (lane == 0) { W.wmax[warp][0] = maxhalf; W.wmax[warp][1] = maxreach; }
-    const int n_seg = W.n_seg;
-    if (warp == 0) {
-        // exclusive prefix of the segment lengths (in place)
-        uint32_t carry = 0;
-        for (int b = 0; b < n_seg; b += 32) {
-            const int i = b + lane;
-            const uint32_t v = i < n_seg ? W.seg_pre[i] : 0u;
-            uint32_t inc = v;
+    // exclusive prefix of the segment lengths (in place)
+    uint32_t carry = 0;
+    for (int b = 0; b < n_seg; b += 32) {
+        int i = b + lane;
+        uint32_t v = i < n_seg ? ws.seg_pre[i] : 0u, inc = v;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(FULLMASK, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (i < n_seg) W.seg_pre[i] = carry + inc - v;
-            carry += __shfl_sync(FULLMASK, inc, 31);
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(FULLMASK, inc, o);
+            if (lane >= o) inc += t;
         }
-        if (lane == 0) { W.seg_pre[n_seg] = carry; W.total = carry; }
+        if (i < n_seg) ws.seg_pre[i] = carry + inc - v;
+        carry += __shfl_sync(FULLMASK, inc, 31);
     }
-    __syncthreads();
-    if (tid == 0) {
-#pragma unroll
-        for (int w = 0; w < SPH_WARPS; w++) { maxhalf = fmaxf(maxhalf, W.wmax[w][0]); maxreach = fmaxf(maxreach, W.wmax[w][1]); }
-        // Frame choice, per axis.  ext bounds how far any candidate of this batch can lie from the group's
-        // bounding box.  (i) The group, its reach and every candidate cell stay clear of both box faces:
-        // plain differences of raw coordinates ARE the minimum-image differences (thr = +inf).  (ii) They
-        // cross a face but span less than half the box: map every coordinate x >= L/2 to x - L (exact), for
-        // actives and candidates alike; all of them then lie in one interval inside (-L/2, L/2) and plain
-        // differences are again the minimum-image differences, while a candidate outside that span can only
-        // look farther away than it is, never closer.  (iii) Otherwise (a reach comparable to the box):
-        // per-pair image.
-        const float inf = __int_as_float(0x7f800000);
-        const float ext = maxreach * (1.f + 1e-5f) + 2.f * maxhalf + 4.f * pad;
-        const float hl = 0.5f * L, ql = 0.249f * L; // span = 2 (gh + ext) < L/2
-        const bool okx = gcx - ghx - ext >= 0.f && gcx + ghx + ext < L;
-        const bool oky = gcy - ghy - ext >= 0.f && gcy + ghy + ext < L;
-        const bool okz = gcz - ghz - ext >= 0.f && gcz + ghz + ext < L;
-        W.thx = okx ? inf : hl;
-        W.thy = oky ? inf : hl;
-        W.thz = okz ? inf : hl;
-        W.pairwrap = ((!okx && ghx + ext >= ql) || (!oky && ghy + ext >= ql) || (!okz && ghz + ext >= ql)) ? 1 : 0;
-    }
-    __syncthreads();
+    if (lane == 0) ws.seg_pre[n_seg] = carry;
+    __syncwarp();
+    ctl.sp = sp;
+    ctl.n_seg = n_seg;
+    ctl.total = carry;
+    // Frame choice, per axis.  ext bounds how far any candidate of this batch can lie from the group's
+    // bounding box.  (i) The group, its reach and every candidate cell stay clear of both box faces:
+    // plain differences of raw coordinates ARE the minimum-image differences (thr = +inf).  (ii) They
+    // cross a face but span less than half the box: map every coordinate x >= L/2 to x - L (exact), for
+    // actives and candidates alike; all of them then lie in one interval inside (-L/2, L/2) and plain differences are
+    // again the minimum-image differences, while a candidate outside that span can only look farther
+    // away than it is, never closer.  (iii) Otherwise (a reach comparable to the box): per-pair image.
+    const float inf = __int_as_float(0x7f800000);
+    const float ext = maxreach * (1.f + 1e-5f) + 2.f * maxhalf + 4.f * pad;
+    const float hl = 0.5f * L, ql = 0.249f * L; // span = 2 (gh + ext) < L/2
+    const bool okx = gcx - ghx - ext >= 0.f && gcx + ghx + ext < L;
+    const bool oky = gcy - ghy - ext >= 0.f && gcy + ghy + ext < L;
+    const bool okz = gcz - ghz - ext >= 0.f && gcz + ghz + ext < L;
+    ctl.thx = okx ? inf : hl;
+    ctl.thy = oky ? inf : hl;
+    ctl.thz = okz ? inf : hl;
+    ctl.pairwrap = (!okx && ghx + ext >= ql) || (!oky && ghy + ext >= ql) || (!okz && ghz + ext >= ql);
 }
 
-// the group's bounding box and reach, published by warp 0 (has: this lane holds an active of the group)
-__device__ __forceinline__ void publish_box(WalkShared &W, bool has, float x, float y, float z, float reach)
-{
-    const float inf = __int_as_float(0x7f800000);
-    const float x0 = warp_min(has ? x : inf), x1 = warp_max(has ? x : -inf);
-    const float y0 = warp_min(has ? y : inf), y1 = warp_max(has ? y : -inf);
-    const float z0 = warp_min(has ? z : inf), z1 = warp_max(has ? z : -inf);
-    if ((threadIdx.x & 31) == 0) {
-        W.box[0] = 0.5f * (x0 + x1); W.box[3] = 0.5f * (x1 - x0) * (1.f + 1e-6f);
-        W.box[1] = 0.5f * (y0 + y1); W.box[4] = 0.5f * (y1 - y0) * (1.f + 1e-6f);
-        W.box[2] = 0.5f * (z0 + z1); W.box[5] = 0.5f * (z1 - z0) * (1.f + 1e-6f);
-        W.box[6] = reach;
-    }
-}
+// ---------------------------------------------------------------------------------------------
+// Candidate staging.  A batch's candidates form one flat index space [0, total) (segment k covers
+// [seg_pre[k], seg_pre[k+1])); chunk c = flat range [c*CH, c*CH+CH).  The warp gathers a chunk into its
+// shared-memory slot itself: lane l takes the four consecutive entries 4l..4l+3, finds their segments
+// (segment heads become bits of a warp-uniform mask; the rank of a position is a population count), loads the
+// four float4 records (one 64-byte run per lane unless a segment boundary intervenes), moves the
+// coordinates into the batch's frame (recentre) and writes them as PAIR records, pair p of the chunk =
+//   slot[p] = (x0,x1,y0,y1)   slot[SPH_CH/2 + p] = (z0,z1,w0,w1)
+// so that the test loops load register pairs ready for packed f32x2 arithmetic.  Entries beyond the
+// ragged tail become NaN (every comparison with NaN is false).
+//
+// Why not TMA bulk copies here (they were the first design, profiles/r1c_packed_tma.md): octree leaves hold ~8
+// particles on average, so a chunk is ~10 pieces of ~100 bytes at arbitrary 16-byte offsets; every
+// piece is one UBLKCP issued through uniform registers, which the compiler serialises lane by lane
+// (ELECT / R2UR / UBLKCP, ~10 issue slots and a long-scoreboard wait per piece): 30 % of the kernel's
+// time went there.  Tiles this small and irregular are not TMA's case; per-lane 16-byte loads are.
+struct GatherCtl { // warp-uniform registers
+    int kseg; // first segment that overlaps the next chunk to gather
+};
 
 __device__ __forceinline__ float4 ldg_nc(const float4 *p)
 {
@@ -284,47 +246,94 @@ __device__ __forceinline__ float4 ldg_nc(const float4 *p)
     return v;
 }
 
-// segment that holds flat position p: largest k < n_seg with seg_pre[k] <= p (branch-free bisection)
-__device__ __forceinline__ int seg_of(const WalkShared &W, int n_seg, uint32_t p)
-{
-    int k = 0;
-#pragma unroll
-    for (int step = SPH_SMAX / 2; step; step >>= 1) {
-        const int k2 = k + step;
-        if (k2 < n_seg && W.seg_pre[k2] <= p) k = k2;
-    }
-    return k;
-}
-
-// Thread layout of a group of g actives in a CTA: thread = a + g * s with a < g the active and s < f the
-// candidate stream, f = floor(SPH_THREADS / g); stream s tests the candidate quads s, s + f, s + 2f, ...
-__device__ __forceinline__ int streams_for(int g) { return SPH_THREADS / g; }
-
-// ---------------------------------------------------------------------------------------------
-// Order in which a staged set of cnt candidates is consumed.  The walk emits candidates in Morton
-// (depth-first) order, so consecutive flat positions are spatial neighbours: they are inside or outside
-// an active's support TOGETHER.  Tested in that order, (i) at any time only the threads whose active
-// lies near the current stretch collect hits, and (ii) a thread's share of the hits, taken in clumps,
-// scatters by a factor of two around the mean -- either way the bulk evaluation of queued hits runs on
-// a few lanes.  The set is therefore dealt candidate by candidate, round-robin, onto SPH_PILES piles
-// that are stored one after the other (slot = (o mod P) * pl + o / P): every stretch of the stored
-// order is a uniform sample of the whole set and no two candidates of a quad are neighbours, so every
-// thread meets its hits at a steady rate and ends with its fair share.  pl is odd: the 32 lanes of a
-// gather window store into 32 different piles, i.e. 32 different banks.
-#define SPH_PILES 64
-struct PileMap {
-    uint32_t pl;   // slots per pile
-    uint32_t np;   // slots in use = SPH_PILES * pl (a multiple of 64)
+// The gather is split in two, so that the loads of chunk c + 1 can be in flight while chunk c is
+// tested: gather_load computes the addresses and issues the 16-byte loads into registers, gather_store
+// (after the consumer is done with the slot) fixes up and writes the pair records
+// (slotp: [SPH_CH] float4; gidx: [SPH_CH] sorted slot of every entry or NULL).
+struct GatherRegs {
+    float4 c[4];   // entries 2 l, 2 l + 1, 2 (l + 32), 2 (l + 32) + 1 of the chunk
+    uint32_t j[4]; // their sorted slots
+    uint32_t lo, hi;
 };
-__device__ __forceinline__ PileMap pile_map(uint32_t cnt)
+
+__device__ __forceinline__ void gather_load(const WarpWalk &ws, const WalkCtl &ctl, GatherCtl &gc, uint32_t chunk,
+                                            GatherRegs &G, const float4 *__restrict__ src)
 {
-    PileMap m;
-    m.pl = ((cnt + SPH_PILES - 1u) / SPH_PILES) | 1u;
-    m.np = SPH_PILES * m.pl;
-    return m;
+    const int lane = threadIdx.x & 31;
+    const uint32_t lo = chunk * SPH_CH, hi = min(lo + SPH_CH, ctl.total);
+    G.lo = lo; G.hi = hi;
+    const int kfirst = gc.kseg;
+    uint32_t w0 = 0u, w1 = 0u, w2 = 0u, w3 = 0u;
+    int k0 = kfirst;
+    for (;;) {
+        const int k = k0 + lane;
+        const bool in = k < ctl.n_seg;
+        const uint32_t p0 = in ? ws.seg_pre[k] : 0xffffffffu, p1 = in ? ws.seg_pre[k + 1] : 0xffffffffu;
+        const bool ov = in && p0 < hi && p1 > lo;
+        const uint32_t pos = max(p0, lo) - lo, bit = ov ? 1u << (pos & 31u) : 0u, wd = pos >> 5;
+        w0 |= __reduce_or_sync(FULLMASK, wd == 0u ? bit : 0u);
+        w1 |= __reduce_or_sync(FULLMASK, wd == 1u ? bit : 0u);
+        w2 |= __reduce_or_sync(FULLMASK, wd == 2u ? bit : 0u);
+        w3 |= __reduce_or_sync(FULLMASK, wd == 3u ? bit : 0u);
+        const unsigned m = __ballot_sync(FULLMASK, in && p1 > hi);
+        if (m) { k0 += __ffs(m) - 1; break; }
+        k0 += 32;
+        if (k0 >= ctl.n_seg) { k0 = ctl.n_seg; break; }
+    }
+    gc.kseg = k0;
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+        const int pr = lane + 32 * r;
+        if (pr < SPH_CH / 2) {
+            const int e0 = 2 * pr, wl = e0 >> 5, sh = e0 & 31;
+            const uint32_t wmine = wl == 0 ? w0 : wl == 1 ? w1 : wl == 2 ? w2 : w3;
+            const int below = kfirst - 1 + (wl > 0 ? __popc(w0) : 0) + (wl > 1 ? __popc(w1) : 0) + (wl > 2 ? __popc(w2) : 0);
+            const int ka = below + __popc(wmine & (0xffffffffu >> (31 - sh)));
+            const int kb = below + __popc(wmine & (0xffffffffu >> (30 - sh)));
+            SPH_ASSERT(ka >= kfirst && kb < ctl.n_seg);
+            const uint32_t pa = min(lo + e0, hi - 1u), pb = min(lo + e0 + 1u, hi - 1u);
+            G.j[2 * r] = ws.seg_start[ka] + (pa - ws.seg_pre[ka]);
+            G.j[2 * r + 1] = ws.seg_start[kb] + (pb - ws.seg_pre[kb]);
+            G.c[2 * r] = ldg_nc(src + G.j[2 * r]);
+            G.c[2 * r + 1] = ldg_nc(src + G.j[2 * r + 1]);
+        }
+    }
 }
-__device__ __forceinline__ uint32_t pile_slot(const PileMap &m, uint32_t o) // flat offset in the set -> stored slot
+
+template <bool SQUARE_W, bool NEED_W>
+__device__ __forceinline__ void gather_store(const WalkCtl &ctl, GatherRegs &G, float4 *slotp, uint32_t *gidx, float L)
 {
-    return (o & (SPH_PILES - 1u)) * m.pl + o / SPH_PILES;
+    const int lane = threadIdx.x & 31;
+    __syncwarp(); // every lane is done reading the slot's previous contents
+    const bool rec = !ctl.pairwrap && (ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f); // warp-uniform
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+        const int pr = lane + 32 * r;
+        if (pr < SPH_CH / 2) {
+            float4 ca = G.c[2 * r], cb = G.c[2 * r + 1];
+            const uint32_t e0 = 2u * pr;
+            if (G.lo + e0 >= G.hi) ca.x = SPH_NANF;
+            if (G.lo + e0 + 1u >= G.hi) cb.x = SPH_NANF;
+            if (rec) {
+                ca.x = recentre(ca.x, ctl.thx, L); ca.y = recentre(ca.y, ctl.thy, L); ca.z = recentre(ca.z, ctl.thz, L);
+                cb.x = recentre(cb.x, ctl.thx, L); cb.y = recentre(cb.y, ctl.thy, L); cb.z = recentre(cb.z, ctl.thz, L);
+            }
+            if (SQUARE_W) { ca.w *= ca.w; cb.w *= cb.w; }
+            slotp[pr] = make_float4(ca.x, cb.x, ca.y, cb.y);
+            if (NEED_W) slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, ca.w, cb.w);
+            else slotp[SPH_CH / 2 + pr] = make_float4(ca.z, cb.z, 0.f, 0.f); // w is never read: its registers are free during the tests
+            if (gidx) reinterpret_cast<uint2 *>(gidx)[pr] = make_uint2(G.j[2 * r], G.j[2 * r + 1]);
+        }
+    }
+    __syncwarp();
 }
-#define SPH_PILE_SLACK (2 * SPH_PILES) // slots a set of cnt candidates can need beyond cnt (rounding of pl)
+
+// Lane layout of a group of g actives: lane = a + g * s with a < g the active and s < f the candidate
+// stream; f is the largest divisor of SPH_CH / 2 (candidate pairs per chunk) with g * f <= 32, so that
+// every chunk splits evenly over the streams.
+__device__ __forceinline__ int streams_for(int g)
+{
+    int f = 32 / g;
+    while ((SPH_CH / 2) % f) f--;
+    return f;
+}

@@ -10,7 +10,10 @@ from paper_2003_10850_b200 import binding as B
 
 RTOL_RHO = 1e-5    # north_star: density and h within 1e-5 relative
 RTOL_FORCE = 1e-4  # north_star: acceleration and du/dt within 1e-4 relative
-FLOOR = 1e-2       # DESIGN.md R15: |a| is compared against max(|a|, FLOOR * sum_j |pair term|)
+FLOOR = 1e-3       # DESIGN.md R15: |a| is compared against max(|a|, FLOOR * sum_j |pair term|)
+FLOOR_E2E = 1.0    # DESIGN.md R15c: end-to-end force (each side's own H, rho, Omega, equal only to 1e-5)
+ULPS = 16          # DESIGN.md R15: fp32 resolution of a sum of pair terms, ULPS * 2^-24 * sqrt(sum_j term_j^2)
+EDGE_MAX = 0.02    # upper bound on the edge-class fraction of an end-to-end density comparison
 
 
 def dev(a, dtype=None):
@@ -71,21 +74,24 @@ def check_density_stage(g, o, sel=None, label=""):
     rel = np.abs(grho - o["rho"]) / o["rho"]
     assert rel.max() <= RTOL_RHO, f"{label}: rho rel err {rel.max():.3e}"
     om_o = o["omega"]
-    # Omega = 1 - D/(3S) cancels (exactly to 0 for a lone particle): its error is measured against the
-    # magnitude of the terms that cancel, 1 + |1 - Omega| (R15); for converged sets Omega ~ 1 and
-    # this is the plain 1e-5 relative bound
-    relo = np.abs(gom - om_o) / (1.0 + np.abs(1.0 - om_o))
+    # Omega: plain 1e-5 relative (north_star).  Only where Omega = 1 - D/(3S) has cancelled to |Omega| < 0.5
+    # (arbitrary, unconverged H of the randomised sets; exactly 0 for a lone particle) is its error measured
+    # against the magnitude of the terms that cancel, 1 + |1 - Omega| (R15b)
+    small = np.abs(om_o) < 0.5
+    relo = np.where(small, np.abs(gom - om_o) / (1.0 + np.abs(1.0 - om_o)), np.abs(gom - om_o) / np.maximum(np.abs(om_o), 0.5))
     assert relo.max() <= RTOL_RHO, f"{label}: omega err {relo.max():.3e}"
     return dict(n_edge=int(edge.sum()), n_mismatch=int(mism.sum()), rho_err=float(rel.max()), omega_err=float(relo.max()))
 
 
 def check_density_e2e(g, o, ps_pos, h_guess, kernel, mass_scalar, n_target, n_tol, count_mode=0, sel=None, label="",
-                      box=1.0, mass=None):
+                      box=1.0, mass=None, edge_max=EDGE_MAX):
     """End-to-end iteration parity: non-edge particles H, rho to 1e-5 and N_int exact; edge-class
     particles are counted and checked conditionally (oracle re-evaluated at the GPU's H)."""
     idx = np.arange(len(g["H"])) if sel is None else np.asarray(sel)
     gH, grho, gn = g["H"][idx].astype(np.float64), g["rho"][idx].astype(np.float64), g["Nint"][idx]
     edge = o["edge"] != 0
+    # the edge classes excuse a particle from the strict comparison: they must stay rare, or the test is hollow
+    assert edge_max is None or edge.mean() <= edge_max or edge.sum() <= 2, f"{label}: edge-class fraction {edge.mean():.4f} > {edge_max}"
     relH = np.abs(gH - o["H"]) / o["H"]
     relr = np.abs(grho - o["rho"]) / o["rho"]
     ok = (relH <= RTOL_RHO) & (relr <= RTOL_RHO) & (gn == o["Nint"])
@@ -108,26 +114,53 @@ def check_density_e2e(g, o, ps_pos, h_guess, kernel, mass_scalar, n_target, n_to
         assert np.all(np.abs(grho[chk] - e["rho"]) <= RTOL_RHO * e["rho"])
         mm = gn[chk] != e["Nint"]
         assert np.all(e["edge"][mm] != 0)
-    return dict(n_edge=int(edge.sum()), n_conditional=int(n_cond), H_err=float(relH[ok].max() if ok.any() else 0),
+    return dict(n_edge=int(edge.sum()), edge_fraction=float(edge.mean()), n_conditional=int(n_cond), H_err=float(relH[ok].max() if ok.any() else 0),
                 rho_err=float(relr[ok].max() if ok.any() else 0))
 
 
-def check_force(g, o, sel=None, label="", skip_vsig_edge=True):
+def untainted(pos, H, edge, box=1.0):
+    """Particles that are not edge class and have no edge-class particle among their force neighbours
+    (r < max(H_i, H_j), with a margin): the set on which an end-to-end force comparison is meaningful."""
+    from scipy.spatial import cKDTree
+    ok = ~edge
+    ids = np.flatnonzero(edge)
+    if len(ids) == 0:
+        return ok
+    P = np.mod(pos.astype(np.float64), box)
+    tree = cKDTree(P, boxsize=box)
+    etree = cKDTree(P[ids], boxsize=box)
+    for lst in tree.query_ball_point(P[ids], r=H[ids] * 1.001):  # particles inside an edge particle's support
+        ok[lst] = False
+    hit = etree.query_ball_point(P, r=H * 1.001, return_length=True)  # edge particles inside a particle's support
+    ok &= hit == 0
+    return ok
+
+
+def check_force(g, o, sel=None, label="", skip_vsig_edge=True, floor=FLOOR, mask=None):
     idx = slice(None) if sel is None else sel
     ga, gd, gv = g["acc"][idx].astype(np.float64), g["dudt"][idx].astype(np.float64), g["vsig"][idx].astype(np.float64)
     amag = np.sqrt((o["acc"] ** 2).sum(1))
-    tol_a = RTOL_FORCE * np.maximum(amag, FLOOR * o["asum"])
+    res = ULPS * 2.0 ** -24
+    tol_a = RTOL_FORCE * np.maximum(amag, floor * o["asum"]) + res * np.sqrt(o["asq"])
     err_a = np.sqrt(((ga - o["acc"]) ** 2).sum(1))
     tol_a = np.where(tol_a > 0, tol_a, 1e-30)
+    if mask is not None:  # compare only the particles selected by the mask
+        tol_a = np.where(mask, tol_a, np.inf)
     assert np.all(err_a <= tol_a), f"{label}: acc err/tol max {np.max(err_a / tol_a):.3f} at {np.argmax(err_a / tol_a)}"
-    tol_d = RTOL_FORCE * np.maximum(np.abs(o["dudt"]), FLOOR * o["dusum"])
+    tol_d = RTOL_FORCE * np.maximum(np.abs(o["dudt"]), floor * o["dusum"]) + res * np.sqrt(o["dusq"])
     tol_d = np.where(tol_d > 0, tol_d, 1e-30)
+    if mask is not None:
+        tol_d = np.where(mask, tol_d, np.inf)
     err_d = np.abs(gd - o["dudt"])
-    assert np.all(err_d <= tol_d), f"{label}: dudt err/tol max {np.max(err_d / tol_d):.3f}"
+    wd = int(np.argmax(err_d / tol_d))
+    assert np.all(err_d <= tol_d), (f"{label}: dudt err/tol max {np.max(err_d / tol_d):.3f} at {wd}: npair {o['npair'][wd]} "
+                                    f"dudt {o['dudt'][wd]:.3e} dusum {o['dusum'][wd]:.3e} err {err_d[wd]:.3e}")
     edge = o["edge"] != 0
     relv = np.abs(gv - o["vsig"]) / np.maximum(o["vsig"], 1e-30)
     relv = np.where(o["vsig"] == 0, np.abs(gv), relv)
     m = ~edge if skip_vsig_edge else np.ones_like(edge)
+    if mask is not None:
+        m = m & mask
     assert np.all(relv[m] <= RTOL_RHO), f"{label}: vsig rel err {relv[m].max():.3e}"
     return dict(acc_err_over_tol=float(np.max(err_a / tol_a)), acc_relerr_max=float(np.max(err_a / np.maximum(amag, 1e-300))),
                 dudt_err_over_tol=float(np.max(err_d / tol_d)), vsig_err=float(relv[m].max() if m.any() else 0),

@@ -14,8 +14,31 @@ from parity_util import GpuRun, check_density_e2e, check_force
 
 pytestmark = pytest.mark.gpu
 
-SAMPLE = 192
+SAMPLE = 4096
 _cache = {}
+
+
+def _stratified_sample(ps, pool, rng):
+    """SAMPLE particle ids of the pool.  Sets with haloes (generator metadata aux["halo"], aux["radius"]) are
+    sampled by strata of halo-centric radius -- background, then eight logarithmic bins of r / r_vir down to the
+    cusps -- so that the deep octree levels and the cores of the largest haloes are represented; other sets
+    uniformly."""
+    aux = ps.aux
+    if "halo" not in aux or "r_vir" not in aux:
+        return np.sort(rng.choice(pool, min(SAMPLE, len(pool)), replace=False)).astype(np.int32)
+    halo = aux["halo"][pool]
+    x = np.where(halo >= 0, aux["radius"][pool] / aux["r_vir"][np.maximum(halo, 0)], np.inf)
+    edges = np.concatenate([[0.0], np.logspace(-2.5, 0.0, 8)])
+    strata = [pool[halo < 0]] + [pool[(halo >= 0) & (x > lo) & (x <= hi)] for lo, hi in zip(edges[:-1], edges[1:])]
+    strata = [st for st in strata if len(st)]
+    per = SAMPLE // len(strata)
+    pick = [rng.choice(st, min(per, len(st)), replace=False) for st in strata]
+    # the cores of the ten largest haloes: the deepest octree levels
+    big = np.argsort(-aux["per"])[:10]
+    core = pool[np.isin(halo, big) & (x <= edges[2])]
+    if len(core):
+        pick.append(rng.choice(core, min(per // 2, len(core)), replace=False))
+    return np.unique(np.concatenate(pick)).astype(np.int32)
 
 
 def _set(name):
@@ -28,7 +51,7 @@ def _set(name):
 def _sampled_parity(ps, active_all, label):
     rng = np.random.default_rng(I.SEED_BASE + 77)
     pool = np.arange(ps.n, dtype=np.int32) if active_all is None else active_all
-    sample = np.sort(rng.choice(pool, SAMPLE, replace=False)).astype(np.int32)
+    sample = _stratified_sample(ps, pool, rng)
     g = GpuRun(ps.pos, ps.kernel, ps.mass)
     gd = g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=active_all)
     assert gd["unconv"] == 0
@@ -74,7 +97,7 @@ def test_fullsize_config5_active_subset():
     g0.close()
     assert full["unconv"] == 0
     hg = I.perturb_h(full["H"], act, I.SEED_BASE + 5)
-    ps5 = I.ParticleSet("C5", ps.pos, ps.vel, ps.u, hg, ps.mass, ps.kernel, ps.n_ngb, ps.n_tol)
+    ps5 = I.ParticleSet("C5", ps.pos, ps.vel, ps.u, hg, ps.mass, ps.kernel, ps.n_ngb, ps.n_tol, aux=ps.aux)
     g, gd, sample, rep = _sampled_parity(ps5, act, "C5 full e2e")
     H = hg.copy(); H[act] = gd["H"][act]
     rho = full["rho"].copy(); rho[act] = gd["rho"][act]
