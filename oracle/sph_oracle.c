@@ -19,10 +19,19 @@
  * central values 8/pi, 1365/(64 pi); finite-difference derivative identities; equal-mass
  * identity N_w = (4 pi/3) H^3 rho/m; perfect-lattice values; two-particle hand computation;
  * brute force == cell list; momentum and energy conservation; viscous heating >= 0; static gas
- * v_sig = 2 sqrt(gamma (gamma-1) u); permutation / translation / axis-swap / scaling symmetries.
- * PARITY UNPINNED: the trajectory of the h iteration (which H inside the tolerance band is
- * returned) is fixed only by the rule R7 written here, not by the paper; its fixed point is
- * pinned (perfect lattice root, final neighbour number inside the band).
+ * v_sig = 2 sqrt(gamma (gamma-1) u); permutation / translation / axis-swap / scaling symmetries;
+ * the sums S, D', rho, d rho/dH and Omega of an evaluation against centred finite differences of
+ * S(H) and rho(H); the R7 step: exact landing on the root of a power-law medium whose logarithmic
+ * slope is not 3 (pins the slope factor g and the logarithmic Newton step), the clamp 2^(-1/3) as a
+ * closed form, and a constructed integer-count case with the closed-form trajectory
+ * clamp, clamp, clamp, bracket, 19 volume bisections hi_k^3 = 1 + 2^-k, BRACKET flag
+ * (pins the bracket, the strict r < H, the bisection and the collapse rule); the edge-class flags are
+ * bounded (<= 2 % of a config-1 set).
+ * PARITY UNPINNED BY THE PAPER: which H inside the tolerance band is returned follows from the rule
+ * R7 written here (the paper says only "multiple iterations"); R7 is FROZEN since round 2:
+ * tests/golden/h_trajectory.txt (written by tests/golden/make_h_trajectory.py from this file alone)
+ * holds the trajectories of a seeded set, and any change to the rule must come with a new pin and a
+ * DESIGN.md reading.
  *
  * Summation order: ascending j inside a cell, cells in ascending index order; brute force in
  * ascending j.  No blocking, fusion or reordering beyond the definitions.
@@ -219,11 +228,9 @@ static inline void dens_pair(const dens_ctx *c, const double *xi, double H, int6
     double r = sqrt(r2);
     if (fabs(r / H - 1.0) < 1e-6) e->edge = 1;
     if (!(r2 < H * H)) return; /* strict (R4) */
-    double q = r / H;
     double mj = c->mass ? (double)c->mass[j] : c->mass_scalar;
-    double sg = k_sigma(c->p->kernel);
-    double W = sg / (H * H * H) * k_w(c->p->kernel, q);
-    double dWdH = -sg / (H * H * H * H) * (3.0 * k_w(c->p->kernel, q) + q * k_dw(c->p->kernel, q));
+    double W = orc_W(c->p->kernel, r, H);       /* the pinned kernel functions themselves (R1) */
+    double dWdH = orc_dWdH(c->p->kernel, r, H);
     e->S += W;
     e->Dp += dWdH;
     e->rho += mj * W;

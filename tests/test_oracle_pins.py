@@ -366,3 +366,134 @@ def test_smooth_field_pressure_gradient():
     err = np.abs(f["acc"][:, 0] - expect).max() / np.abs(expect).max()
     assert err < 0.05
     assert np.abs(f["acc"][:, 1:]).max() < 1e-6 * np.abs(expect).max()
+
+
+# ------------------------------------------------------------------ sums of one evaluation against finite differences
+@pytest.mark.parametrize("k", [0, 1])
+def test_density_eval_derivatives_against_finite_differences(k):
+    """D' = dS/dH, drho/dH and Omega = 1 + (H / 3 rho) drho/dH of orc_density_eval against centred finite differences of
+    its own S(H) and rho(H) (the h-derivative sums feed the Newton slope and, through Omega, every force)."""
+    ps = I.config1(10)
+    rng = np.random.default_rng(5)
+    mass = rng.uniform(0.5, 1.5, ps.n).astype(np.float32)
+    H0 = (ps.h_guess * (1.25 if k else 1.0)).astype(np.float32)
+    d = 2.0 ** -12
+    Hp, Hm = (H0 * np.float32(1 + d)).astype(np.float32), (H0 * np.float32(1 - d)).astype(np.float32)
+    e0, ep, em = (O.density_eval(ps.pos, h, kernel=k, mass=mass, brute=True) for h in (H0, Hp, Hm))
+    dH = Hp.astype(np.float64) - Hm.astype(np.float64)
+    fdS = (ep["S"] - em["S"]) / dH
+    fdR = (ep["rho"] - em["rho"]) / dH
+    # D' is a sum of terms of both signs, -(3 w + q w') sigma / H^4, that nearly cancels (it vanishes in a uniform
+    # medium): its error is measured against the size of its terms, 3 S / H, as is Omega - 1 = H D' / (3 S)
+    Hd = H0.astype(np.float64)
+    assert np.max(np.abs(fdS - e0["Dp"]) / (3.0 * e0["S"] / Hd)) < 1e-5
+    assert np.max(np.abs(fdR - e0["drho"]) / (3.0 * e0["rho"] / Hd)) < 1e-5
+    om_fd = 1.0 + H0.astype(np.float64) / (3.0 * e0["rho"]) * fdR
+    assert np.max(np.abs(om_fd - e0["omega"]) / np.abs(e0["omega"])) < 1e-5
+    # orc_density returns the same Omega from its last evaluation
+    o = O.density(ps.pos, H0, kernel=k, n_target=64.0, n_tol=float("inf"), mass=mass, brute=True)
+    assert np.max(np.abs(o["omega"] - e0["omega"])) < 1e-14 and np.max(np.abs(o["rho"] - e0["rho"]) / e0["rho"]) < 1e-15
+
+
+# ------------------------------------------------------------------ the R7 step
+def _powerlaw_medium(alpha=1.5, K=40000, R=0.4, seed=3):
+    """One particle at the centre of the unit box and K particles on stratified radii with N(<r) = K (r/R)^(3-alpha):
+    the kernel-weighted neighbour number of the centre depends on the radii only and is, up to the constant self term,
+    a power law of H with logarithmic slope 3 - alpha."""
+    rng = np.random.default_rng(seed)
+    r = R * ((np.arange(K) + 0.5) / K) ** (1.0 / (3.0 - alpha))
+    v = rng.normal(size=(K, 3))
+    v /= np.linalg.norm(v, axis=1)[:, None]
+    return np.concatenate([[[0.5, 0.5, 0.5]], 0.5 + r[:, None] * v]).astype(np.float32)
+
+
+def test_newton_step_lands_on_the_root_of_a_power_law_medium():
+    """R7: the step is Newton's on ln N(ln H) with slope 3/g.  Where N_w(H) is a power law whose exponent is NOT 3
+    (here 1.5) it lands on the root at once; a step that ignored the slope factor g (exponent 1/3 instead of g/3)
+    would stop half way, 10 % off.  Root by bisection on the (separately pinned) single evaluation."""
+    pos = _powerlaw_medium()
+    act = np.array([0], np.int32)
+    nt = 295.0
+
+    def nw(H):
+        h = np.full(len(pos), H, np.float32)
+        return O.density_eval(pos, h, kernel=1, mass_scalar=1.0, active=act)["Nw"][0]
+
+    lo, hi = 0.005, 0.1
+    for _ in range(60):
+        mid = 0.5 * (lo + hi)
+        lo, hi = (mid, hi) if nw(mid) < nt else (lo, mid)
+    root = 0.5 * (lo + hi)
+    for f in (math.exp(0.2), math.exp(-0.2)):
+        h = np.full(len(pos), root * f, np.float32)
+        o = O.density(pos, h, kernel=1, n_target=nt, n_tol=1e-9, mass_scalar=1.0, active=act, max_iter=2)
+        assert o["iters"][0] == 2
+        assert abs(o["H"][0] / root - 1.0) < 0.01, (f, o["H"][0] / root)     # the slope-blind step would be off by 10 %
+        o3 = O.density(pos, h, kernel=1, n_target=nt, n_tol=1e-9, mass_scalar=1.0, active=act, max_iter=3)
+        assert abs(o3["H"][0] / root - 1.0) < 1e-4                             # quadratic convergence
+
+
+def test_step_clamp_is_a_factor_two_in_volume():
+    """R7: a step changes the support volume by at most a factor 2 -- H <- H 2^(+-1/3) exactly."""
+    n = 12
+    pos = I.perfect_lattice(n)
+    act = np.array([0], np.int32)
+    H_root = 2.48232 / n
+    for f, s in ((2.0, 2.0 ** (-1.0 / 3.0)), (0.5, 2.0 ** (1.0 / 3.0))):
+        h = np.full(len(pos), H_root * f, np.float32)
+        o = O.density(pos, h, kernel=0, n_target=64.0, n_tol=1e-3, mass_scalar=1.0, active=act, max_iter=2, brute=True)
+        assert o["iters"][0] == 2 and o["flags"][0] == O.F_NOTCONV
+        assert abs(o["H"][0] - float(h[0]) * s) <= 1e-15 * float(h[0])
+
+
+def test_bracket_bisection_and_collapse_closed_form():
+    """R7 safeguards on a constructed integer-count case (count_mode 1, N_t = 20, tol = 0): the centre particle has
+    itself and 3 particles inside r < 0.26, then 48 particles at exactly r = 1: N_int jumps from 4 to 52, the target
+    is unreachable.  From H = 1/2 the rule must go: three clamped steps up (N = 4: 2^(-2/3), 2^(-1/3), 1 -- r < H is
+    strict, so H = 1 still counts 4), a fourth to 2^(1/3) (N = 52: bracket (1, 2^(1/3))), then every Newton step falls
+    outside the bracket and the volume bisection takes over, hi_k^3 = 1 + 2^-k, until hi - lo <= 1e-6 lo at k = 19:
+    24 evaluations, flag BRACKET, H = (1 + 2^-19)^(1/3), N_int = 52."""
+    L = 4.0
+    c = np.array([2.0, 2.0, 2.0])
+    inner = [c + [0.125, 0, 0], c + [0, 0.1875, 0], c + [0, 0, -0.25]]
+    axes = [(1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+    shell = [c + np.array(a, float) for a in axes for _ in range(8)]
+    pos = np.array([c] + inner + shell, np.float32)
+    h = np.full(len(pos), 0.5, np.float32)
+    act = np.array([0], np.int32)
+    expect = [0.5, 2.0 ** (-2 / 3), 2.0 ** (-1 / 3), 1.0, 2.0 ** (1 / 3)] + [(1.0 + 2.0 ** -k) ** (1 / 3) for k in range(1, 20)]
+    assert len(expect) == 24
+    for it, H in enumerate(expect, start=1):
+        o = O.density(pos, h, kernel=1, n_target=20.0, n_tol=0.0, box=L, mass_scalar=1.0, active=act, count_mode=1,
+                      max_iter=it, brute=True)
+        assert o["iters"][0] == it and abs(o["H"][0] - H) <= 4e-16 * H, (it, o["H"][0], H)
+        assert o["Nint"][0] == (4 if it <= 4 else 52)
+        assert o["flags"][0] == O.F_NOTCONV  # (the evaluation cap is tested before the bracket)
+    o = O.density(pos, h, kernel=1, n_target=20.0, n_tol=0.0, box=L, mass_scalar=1.0, active=act, count_mode=1, brute=True)
+    assert o["iters"][0] == 24 and o["flags"][0] == O.F_BRACKET and o["Nint"][0] == 52
+    assert o["edge"][0] & O.E_RADIUS  # the evaluation at H = 1 had neighbours exactly on the support radius
+
+
+def test_edge_classes_are_rare():
+    """The edge classes excuse particles from the strict GPU comparison (tests/parity_util.py): on a config-1 set
+    they must stay below 2 %, or the end-to-end parity tests would be hollow."""
+    ps = I.config1()
+    o = O.density(ps.pos, ps.h_guess, kernel=ps.kernel, n_target=ps.n_ngb, n_tol=ps.n_tol, mass_scalar=ps.mass)
+    assert (o["edge"] != 0).mean() <= 0.02
+    assert ((o["edge"] & O.E_BRANCH) != 0).mean() <= 0.002
+
+
+def test_h_trajectories_are_frozen():
+    """R7 is frozen: the trajectories of a seeded set, written by tests/golden/make_h_trajectory.py from the
+    oracle alone, must be reproduced exactly -- H after 1, 2, 3 evaluations and at the end, evaluations used, flags."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_h_trajectory", os.path.join(GOLD, "make_h_trajectory.py"))
+    m = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(m)
+    rows = [l.split() for l in open(os.path.join(GOLD, "h_trajectory.txt")) if l.strip() and not l.startswith("#")]
+    now = m.trajectories()
+    assert len(rows) == len(now)
+    for r, t in zip(rows, now):
+        assert [int(r[0]), int(r[1]), int(r[2])] == list(t[:3])
+        for a, b in zip(r[3:], t[3:]):
+            assert float.fromhex(a) == b
