@@ -39,8 +39,33 @@ UNIT = "updates/s"
 # algorithmic flops per true pair (frozen from the oracle's inner loops)
 FLOP_DENSITY_PAIR = {0: 30.0, 1: 40.0}  # cubic spline / Wendland C6
 FLOP_FORCE_PAIR = 80.0
-# derived FP32 peak: 148 SMs x 128 FP32 lanes x 2 flop/FMA x max SM clock
+# derived FP32 peak: 148 SMs x 128 FP32 lanes x 2 flop/FMA x max SM clock; reported beside
+# the measured one (bench_probe.cu), which is the roofline's denominator
 FP32_LANES_PER_SM = 128
+PROBE_SRC = os.path.join(ROOT, "bench_probe.cu")
+PROBE_LIB = os.path.join(ROOT, "bench_probe.so")
+
+
+def build_probe(force: bool = False) -> str:
+    """nvcc -> bench_probe.so (the FP32 FMA issue-rate probe; bench harness only, not part of libsph.so)."""
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SRC):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "--shared",
+                               "-Xcompiler", "-fPIC", "-o", PROBE_LIB, PROBE_SRC])
+    return PROBE_LIB
+
+
+def fp32_peak(stream_ptr: int, packed: bool, iters: int = 32) -> float:
+    """Measured FP32 FMA rate of this device in TFLOP/s (register-only FMA chains on every SM)."""
+    import ctypes as C
+
+    lib = C.CDLL(build_probe())
+    lib.bench_fp32_peak.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]
+    out = C.c_double(0.0)
+    rc = lib.bench_fp32_peak(C.c_void_p(stream_ptr), iters, int(packed), C.byref(out))
+    if rc:
+        raise RuntimeError(f"bench_fp32_peak: cudaError {rc}")
+    return float(out.value)
 
 
 def make_workload(name: str, n: int | None):
@@ -72,7 +97,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -268,8 +293,8 @@ def main():
         sph.sph_hydro_force(vel, u, h, rho, om, acc, du, vs, active=active)
         return unconv
 
-    peak_scalar = sph.sph_fp32_peak(32, False)
-    peak_packed = sph.sph_fp32_peak(32, True)
+    peak_scalar = fp32_peak(stream.cuda_stream, False)
+    peak_packed = fp32_peak(stream.cuda_stream, True)
     for _ in range(max(args.warmup, 0)):
         step()
         if flush is not None:
@@ -341,7 +366,7 @@ def main():
         sph2.close()
 
     if rank == 0:
-        # roofline of the dominant kernel (the persistent density gather + h-iteration kernel)
+        # roofline of the dominant kernel = the gather kernel with the larger event time in this run
         tk = float(np.mean([p["t_density_kernel_ms"] for p in per]))
         tf = float(np.mean([p["t_force_kernel_ms"] for p in per]))
         ti = float(np.mean([p["t_index_ms"] for p in per]))
@@ -351,24 +376,41 @@ def main():
         fl_f = FLOP_FORCE_PAIR * st["force_pairs"]
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
         sm_max = clocks.get("sm_max_mhz") or 1965.0
-        peak = sm_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
-        # DRAM bytes per launch of the dominant kernel, from the committed ncu capture (profiles/traffic.csv)
-        traffic = None
+        derived = sm_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
+        peak = peak_packed  # measured on this device in this run; the derived figure beside it
+        hbm_peak, hbm_src = 6650.0, "fallback of B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+        try:
+            hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+            hbm_src = "measured copy bandwidth, MEASURED_PEAKS.json"
+        except (OSError, KeyError, ValueError):
+            pass
+        # DRAM bytes per launch from the committed ncu capture (profiles/traffic.csv), labelled with its commit
+        traffic = {}
         tpath = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tpath):
             import csv
             for row in csv.DictReader(open(tpath)):
-                if row["workload"] == w and row["kernel"] == "k_density":
-                    traffic = int(row["dram_bytes_per_launch"])
-        roof = {"bound": "alu", "kernel": "k_density (a6-a9)", "achieved": fl_d / (tk * 1e-3) * 1e-12, "peak": peak,
-                "unit": "TFLOP/s", "frac": fl_d / (tk * 1e-3) * 1e-12 / peak, "traffic": traffic,
-                "peak_source": f"derived: {sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md); "
-                               f"measured FMA probe on this device: {peak_scalar:.1f} TFLOP/s scalar, {peak_packed:.1f} packed f32x2",
-                "algorithmic_flops_per_launch": fl_d, "kernel_ms": tk,
-                "force_kernel": {"achieved": fl_f / (tf * 1e-3) * 1e-12, "frac": fl_f / (tf * 1e-3) * 1e-12 / peak,
-                                 "kernel_ms": tf, "algorithmic_flops_per_launch": fl_f},
+                if row["workload"] == w:
+                    traffic[row["kernel"]] = (int(row["dram_bytes_per_launch"]), row.get("commit", "?"))
+
+        def kroof(name, steps_, flops, t_ms):
+            tr = traffic.get(name)
+            return {"kernel": f"{name} ({steps_})", "achieved": flops / (t_ms * 1e-3) * 1e-12, "frac": flops / (t_ms * 1e-3) * 1e-12 / peak,
+                    "frac_of_derived": flops / (t_ms * 1e-3) * 1e-12 / derived, "kernel_ms": t_ms,
+                    "algorithmic_flops_per_launch": flops, "traffic": None if tr is None else tr[0],
+                    "traffic_source": None if tr is None else f"ncu dram__bytes_read+write per launch, captured at commit {tr[1]} "
+                                                              "(profiles/traffic.csv); not re-measured by this run"}
+
+        rd, rf = kroof("k_density", "a6-a9", fl_d, tk), kroof("k_force", "a10-a11", fl_f, tf)
+        dom, other = (rf, rd) if tf >= tk else (rd, rf)
+        roof = {"bound": "alu", **dom, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": f"measured: packed fma.rn.f32x2 probe on this device in this run (bench_probe.cu); scalar FFMA "
+                               f"probe {peak_scalar:.1f}; derived {sm_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 x "
+                               f"{sm_max:.0f} MHz = {derived:.1f}",
+                "peak_derived": derived, "other_gather_kernel": other,
                 "index_build": {"bound": "hbm", "ms": ti, "achieved_GBps": 200.0 * n / (ti * 1e-3) * 1e-9,
-                                "algorithmic_bytes": 200.0 * n}}
+                                "algorithmic_bytes": 200.0 * n, "peak_GBps": hbm_peak, "peak_source": hbm_src,
+                                "frac": 200.0 * n / (ti * 1e-3) * 1e-9 / hbm_peak}}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

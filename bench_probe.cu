@@ -1,6 +1,7 @@
-// sph_probe.cu -- FP32 FMA issue-rate probe: the measured counterpart of the derived ALU roofline
-// denominator.  Measurement support only; no step of the path runs here.
-#include "sph_internal.cuh"
+// bench_probe.cu -- FP32 FMA issue-rate probe of bench.py: the measured denominator of the ALU roofline
+// ("measured on the box in the same session").  Bench harness only: it is
+// built into bench_probe.so beside bench.py, not into libsph.so, and no step of the path runs here.
+#include <cuda_runtime.h>
 
 namespace {
 
@@ -55,29 +56,38 @@ __global__ void __launch_bounds__(256) k_probe_packed(int iters, float a, float 
 
 } // namespace
 
-extern "C" int sph_fp32_peak(sph_ctx *ctx, int iters, int packed, double *tflops_host)
+// Runs a register-only chain of fused multiply-adds on every SM (about iters x 4096 FMAs per thread) on the given
+// stream and returns the achieved rate in TFLOP/s (2 flop per FMA) in *tflops_host; packed != 0 uses the two-wide
+// fma.rn.f32x2 form of sm_100.  Returns 0, or a cudaError_t value.  Synchronises the stream.
+extern "C" int bench_fp32_peak(void *cuda_stream, int iters, int packed, double *tflops_host)
 {
-    if (!ctx || !tflops_host || iters < 1) return SPH_E_ARG;
-    cudaStream_t st = ctx->stream;
-    float *dummy = reinterpret_cast<float *>(ctx->cnt); // never written (see the kernels)
-    const int blocks = ctx->device_sms * 8, threads = 256;
+    if (!tflops_host || iters < 1) return (int)cudaErrorInvalidValue;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return (int)e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return (int)e;
+    float *dummy = nullptr; // never written (see the kernels)
+    if ((e = cudaMalloc((void **)&dummy, 256)) != cudaSuccess) return (int)e;
+    const int blocks = sms * 8, threads = 256;
     cudaEvent_t e0, e1;
-    SPH_CUDA(ctx, cudaEventCreate(&e0));
-    SPH_CUDA(ctx, cudaEventCreate(&e1));
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
     for (int rep = 0; rep < 2; rep++) { // first launch warms up
-        SPH_CUDA(ctx, cudaEventRecord(e0, st));
+        cudaEventRecord(e0, st);
         if (packed) k_probe_packed<<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, dummy);
         else k_probe_scalar<<<blocks, threads, 0, st>>>(iters, 0.999f, 0.001f, dummy);
-        SPH_CUDA(ctx, cudaEventRecord(e1, st));
-        SPH_CUDA(ctx, cudaStreamSynchronize(st));
+        cudaEventRecord(e1, st);
+        cudaStreamSynchronize(st);
     }
-    SPH_CUDA(ctx, cudaGetLastError());
     float ms = 0.f;
-    SPH_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    double fmas = (double)blocks * threads * (double)iters * PROBE_INNER * PROBE_ACC;
+    cudaFree(dummy);
+    if (e != cudaSuccess) return (int)e;
+    const double fmas = (double)blocks * threads * (double)iters * PROBE_INNER * PROBE_ACC;
     *tflops_host = 2.0 * fmas / ((double)ms * 1e-3) * 1e-12;
-    ctx->launches += 2;
-    return SPH_OK;
+    return 0;
 }

@@ -15,9 +15,17 @@
  *    in _host.  The library never frees or reallocates caller arrays; it writes only the entries of
  *    ACTIVE particles, indexed by the caller's particle id.  Sorted copies, the octree and scratch
  *    are private to the context.
- *  - Work is enqueued on the CUDA stream given to sph_create.  sph_build_index synchronises once
- *    (it reads back the octree size); sph_density synchronises once (to return n_unconverged);
- *    sph_hydro_force is fully asynchronous.  The *_host entry points synchronise before returning.
+ *  - Work is enqueued on the CUDA stream given to sph_create.  sph_build_index and sph_hydro_force are
+ *    fully asynchronous; sph_density synchronises once (to return n_unconverged); sph_get_stats and the
+ *    *_host entry points synchronise before returning.
+ *  - Preconditions are checked on the device: 0 <= x < box for every coordinate (sph_build_index);
+ *    active ids in [0, n) and listed once; 0 < H < box/2 and finite for the guesses of the active
+ *    particles (sph_density) and for h of ALL particles (sph_hydro_force), whose rho must be > 0 and
+ *    whose rho, omega, u, vel must be finite.  A call whose inputs violate one computes and writes
+ *    NOTHING; the failure is sticky and is returned -- SPH_E_ARG, or SPH_E_HRANGE if the only
+ *    violation is H >= box/2 -- by that call if it synchronises, else by the next synchronising call
+ *    (sph_density, sph_get_stats, sph_step_host), which then computes nothing itself and clears it.
+ *    Bad positions invalidate the index: every call reports them until sph_build_index is called again.
  *  - Geometry: periodic cube [0, box)^3, minimum-image distances, support radius H < box/2.
  *    H is the radius at which the kernel reaches zero (W = 0 for r >= H).
  *  - Errors are return codes (sph_status); no exceptions, no abort, no printing.  A sticky CUDA error
@@ -43,6 +51,7 @@ typedef enum {
     SPH_E_NOINDEX = 3,  /* sph_density / sph_hydro_force before sph_build_index */
     SPH_E_OOM = 4,      /* device allocation failed */
     SPH_E_INTERNAL = 5, /* an internal capacity was exceeded (reported, never silent) */
+    SPH_E_HRANGE = 6,   /* a support radius >= box / 2 (minimum image undefined) */
     SPH_W_NOCONV = 16   /* warning: some active particles stopped without |N - N_t| <= tol */
 } sph_status;
 
@@ -85,6 +94,8 @@ typedef struct {
     float t_density_kernel_ms; /* the persistent gather + h-iteration kernel alone (a6-a9) */
     float t_force_prep_ms;     /* sorted force state + per-node max H (a9/a4 refresh) */
     float t_force_kernel_ms;   /* the hydro-force gather kernel alone (a10-a11) */
+    int64_t node_pool_overflow; /* != 0: the octree node pool ran out during sph_build_index (extremely clumped input);
+                                   some leaves then hold more than 32 particles -- results stay correct, the gather slows down */
 } sph_stats;
 
 /* Create a context. `cuda_stream` is a cudaStream_t (NULL = legacy default stream). */
@@ -98,10 +109,11 @@ int sph_destroy(sph_ctx *ctx);
  * octree nodes holding <= group_node particles, each cut into balanced runs of <= group_cap consecutive
  * sorted particles (one warp per group).  Replaces the paper's Hilbert keys + domain decomposition +
  * tree build (PAPER.md:25, :41 §1, :194-196 §4).
- *   pos   [n*3] device, x,y,z per particle, 0 <= x < box (values outside are clamped into the
- *         boundary cells for the search and otherwise used as given);
+ *   pos   [n*3] device, x,y,z per particle, 0 <= x < box (checked on the device, see Conventions);
  *   mass  [n] device or NULL; if NULL every particle has mass_scalar.
- * n = 0 is valid (later calls do nothing).  Synchronises the stream once.
+ * n = 0 is valid (later calls do nothing).  Asynchronous.  If the octree node pool runs out (more than
+ * about two nodes per particle: extremely clumped input) the remaining cells stay oversize leaves: results
+ * are unaffected, the gather slows down, and sph_stats.node_pool_overflow reports it.
  */
 int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar);
 
@@ -115,14 +127,15 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
  *   omega[id]     1 + (H_i / 3 rho_i) d rho_i / d H_i,
  *   ngb_count[id] integer count #{j : r_ij < H_i} at the returned H (self included),
  *   status[id]    evaluations used | SPH_ST_* flags (status may be NULL).
- *   active        [n_active] device int32 particle ids (unique, in range); NULL with n_active != 0
+ *   active        [n_active] device int32 particle ids (in range, each listed once); NULL with n_active != 0
  *                 (conventionally -1) means all particles; n_active == 0 is the empty list (nothing
  *                 is computed or written, whatever the pointer);
  *   n_ngb_tol     +inf means "evaluate once at the given h";
  *   n_unconverged_host  HOST pointer (may be NULL): number of active particles that stopped
  *                 without SPH_ST_CONVERGED.
  * Returns SPH_OK, or SPH_W_NOCONV if *n_unconverged_host would be > 0.  Synchronises once.
- * An active id outside [0, n) makes the call compute and write nothing and return SPH_E_ARG.
+ * A failed precondition (ids, guesses; see Conventions) makes the call compute and write nothing and
+ * return SPH_E_ARG / SPH_E_HRANGE.
  */
 int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol,
                 float *h, float *rho, float *omega, int32_t *ngb_count, int32_t *status,
@@ -137,8 +150,9 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
  * with A = (gamma-1) u / (omega rho), F_ij(H) = dW/dr(r_ij, H), Pi_ij the signal-velocity viscosity.
  *   vel [n*3], u [n], h [n], rho [n], omega [n]: device, valid for ALL n particles (inactive
  *   neighbours contribute with their current values, R12); acc [n*3], dudt [n], vsig_max [n]: device,
- *   written for active particles only.  Asynchronous: an active id outside [0, n) makes the call compute
- *   and write nothing, and the next synchronising call (sph_density, sph_get_stats) returns SPH_E_ARG.
+ *   written for active particles only.  Asynchronous: a failed precondition (ids, h, rho, ...; see
+ *   Conventions) makes the call compute and write nothing, and the next synchronising call
+ *   (sph_density, sph_get_stats) returns SPH_E_ARG / SPH_E_HRANGE instead of doing its own work.
  */
 int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
                     const float *h, const float *rho, const float *omega, float *acc, float *dudt,
@@ -158,20 +172,12 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
                   int32_t *ngb_count_host, float *acc_host, float *dudt_host, float *vsig_host,
                   int64_t *n_unconverged_host);
 
-/* Counters of the last calls (host struct filled; synchronises the stream). */
+/* Counters of the last calls (host struct filled; synchronises the stream).  Reports a pending
+ * precondition failure of an earlier asynchronous call (see Conventions). */
 int sph_get_stats(sph_ctx *ctx, sph_stats *out_host);
 
 /* Text of the most recent error of this context ("" if none). Never NULL; valid until the next call. */
 const char *sph_last_error(const sph_ctx *ctx);
-
-/*
- * FP32 FMA issue-rate probe (measurement support, not part of the path): runs a register-only
- * chain of fused multiply-adds on every SM for about `iters` x 4096 FMAs per thread and returns the
- * achieved rate in TFLOP/s (2 flop per FMA) in *tflops_host.  packed != 0 uses the two-wide
- * fma.rn.f32x2 form of sm_100.  Synchronises.  Used by bench.py to report the ALU roofline
- * denominator measured on the same device next to the derived one.
- */
-int sph_fp32_peak(sph_ctx *ctx, int iters, int packed, double *tflops_host);
 
 /* Library version string and the compute capability it was built for ("sm_100a"). */
 const char *sph_version(void);

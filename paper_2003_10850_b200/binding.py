@@ -14,12 +14,12 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsph.so")
 
-SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL, SPH_W_NOCONV = 0, 1, 2, 3, 4, 5, 16
+SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL, SPH_E_HRANGE, SPH_W_NOCONV = 0, 1, 2, 3, 4, 5, 6, 16
 ST_CONVERGED, ST_BRACKET, ST_NOTCONV, ST_STALLED = 1 << 8, 1 << 9, 1 << 10, 1 << 11
 KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
-           "sph_get_stats", "sph_fp32_peak", "sph_last_error", "sph_version"]
+           "sph_get_stats", "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -30,7 +30,8 @@ class SphParams(C.Structure):
 class SphStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("n", "n_nodes", "n_groups", "launches", "dens_evals", "dens_candidates",
                                          "dens_pairs", "force_candidates", "force_pairs")] + \
-               [(k, C.c_float) for k in ("t_index_ms", "t_density_kernel_ms", "t_force_prep_ms", "t_force_kernel_ms")]
+               [(k, C.c_float) for k in ("t_index_ms", "t_density_kernel_ms", "t_force_prep_ms", "t_force_kernel_ms")] + \
+               [("node_pool_overflow", C.c_int64)]
 
 
 class SphError(RuntimeError):
@@ -59,11 +60,10 @@ def load():
         lib.sph_step_host.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                       C.c_int64, C.c_float, C.c_float] + [C.c_void_p] * 7 + [C.POINTER(C.c_int64)]
         lib.sph_get_stats.argtypes = [C.c_void_p, C.POINTER(SphStats)]
-        lib.sph_fp32_peak.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]
         lib.sph_last_error.argtypes = [C.c_void_p]
         lib.sph_last_error.restype = C.c_char_p
         lib.sph_version.restype = C.c_char_p
-        for name in EXPORTS[:8]:
+        for name in EXPORTS[:7]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -173,12 +173,6 @@ class Sph:
         s = SphStats()
         self._check(self._lib.sph_get_stats(self._h, C.byref(s)))
         return {k: (int if t is C.c_int64 else float)(getattr(s, k)) for k, t in SphStats._fields_}
-
-    def sph_fp32_peak(self, iters=64, packed=False) -> float:
-        """Measured FP32 FMA rate of the device in TFLOP/s (measurement support)."""
-        out = C.c_double(0.0)
-        self._check(self._lib.sph_fp32_peak(self._h, int(iters), int(bool(packed)), C.byref(out)))
-        return float(out.value)
 
 
 def version() -> str:

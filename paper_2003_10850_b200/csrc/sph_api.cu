@@ -4,6 +4,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "sph_internal.cuh"
 
 int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...)
@@ -24,6 +26,29 @@ void dfree(T *&p)
 {
     if (p) cudaFree(p);
     p = nullptr;
+}
+
+// NVTX range around an entry point (the paper reads its timelines from nvToolsExt ranges, Fig. 2)
+struct Range {
+    explicit Range(const char *name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+};
+
+// Report and clear the device-side precondition failures (SphCounters::err: sticky since the call that found them,
+// which may be an earlier asynchronous one; idx_err: the state of the current index, kept until the next build).
+int report(sph_ctx *ctx, const char *where, unsigned int err, unsigned int idx_err)
+{
+    if (!err && !idx_err) return SPH_OK;
+    if (err) cudaMemsetAsync(&ctx->cnt->err, 0, sizeof(unsigned int), ctx->stream);
+    const bool range_only = !idx_err && err == SPH_ERR_HRANGE;
+    return sph_fail(ctx, range_only ? SPH_E_HRANGE : SPH_E_ARG,
+                    "%s: precondition failed on the device, in this call or in an asynchronous one before it:%s%s%s%s%s%s "
+                    "-- the calls concerned computed and wrote nothing",
+                    where, (err & SPH_ERR_IDS) ? " active id outside [0, n);" : "", (err & SPH_ERR_DUP) ? " active id listed twice;" : "",
+                    (err & SPH_ERR_H) ? " support radius <= 0 or not finite;" : "",
+                    (err & SPH_ERR_HRANGE) ? " support radius >= box / 2;" : "",
+                    (err & SPH_ERR_STATE) ? " rho <= 0, u < 0 or a non-finite rho, omega, u, vel;" : "",
+                    (idx_err & SPH_ERR_POS) ? " position outside [0, box) in sph_build_index (rebuild the index);" : "");
 }
 
 int check_sticky(sph_ctx *ctx)
@@ -101,6 +126,7 @@ int sph_destroy(sph_ctx *ctx)
 int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar)
 {
     if (!ctx) return SPH_E_ARG;
+    Range nv("sph_build_index");
     if (n < 0 || n > 0x7fffff00ll || (n > 0 && !pos)) return sph_fail(ctx, SPH_E_ARG, "sph_build_index: bad n or pos");
     if (!mass && !(mass_scalar > 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_build_index: mass_scalar must be > 0");
     int rc = check_sticky(ctx);
@@ -121,6 +147,7 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
                 float *rho, float *omega, int32_t *ngb_count, int32_t *status, int64_t *n_unconverged_host)
 {
     if (!ctx) return SPH_E_ARG;
+    Range nv("sph_density");
     if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_density before sph_build_index");
     if (n_unconverged_host) *n_unconverged_host = 0;
     if (!(n_ngb_target > 0.f) || !(n_ngb_tol >= 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_density: bad target/tolerance");
@@ -132,13 +159,13 @@ int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_n
     int rc = check_sticky(ctx);
     if (rc) return rc;
     if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
-    if ((rc = sph_density_launch(ctx, active != nullptr, items, n_ngb_target, n_ngb_tol, h, rho, omega, ngb_count, status)))
+    if ((rc = sph_density_launch(ctx, active, items, n_ngb_target, n_ngb_tol, h, rho, omega, ngb_count, status)))
         return rc;
-    unsigned int res[2] = {0, 0}; // n_unconv, bad_ids (adjacent counters)
+    unsigned int res[3] = {0, 0, 0}; // n_unconv, err, idx_err (adjacent counters)
     SPH_CUDA(ctx, cudaMemcpyAsync(res, &ctx->cnt->n_unconv, sizeof(res), cudaMemcpyDeviceToHost, ctx->stream));
     SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     SPH_CUDA(ctx, cudaGetLastError());
-    if (res[1]) return sph_fail(ctx, SPH_E_ARG, "sph_density: %u active ids outside [0, n): nothing was computed", res[1]);
+    if ((rc = report(ctx, "sph_density", res[1], res[2]))) return rc;
     if (n_unconverged_host) *n_unconverged_host = res[0];
     return res[0] ? SPH_W_NOCONV : SPH_OK;
 }
@@ -147,6 +174,7 @@ int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const
                     const float *h, const float *rho, const float *omega, float *acc, float *dudt, float *vsig_max)
 {
     if (!ctx) return SPH_E_ARG;
+    Range nv("sph_hydro_force");
     if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_hydro_force before sph_build_index");
     const bool subset = active != nullptr || n_active == 0;
     if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force: n_active < 0");
@@ -170,8 +198,10 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
                             !ngb_count_host || !acc_host || !dudt_host || !vsig_host)))
         return sph_fail(ctx, SPH_E_ARG, "sph_step_host: NULL host array");
     if (n == 0) return SPH_OK;
+    Range nv("sph_step_host");
     cudaStream_t st = ctx->stream;
     if (n > ctx->cap_host) {
+        ctx->cap_host = 0; // (an allocation failure below leaves no stale capacity behind)
         dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
         dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
         size_t c = (size_t)n;
@@ -228,14 +258,17 @@ int sph_get_stats(sph_ctx *ctx, sph_stats *out)
     if (!ctx || !out) return SPH_E_ARG;
     memset(out, 0, sizeof(*out));
     out->n = ctx->n;
-    out->n_nodes = ctx->n_nodes;
-    out->n_groups = ctx->n_groups;
     out->launches = ctx->launches;
     SphCounters h;
     SPH_CUDA(ctx, cudaMemcpyAsync(&h, ctx->cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
     SPH_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    if (h.bad_ids)
-        return sph_fail(ctx, SPH_E_ARG, "%u active ids outside [0, n) in the last call: nothing was computed", h.bad_ids);
+    if (ctx->have_index && ctx->n > 0) {
+        out->n_nodes = h.n_nodes;
+        out->n_groups = h.n_groups;
+        out->node_pool_overflow = h.overflow;
+    }
+    int rc = report(ctx, "sph_get_stats", h.err, ctx->have_index ? h.idx_err : 0u);
+    if (rc) return rc;
     out->dens_evals = (int64_t)h.dens_evals;
     out->dens_candidates = (int64_t)h.dens_cands;
     out->dens_pairs = (int64_t)h.dens_pairs;

@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     DensWarp<HAS_MASS> &W = reinterpret_cast<DensWarp<HAS_MASS> *>(smem_raw)[warp];
-    if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
+    if (a.cnt->err | a.cnt->idx_err) return; // a precondition failed (ids, h, positions): compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_evals = 0, st_cands = 0, st_pairs = 0; // meaningful in lane 0 only
     unsigned int st_unconv = 0;
@@ -470,10 +470,22 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS) k_density(DensArgs a)
     }
 }
 
+// precondition 0 < H < box / 2 on the guesses of the active particles (not finite counts as <= 0)
+__global__ void k_check_h(int64_t n_items, int64_t n, const int32_t *__restrict__ active, const float *__restrict__ h, float half_box,
+                          SphCounters *cnt)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_items) return;
+    int64_t id = active ? (int64_t)active[k] : k;
+    if (id < 0 || id >= n) return; // (reported by the active-list pass)
+    const float H = h[id];
+    if (!(H > 0.f) || !(H < __int_as_float(0x7f800000))) atomicOr(&cnt->err, SPH_ERR_H);
+    else if (!(H < half_box)) atomicOr(&cnt->err, SPH_ERR_HRANGE);
+}
+
 __global__ void k_reset_counters(SphCounters *c, int which, bool subset)
 {
     c->work = 0;
-    if (!subset) c->bad_ids = 0; // no active list in this call
     if (which == 0) { c->n_unconv = 0; c->dens_evals = 0; c->dens_cands = 0; c->dens_pairs = 0; }
     else { c->force_cands = 0; c->force_pairs = 0; }
 }
@@ -504,9 +516,10 @@ void sph_reset_counters(sph_ctx *ctx, int which, bool subset)
     ctx->launches++;
 }
 
-int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_target, float n_tol, float *h, float *rho,
+int sph_density_launch(sph_ctx *ctx, const int32_t *active, int64_t n_items, float n_target, float n_tol, float *h, float *rho,
                        float *omega, int32_t *ngb, int32_t *status)
 {
+    const bool subset = active != nullptr;
     DensArgs a;
     a.nodes = ctx->nodes;
     a.xyzm = ctx->xyzm;
@@ -525,7 +538,9 @@ int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_targe
     a.mass_scalar = ctx->mass_scalar;
     a.h = h; a.rho = rho; a.omega = omega; a.ngb = ngb; a.status = status;
     sph_reset_counters(ctx, 0, subset);
-    int64_t est_groups = subset ? n_items : ctx->n_groups;
+    k_check_h<<<(int)((n_items + 255) / 256), 256, 0, ctx->stream>>>(n_items, ctx->n, active, h, 0.5f * ctx->prm.box, ctx->cnt);
+    ctx->launches++;
+    int64_t est_groups = n_items; // (an upper bound: the group count stays on the device)
     int rc;
     cudaEventRecord(ctx->ev[2], ctx->stream);
     if (ctx->prm.kernel == SPH_KERNEL_CUBIC)

@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ForceWarp &W = reinterpret_cast<ForceWarp *>(smem_raw)[warp];
     const float L = a.L;
-    if (a.cnt->bad_ids) return; // an active id was out of range: compute nothing (uniform over the grid)
+    if (a.cnt->err | a.cnt->idx_err) return; // a precondition failed (ids, h, state, positions): compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_cands = 0, st_pairs = 0;
     uint32_t *qp = W.q + lane;
@@ -319,14 +319,24 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
 // gather the caller-order state into the sorted float4 arrays the gather streams through shared memory
 __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const float4 *__restrict__ xyzm,
                              const float *__restrict__ vel, const float *__restrict__ u, const float *__restrict__ h,
-                             const float *__restrict__ rho, const float *__restrict__ omega, float gamma,
-                             float4 *__restrict__ xyzh, float4 *__restrict__ vc)
+                             const float *__restrict__ rho, const float *__restrict__ omega, float gamma, float half_box,
+                             float4 *__restrict__ xyzh, float4 *__restrict__ vc, SphCounters *cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     uint32_t id = perm[i];
     float4 p = xyzm[i];
     float ui = u[id], ri = rho[id];
+    // preconditions on the state of ALL particles (inactive neighbours contribute, R12): 0 < H < box / 2, rho > 0,
+    // u >= 0, everything finite (a comparison with NaN is false)
+    {
+        const float inf = __int_as_float(0x7f800000);
+        const float H = h[id], om = omega[id];
+        const float v2 = fabsf(vel[3 * (int64_t)id]) + fabsf(vel[3 * (int64_t)id + 1]) + fabsf(vel[3 * (int64_t)id + 2]);
+        if (!(H > 0.f) || !(H < inf)) atomicOr(&cnt->err, SPH_ERR_H);
+        else if (!(H < half_box)) atomicOr(&cnt->err, SPH_ERR_HRANGE);
+        if (!(ri > 0.f) || !(ri < inf) || !(ui >= 0.f) || !(ui < inf) || !(fabsf(om) < inf) || !(v2 < inf)) atomicOr(&cnt->err, SPH_ERR_STATE);
+    }
     float c = sqrtf(gamma * (gamma - 1.f) * ui);
     float A = (gamma - 1.f) * ui / (omega[id] * ri); // P/(Omega rho^2), P = (gamma-1) rho u
     xyzh[i] = make_float4(p.x, p.y, p.z, h[id]);
@@ -336,6 +346,12 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
 
 // largest support radius inside every octree node: leaves scan their particles, then push the value
 // up the parent chain with integer atomicMax (H > 0, so the float bit patterns order like integers)
+__global__ void k_zero_hmax(const SphCounters *cnt, float *__restrict__ hmax)
+{
+    uint32_t nn = cnt->n_nodes;
+    for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) hmax[nd] = 0.f;
+}
+
 __global__ void k_node_hmax(const SphCounters *cnt, const SphNode *__restrict__ nodes, const float4 *__restrict__ xyzh,
                             float *__restrict__ hmax)
 {
@@ -382,11 +398,11 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     const int T = 256;
     cudaEventRecord(ctx->ev[4], st);
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
-                                                       ctx->f_xyzh, ctx->f_vc);
-    SPH_CUDA(ctx, cudaMemsetAsync(ctx->node_hmax, 0, sizeof(float) * ctx->n_nodes, st));
+                                                       0.5f * ctx->prm.box, ctx->f_xyzh, ctx->f_vc, ctx->cnt);
+    k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
     k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
     sph_reset_counters(ctx, 1, subset);
-    ctx->launches += 3;
+    ctx->launches += 4;
     cudaEventRecord(ctx->ev[5], st);
     ctx->ev_set[2] = true;
 
@@ -403,7 +419,7 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     a.L = ctx->prm.box;
     a.alpha = ctx->prm.alpha_visc;
     a.acc = acc; a.dudt = dudt; a.vsig = vsig;
-    int64_t est_groups = subset ? n_items : ctx->n_groups;
+    int64_t est_groups = n_items; // (an upper bound: the group count stays on the device)
     cudaEventRecord(ctx->ev[6], st);
     int rc = ctx->prm.kernel == SPH_KERNEL_CUBIC ? launch<SPH_KERNEL_CUBIC>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6>(ctx, a, est_groups);
     cudaEventRecord(ctx->ev[7], st);

@@ -3,6 +3,8 @@
 //
 // Replaces the paper's Hilbert keys + domain decomposition + serial tree build (§1,
 // :72 §2.1, :194-196 §4) and its N_min CPU fallback for small active sets (§2.2).
+#include <stddef.h>
+
 #include <cub/cub.cuh>
 
 #include "sph_internal.cuh"
@@ -28,12 +30,14 @@ __device__ __forceinline__ uint32_t cell16(float x, float scale)
 }
 
 // a1: key generation
-__global__ void k_keys(int64_t n, const float *__restrict__ pos, float scale, uint64_t *__restrict__ keys,
-                       uint32_t *__restrict__ perm)
+__global__ void k_keys(int64_t n, const float *__restrict__ pos, float scale, float box, uint64_t *__restrict__ keys,
+                       uint32_t *__restrict__ perm, SphCounters *cnt)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    // precondition 0 <= x < box (also catches NaN): the index is marked unusable, every later call reports it
+    if (!(x >= 0.f && x < box && y >= 0.f && y < box && z >= 0.f && z < box)) atomicOr(&cnt->idx_err, SPH_ERR_POS);
     uint64_t k = part1by2_16(cell16(x, scale)) | (part1by2_16(cell16(y, scale)) << 1) |
                  (part1by2_16(cell16(z, scale)) << 2);
     keys[i] = k;
@@ -155,15 +159,18 @@ __global__ void k_act_slots(int64_t na, int64_t n, const int32_t *__restrict__ a
     if (k >= na) return;
     const int32_t id = active[k];
     const bool ok = id >= 0 && (int64_t)id < n;
-    if (!ok) atomicAdd(&cnt->bad_ids, 1u); // the gather kernels then return at once; reported as SPH_E_ARG
+    if (!ok) atomicOr(&cnt->err, SPH_ERR_IDS); // the gather kernels then return at once; reported as SPH_E_ARG
     slot[k] = ok ? inv[id] : 0u;
 }
 
 __global__ void k_act_flags(int64_t na, const uint32_t *__restrict__ slot, const uint32_t *__restrict__ gid,
-                            uint32_t *__restrict__ flag)
+                            uint32_t *__restrict__ flag, SphCounters *cnt)
 {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < na) flag[k] = (k == 0 || gid[slot[k]] != gid[slot[k - 1]]) ? 1u : 0u;
+    if (k >= na) return;
+    flag[k] = (k == 0 || gid[slot[k]] != gid[slot[k - 1]]) ? 1u : 0u;
+    // an id listed twice sits next to itself in the sorted slots (and would make a group larger than a warp)
+    if (k > 0 && slot[k] == slot[k - 1] && !(cnt->err & SPH_ERR_IDS)) atomicOr(&cnt->err, SPH_ERR_DUP);
 }
 
 template <typename T>
@@ -199,6 +206,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     int rc;
     if (n > ctx->cap_n) {
         int64_t cap = n + n / 8 + 1024;
+        ctx->cap_n = 0; // (an allocation failure below leaves no stale capacity behind)
         if ((rc = ensure(ctx, &ctx->keys, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->keys_alt, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->perm, cap))) return rc;
@@ -220,13 +228,17 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
         ctx->node_cap = ncap;
         ctx->cap_n = cap;
     }
-    ctx->n_nodes = 0;
-    ctx->n_groups = 0;
-    if (n == 0) { ctx->have_index = true; return SPH_OK; }
+    if (n == 0) {
+        SPH_CUDA(ctx, cudaMemsetAsync(ctx->cnt, 0, offsetof(SphCounters, err), st)); // n_nodes, n_groups, ... (not the pending errors)
+        SPH_CUDA(ctx, cudaMemsetAsync(&ctx->cnt->idx_err, 0, sizeof(unsigned int), st));
+        ctx->have_index = true;
+        return SPH_OK;
+    }
 
     const int T = 256;
     float scale = (float)(1 << SPH_LMAX) / ctx->prm.box;
-    k_keys<<<nblocks(n, T), T, 0, st>>>(n, pos, scale, ctx->keys, ctx->perm);
+    SPH_CUDA(ctx, cudaMemsetAsync(&ctx->cnt->idx_err, 0, sizeof(unsigned int), st));
+    k_keys<<<nblocks(n, T), T, 0, st>>>(n, pos, scale, ctx->prm.box, ctx->keys, ctx->perm, ctx->cnt);
     ctx->launches++;
 
     // a2: stable LSD radix sort of (key, id) on the 48 key bits
@@ -275,12 +287,9 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     { uint64_t *t = ctx->keys; ctx->keys = ctx->keys_alt; ctx->keys_alt = t; }
     { uint32_t *t = ctx->perm; ctx->perm = ctx->perm_alt; ctx->perm_alt = t; }
 
-    unsigned int hc[4];
-    SPH_CUDA(ctx, cudaMemcpyAsync(hc, ctx->cnt, sizeof(hc), cudaMemcpyDeviceToHost, st));
-    SPH_CUDA(ctx, cudaStreamSynchronize(st));
+    // asynchronous: the octree and group counts stay on the device (the kernels read them there; the grids of the
+    // persistent gather kernels are sized from the particle count)
     SPH_CUDA(ctx, cudaGetLastError());
-    ctx->n_nodes = hc[0];
-    ctx->n_groups = hc[1];
     ctx->have_index = true;
     return SPH_OK;
 }
@@ -292,6 +301,7 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
     int rc;
     if (na > ctx->cap_act) {
         int64_t cap = na + na / 8 + 1024;
+        ctx->cap_act = 0;
         if ((rc = ensure(ctx, &ctx->act_slot, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->act_slot_alt, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->act_flag, cap))) return rc;
@@ -299,7 +309,6 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
         ctx->cap_act = cap;
     }
     const int T = 256;
-    SPH_CUDA(ctx, cudaMemsetAsync(&ctx->cnt->bad_ids, 0, sizeof(unsigned int), st));
     k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, ctx->n, active, ctx->inv, ctx->act_slot_alt, ctx->cnt);
     int bits = 1;
     while (bits < 32 && ((int64_t)1 << bits) < ctx->n) bits++;
@@ -311,7 +320,7 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
     if ((rc = ensure_tmp(ctx, tb))) return rc;
     size_t tbs = ctx->cub_tmp_bytes;
     SPH_CUDA(ctx, cub::DeviceRadixSort::SortKeys(ctx->cub_tmp, tbs, ctx->act_slot_alt, ctx->act_slot, (int)na, 0, bits, st));
-    k_act_flags<<<nblocks(na, T), T, 0, st>>>(na, ctx->act_slot, ctx->gid_of_slot, ctx->act_flag);
+    k_act_flags<<<nblocks(na, T), T, 0, st>>>(na, ctx->act_slot, ctx->gid_of_slot, ctx->act_flag, ctx->cnt);
     tbs = ctx->cub_tmp_bytes;
     SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),
                                              ctx->act_flag, ctx->agrp_start, &ctx->cnt->n_agroups, (int)na, st));

@@ -51,6 +51,14 @@
 #define SPH_GBLOCK 1         // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
 #endif
 
+// device-side precondition failures (SphCounters::err / idx_err)
+#define SPH_ERR_IDS 1u      // an active id outside [0, n)
+#define SPH_ERR_DUP 2u      // an active id listed twice
+#define SPH_ERR_H 4u        // a support radius <= 0 or not finite (guess of sph_density, h of sph_hydro_force)
+#define SPH_ERR_HRANGE 8u   // a support radius >= box / 2
+#define SPH_ERR_STATE 16u   // rho <= 0 or rho / omega / u / vel not finite in sph_hydro_force
+#define SPH_ERR_POS 32u     // a coordinate outside [0, box) or not finite in sph_build_index
+
 // octree node, 32 bytes, read as two 16-byte loads
 struct __align__(16) SphNode {
     uint32_t start;   // first sorted slot
@@ -69,7 +77,9 @@ struct SphCounters {
     unsigned int overflow;     // node pool exhausted (graceful: oversize leaves)
     unsigned int work;         // persistent-kernel group counter
     unsigned int n_unconv;     // density: particles stopped without convergence
-    unsigned int bad_ids;      // active ids outside [0, n) in the current active list (the call computes nothing)
+    unsigned int err;          // SPH_ERR_* bits of the calls since the last report: sticky, the gather kernels compute
+                               // nothing while it is set; the next synchronising call reports and clears it
+    unsigned int idx_err;      // SPH_ERR_POS: state of the current index (cleared by the next sph_build_index)
     unsigned int lvl_begin[SPH_LMAX + 3];
     unsigned int lvl_done[SPH_LMAX + 3];
     unsigned long long dens_evals, dens_cands, dens_pairs, force_cands, force_pairs;
@@ -98,7 +108,6 @@ struct sph_ctx {
     SphCounters *cnt;
     void *cub_tmp;
     size_t cub_tmp_bytes;
-    int64_t n_nodes, n_groups;
 
     // force pass (device)
     float4 *f_xyzh, *f_vc;
@@ -134,7 +143,7 @@ int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
 void sph_reset_counters(sph_ctx *ctx, int which, bool subset); // 0: density, 1: force
 int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t n_active);
-int sph_density_launch(sph_ctx *ctx, bool subset, int64_t n_items, float n_target, float n_tol, float *h,
+int sph_density_launch(sph_ctx *ctx, const int32_t *active, int64_t n_items, float n_target, float n_tol, float *h,
                        float *rho, float *omega, int32_t *ngb, int32_t *status);
 int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
                      const float *rho, const float *omega, float *acc, float *dudt, float *vsig);

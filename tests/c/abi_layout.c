@@ -1,0 +1,25 @@
+/* Prints size and field offsets of the structs of include/sph.h as the C compiler lays them out; the
+ * test compares them with the ctypes mirror of paper_2003_10850_b200/binding.py (tests/test_library_abi.py). */
+#include <stddef.h>
+#include <stdio.h>
+
+#include "sph.h"
+
+#define F(s, f) printf(#s "." #f " %zu\n", offsetof(s, f))
+
+int main(void)
+{
+    printf("sph_params %zu\n", sizeof(sph_params));
+    F(sph_params, kernel); F(sph_params, box); F(sph_params, gamma); F(sph_params, alpha_visc);
+    F(sph_params, count_mode); F(sph_params, max_iter); F(sph_params, group_cap); F(sph_params, group_node);
+    printf("sph_stats %zu\n", sizeof(sph_stats));
+    F(sph_stats, n); F(sph_stats, n_nodes); F(sph_stats, n_groups); F(sph_stats, launches);
+    F(sph_stats, dens_evals); F(sph_stats, dens_candidates); F(sph_stats, dens_pairs);
+    F(sph_stats, force_candidates); F(sph_stats, force_pairs);
+    F(sph_stats, t_index_ms); F(sph_stats, t_density_kernel_ms); F(sph_stats, t_force_prep_ms);
+    F(sph_stats, t_force_kernel_ms); F(sph_stats, node_pool_overflow);
+    printf("status %d %d %d %d %d %d %d %d\n", SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL,
+           SPH_E_HRANGE, SPH_W_NOCONV);
+    printf("flags %d %d %d %d\n", SPH_ST_CONVERGED, SPH_ST_BRACKET, SPH_ST_NOTCONV, SPH_ST_STALLED);
+    return 0;
+}

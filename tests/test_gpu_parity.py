@@ -362,3 +362,83 @@ def test_active_ids_out_of_range_are_reported_and_nothing_is_written():
     assert ok["unconv"] == 0 and ok["rho"][3] > 0 and ok["rho"][4] == -1
     g.sph.stats()
     g.close()
+
+
+def test_pending_error_of_an_asynchronous_call_is_sticky():
+    """after sph_hydro_force(bad ids) the NEXT synchronising call reports it -- also when that call is a
+    sph_density with a valid list (which then computes nothing itself) -- and the call after that works."""
+    ps = I.config1(8)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    one = np.ones(ps.n, np.float32)
+    gf = g.force(ps.vel, ps.u, ps.h_guess, one, one, active=np.array([2, ps.n + 5], np.int32))
+    assert np.all(gf["acc"] == 7.0)
+    with pytest.raises(B.SphError) as e:
+        g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=np.array([3, 7], np.int32))
+    assert e.value.code == B.SPH_E_ARG and "active id outside" in str(e.value)
+    ok = g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=np.array([3, 7], np.int32))
+    assert ok["unconv"] == 0 and ok["rho"][3] > 0
+    g.close()
+
+
+def test_duplicate_active_ids_are_rejected():
+    ps = I.config1(8)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    dup = np.array([5, 9, 5, 11] + [5] * 40, np.int32)
+    with pytest.raises(B.SphError) as e:
+        g.density(ps.h_guess, ps.n_ngb, ps.n_tol, active=dup)
+    assert e.value.code == B.SPH_E_ARG and "listed twice" in str(e.value)
+    g.close()
+
+
+@pytest.mark.parametrize("bad,code", [(0.0, "ARG"), (-0.1, "ARG"), (float("nan"), "ARG"), (float("inf"), "ARG"),
+                                      (0.5, "HRANGE"), (0.7, "HRANGE")])
+def test_support_radius_preconditions(bad, code):
+    """0 < H < box/2, finite: checked on the device for the guesses of sph_density (active particles only) and for
+    h of all particles in sph_hydro_force; a violation computes and writes nothing."""
+    ps = I.config1(8)
+    want = getattr(B, "SPH_E_" + code)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    hb = ps.h_guess.copy()
+    hb[17] = bad
+    with pytest.raises(B.SphError) as e:
+        g.density(hb, ps.n_ngb, ps.n_tol)
+    assert e.value.code == want
+    # an inactive particle's guess is not looked at by sph_density ...
+    act = np.array([1, 2, 3], np.int32)
+    ok = g.density(hb, ps.n_ngb, ps.n_tol, active=act)
+    assert ok["unconv"] == 0 and np.all(ok["rho"][act] > 0)
+    # ... but its h is a force input (it is somebody's neighbour)
+    full = g.density(ps.h_guess, ps.n_ngb, ps.n_tol)
+    hh = full["H"].copy()
+    hh[17] = bad
+    gf = g.force(ps.vel, ps.u, hh, full["rho"], full["omega"], active=act)
+    assert np.all(gf["acc"] == 7.0)
+    with pytest.raises(B.SphError) as e:
+        g.sph.stats()
+    assert e.value.code == want
+    rb = full["rho"].copy()
+    rb[40] = 0.0
+    g.force(ps.vel, ps.u, full["H"], rb, full["omega"])
+    with pytest.raises(B.SphError) as e:
+        g.sph.stats()
+    assert e.value.code == B.SPH_E_ARG and "rho" in str(e.value)
+    gf = g.force(ps.vel, ps.u, full["H"], full["rho"], full["omega"])
+    g.sph.stats()
+    assert np.all(gf["acc"] != 7.0)
+    g.close()
+
+
+@pytest.mark.parametrize("bad", [1.0, -1e-3, float("nan")])
+def test_position_preconditions(bad):
+    """0 <= x < box: a coordinate outside makes the index unusable; every call reports it until a rebuild."""
+    ps = I.config1(8)
+    pos = ps.pos.copy()
+    pos[100, 1] = bad
+    g = GpuRun(pos, ps.kernel, ps.mass)  # sph_build_index is asynchronous: no error yet
+    for _ in range(2):
+        with pytest.raises(B.SphError) as e:
+            g.density(ps.h_guess, ps.n_ngb, ps.n_tol)
+        assert e.value.code == B.SPH_E_ARG and "position outside" in str(e.value)
+    g.sph.sph_build_index(g.pos.copy_(torch.from_numpy(ps.pos)), None, ps.mass)
+    assert g.density(ps.h_guess, ps.n_ngb, ps.n_tol)["unconv"] == 0
+    g.close()

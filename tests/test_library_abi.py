@@ -20,7 +20,7 @@ def test_header_symbols_exported():
     lib = ctypes.CDLL(build.build())
     names = _declared()
     assert {"sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
-            "sph_get_stats", "sph_fp32_peak", "sph_last_error", "sph_version"} <= set(names)
+            "sph_get_stats", "sph_last_error", "sph_version"} <= set(names)
     for n in names:
         assert hasattr(lib, n), n
     lib.sph_version.restype = ctypes.c_char_p
@@ -31,6 +31,32 @@ def test_binding_lists_the_same_entry_points():
     from paper_2003_10850_b200 import binding
 
     assert sorted(binding.EXPORTS) == _declared()
+
+
+def test_struct_layout_matches_the_c_header(tmp_path):
+    """The ctypes mirror of binding.py against the layout the C compiler gives include/sph.h (tests/c/abi_layout.c),
+    field by field; the enums too.  The C caller itself runs in tests/test_gpu_abi_c.py."""
+    import subprocess
+
+    from paper_2003_10850_b200 import binding as B
+
+    exe = str(tmp_path / "abi_layout")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-o", exe, os.path.join(ROOT, "tests", "c", "abi_layout.c"),
+                           "-I", os.path.join(ROOT, "include")])
+    out = dict(l.split(None, 1) for l in subprocess.check_output([exe], text=True).splitlines())
+    for name, cls in (("sph_params", B.SphParams), ("sph_stats", B.SphStats)):
+        assert int(out[name]) == ctypes.sizeof(cls)
+        fields = [f for f, _ in cls._fields_]
+        assert sorted(k.split(".")[1] for k in out if k.startswith(name + ".")) == sorted(fields)
+        for f in fields:
+            assert int(out[f"{name}.{f}"]) == getattr(cls, f).offset, (name, f)
+    assert [int(x) for x in out["status"].split()] == [B.SPH_OK, B.SPH_E_ARG, B.SPH_E_CUDA, B.SPH_E_NOINDEX, B.SPH_E_OOM,
+                                                       B.SPH_E_INTERNAL, B.SPH_E_HRANGE, B.SPH_W_NOCONV]
+    assert [int(x) for x in out["flags"].split()] == [B.ST_CONVERGED, B.ST_BRACKET, B.ST_NOTCONV, B.ST_STALLED]
+    # the smoke caller compiles against the header, too (it runs on the GPU box)
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-c", "-o", str(tmp_path / "abi_smoke.o"),
+                           os.path.join(ROOT, "tests", "c", "abi_smoke.c"), "-I", os.path.join(ROOT, "include"),
+                           "-I", "/usr/local/cuda/include"])
 
 
 def test_no_cpu_fallback_without_device():
