@@ -5,8 +5,6 @@
 // :72 §2.1, :194-196 §4) and its N_min CPU fallback for small active sets (§2.2).
 #include <stddef.h>
 
-#include <cub/cub.cuh>
-
 #include "sph_internal.cuh"
 
 namespace {
@@ -182,18 +180,6 @@ int ensure(sph_ctx *ctx, T **p, size_t count)
     return SPH_OK;
 }
 
-int ensure_tmp(sph_ctx *ctx, size_t bytes)
-{
-    if (bytes <= ctx->cub_tmp_bytes) return SPH_OK;
-    if (ctx->cub_tmp) cudaFree(ctx->cub_tmp);
-    ctx->cub_tmp = nullptr;
-    ctx->cub_tmp_bytes = 0;
-    bytes = bytes + bytes / 4 + 4096;
-    SPH_CUDA(ctx, cudaMalloc(&ctx->cub_tmp, bytes));
-    ctx->cub_tmp_bytes = bytes;
-    return SPH_OK;
-}
-
 inline int nblocks(int64_t n, int t) { return (int)((n + t - 1) / t); }
 
 } // namespace
@@ -241,23 +227,15 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     k_keys<<<nblocks(n, T), T, 0, st>>>(n, pos, scale, ctx->prm.box, ctx->keys, ctx->perm, ctx->cnt);
     ctx->launches++;
 
-    // a2: stable LSD radix sort of (key, id) on the 48 key bits
-    size_t tb = 0;
-    SPH_CUDA(ctx, cub::DeviceRadixSort::SortPairs(nullptr, tb, ctx->keys, ctx->keys_alt, ctx->perm, ctx->perm_alt,
-                                                  (int)n, 0, SPH_KEY_BITS, st));
-    size_t tb2 = 0, tb3 = 0;
-    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(nullptr, tb2, cub::CountingInputIterator<uint32_t>(0), ctx->grp_mark,
-                                             ctx->grp_start, &ctx->cnt->n_groups, (int)n, st));
-    SPH_CUDA(ctx, cub::DeviceScan::InclusiveSum(nullptr, tb3, ctx->grp_mark, ctx->gid_of_slot, (int)n, st));
-    if (tb2 > tb) tb = tb2;
-    if (tb3 > tb) tb = tb3;
-    if ((rc = ensure_tmp(ctx, tb))) return rc;
-    size_t tbs = ctx->cub_tmp_bytes;
-    SPH_CUDA(ctx, cub::DeviceRadixSort::SortPairs(ctx->cub_tmp, tbs, ctx->keys, ctx->keys_alt, ctx->perm,
-                                                  ctx->perm_alt, (int)n, 0, SPH_KEY_BITS, st));
-    ctx->launches += 1 + 2 * ((SPH_KEY_BITS + 7) / 8); // histogram + (scan+scatter | onesweep) passes, nominal
-    const uint64_t *skeys = ctx->keys_alt;
-    const uint32_t *sperm = ctx->perm_alt;
+    // a2: stable LSD radix sort of (key, id) on the 48 key bits (sph_sort.cu)
+    int in_alt = 0;
+    if ((rc = sph_sort_pairs_u64(ctx, ctx->keys, ctx->keys_alt, ctx->perm, ctx->perm_alt, n, SPH_KEY_BITS, &in_alt))) return rc;
+    if (in_alt) { // the sorted data must sit in ctx->keys / ctx->perm
+        { uint64_t *t = ctx->keys; ctx->keys = ctx->keys_alt; ctx->keys_alt = t; }
+        { uint32_t *t = ctx->perm; ctx->perm = ctx->perm_alt; ctx->perm_alt = t; }
+    }
+    const uint64_t *skeys = ctx->keys;
+    const uint32_t *sperm = ctx->perm;
 
     k_permute<<<nblocks(n, T), T, 0, st>>>(n, pos, mass, ctx->mass_scalar, sperm, ctx->xyzm, ctx->inv);
     ctx->launches++;
@@ -276,16 +254,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)ctx->grp_cap,
                                         (uint32_t)(ctx->grp_node > SPH_LEAF ? ctx->grp_node : SPH_LEAF), ctx->grp_mark);
     ctx->launches++;
-    tbs = ctx->cub_tmp_bytes;
-    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),
-                                             ctx->grp_mark, ctx->grp_start, &ctx->cnt->n_groups, (int)n, st));
-    tbs = ctx->cub_tmp_bytes;
-    SPH_CUDA(ctx, cub::DeviceScan::InclusiveSum(ctx->cub_tmp, tbs, ctx->grp_mark, ctx->gid_of_slot, (int)n, st));
-    ctx->launches += 4;
-
-    // perm must survive in ctx->perm (keys_alt/perm_alt hold the sorted data): swap the handles
-    { uint64_t *t = ctx->keys; ctx->keys = ctx->keys_alt; ctx->keys_alt = t; }
-    { uint32_t *t = ctx->perm; ctx->perm = ctx->perm_alt; ctx->perm_alt = t; }
+    if ((rc = sph_scan_marks(ctx, ctx->grp_mark, n, ctx->gid_of_slot, ctx->grp_start, &ctx->cnt->n_groups))) return rc;
 
     // asynchronous: the octree and group counts stay on the device (the kernels read them there; the grids of the
     // persistent gather kernels are sized from the particle count)
@@ -312,18 +281,11 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
     k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, ctx->n, active, ctx->inv, ctx->act_slot_alt, ctx->cnt);
     int bits = 1;
     while (bits < 32 && ((int64_t)1 << bits) < ctx->n) bits++;
-    size_t tb = 0, tb2 = 0;
-    SPH_CUDA(ctx, cub::DeviceRadixSort::SortKeys(nullptr, tb, ctx->act_slot_alt, ctx->act_slot, (int)na, 0, bits, st));
-    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(nullptr, tb2, cub::CountingInputIterator<uint32_t>(0), ctx->act_flag,
-                                             ctx->agrp_start, &ctx->cnt->n_agroups, (int)na, st));
-    if (tb2 > tb) tb = tb2;
-    if ((rc = ensure_tmp(ctx, tb))) return rc;
-    size_t tbs = ctx->cub_tmp_bytes;
-    SPH_CUDA(ctx, cub::DeviceRadixSort::SortKeys(ctx->cub_tmp, tbs, ctx->act_slot_alt, ctx->act_slot, (int)na, 0, bits, st));
+    int in_alt = 0;
+    if ((rc = sph_sort_keys_u32(ctx, ctx->act_slot_alt, ctx->act_slot, na, bits, &in_alt))) return rc;
+    if (!in_alt) { uint32_t *t = ctx->act_slot; ctx->act_slot = ctx->act_slot_alt; ctx->act_slot_alt = t; } // sorted slots -> act_slot
     k_act_flags<<<nblocks(na, T), T, 0, st>>>(na, ctx->act_slot, ctx->gid_of_slot, ctx->act_flag, ctx->cnt);
-    tbs = ctx->cub_tmp_bytes;
-    SPH_CUDA(ctx, cub::DeviceSelect::Flagged(ctx->cub_tmp, tbs, cub::CountingInputIterator<uint32_t>(0),
-                                             ctx->act_flag, ctx->agrp_start, &ctx->cnt->n_agroups, (int)na, st));
-    ctx->launches += 2 + 2 + 1 + 2 * ((bits + 7) / 8);
+    if ((rc = sph_scan_marks(ctx, ctx->act_flag, na, nullptr, ctx->agrp_start, &ctx->cnt->n_agroups))) return rc;
+    ctx->launches += 2;
     return SPH_OK;
 }

@@ -106,8 +106,10 @@ struct sph_ctx {
     int64_t node_cap;
     uint32_t *grp_mark, *gid_of_slot, *grp_start;
     SphCounters *cnt;
-    void *cub_tmp;
-    size_t cub_tmp_bytes;
+    uint32_t *sort_hist;   // radix sort: per-tile digit histograms + digit bases
+    size_t sort_cap;
+    uint32_t *scan_bsum;   // scan: block sums
+    size_t scan_cap;
 
     // force pass (device)
     float4 *f_xyzh, *f_vc;
@@ -141,6 +143,12 @@ int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
 
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
+// stable LSD radix sort on the low `bits` key bits; *in_alt = 1 if the result ended up in the *_alt buffers
+int sph_sort_pairs_u64(sph_ctx *ctx, uint64_t *keys, uint64_t *keys_alt, uint32_t *vals, uint32_t *vals_alt, int64_t n, int bits,
+                       int *in_alt);
+int sph_sort_keys_u32(sph_ctx *ctx, uint32_t *keys, uint32_t *keys_alt, int64_t n, int bits, int *in_alt);
+// inclusive scan of 0/1 marks (incl may be NULL) + positions of the marks (start) + their number (*count_dev, device)
+int sph_scan_marks(sph_ctx *ctx, const uint32_t *mark, int64_t n, uint32_t *incl, uint32_t *start, unsigned int *count_dev);
 void sph_reset_counters(sph_ctx *ctx, int which, bool subset); // 0: density, 1: force
 int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t n_active);
 int sph_density_launch(sph_ctx *ctx, const int32_t *active, int64_t n_items, float n_target, float n_tol, float *h,
