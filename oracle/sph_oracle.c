@@ -487,3 +487,131 @@ int orc_num_threads(void)
     return 1;
 #endif
 }
+
+/* ================================================================ improved-SPH extension
+ * "Improved SPH" of the paper's ref [6] (PAPER.md:25 §1, :209): the paper only cites it.  What is stated
+ * here are the READINGS R17-R20 of DESIGN.md, restated from the published lineage (velocity-gradient
+ * estimators of the Gadget lineage [2]; shear limiter of Balsara; time-dependent viscosity of Morris &
+ * Monaghan; artificial conduction in the signal-velocity form of Price).
+ *
+ * R17  velocity divergence and curl with the particle's own support radius (gather form, no grad-h factor):
+ *        (div v)_i  = (1/rho_i) sum_j m_j (v_j - v_i) . grad_i W_ij(H_i)
+ *        (curl v)_i = (1/rho_i) sum_j m_j (v_i - v_j) x grad_i W_ij(H_i),   grad_i W_ij = dW/dr(r_ij, H_i) rhat_ij,
+ *      rhat_ij = (x_i - x_j)/r_ij, over j != i with r_ij < H_i.
+ * R18  shear limiter  f_i = |div v_i| / (|div v_i| + |curl v_i| + 1e-4 c_i / H_i);  Pi_ij is multiplied by (f_i + f_j)/2.
+ * R19  per-particle viscosity coefficient alpha_i (input): Pi_ij uses (alpha_i + alpha_j)/2 in place of alpha;
+ *      its evolution equation  d alpha_i/dt = -(alpha_i - alpha_min) / tau_i + S_i,
+ *      tau_i = H_i / (2 l c_i),  S_i = max(0, -div v_i) (alpha_max - alpha_i).
+ * R20  artificial conduction: du_i/dt += sum_j m_j alpha_c vsig^u_ij (u_i - u_j) Fbar_ij / rhobar_ij,
+ *      vsig^u_ij = sqrt(|P_i - P_j| / rhobar_ij), Fbar = (F_ij(H_i) + F_ij(H_j))/2 (<= 0), same pair set as the force.
+ * Everything else (pair set, pressure terms, signal velocity, v_sig maximum) is R8-R12 unchanged.
+ */
+typedef struct {
+    double alpha_min, alpha_max, decay_l; /* R19 */
+    double alpha_cond;                    /* R20; 0 switches conduction off */
+    int balsara;                          /* R18 on/off */
+} orc_improved;
+
+int orc_velocity_gradients(const orc_params *p, int64_t n, const float *pos, const float *vel, const float *mass,
+                           double mass_scalar, const float *h, const float *rho, const int32_t *active, int64_t n_active,
+                           double *divv, double *curlv /* na*3 */)
+{
+    int64_t na = active ? n_active : n;
+    double L = p->box;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        double Hi = (double)h[i], dv = 0.0, cx = 0.0, cy = 0.0, cz = 0.0;
+        for (int64_t j = 0; j < n; j++) { /* plain definition: all j (brute force) */
+            if (j == i) continue;
+            double d[3];
+            for (int k = 0; k < 3; k++) d[k] = min_image((double)pos[3 * i + k] - (double)pos[3 * j + k], L);
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            if (!(r2 < Hi * Hi) || r2 == 0.0) continue;
+            double r = sqrt(r2);
+            double mj = mass ? (double)mass[j] : mass_scalar;
+            double g = mj * orc_dWdr(p->kernel, r, Hi) / r; /* m_j dW/dr / r: grad W = g/m_j * d */
+            double w[3];
+            for (int k = 0; k < 3; k++) w[k] = (double)vel[3 * j + k] - (double)vel[3 * i + k];
+            dv += g * (w[0] * d[0] + w[1] * d[1] + w[2] * d[2]);
+            cx -= g * (w[1] * d[2] - w[2] * d[1]); /* (v_i - v_j) x grad W = -w x grad W */
+            cy -= g * (w[2] * d[0] - w[0] * d[2]);
+            cz -= g * (w[0] * d[1] - w[1] * d[0]);
+        }
+        double ir = 1.0 / (double)rho[i];
+        divv[a] = dv * ir;
+        curlv[3 * a] = cx * ir; curlv[3 * a + 1] = cy * ir; curlv[3 * a + 2] = cz * ir;
+    }
+    return 0;
+}
+
+/* R18 */
+static double balsara_f(double divv, const float *curl, double c, double H)
+{
+    double cm = sqrt((double)curl[0] * curl[0] + (double)curl[1] * curl[1] + (double)curl[2] * curl[2]);
+    return fabs(divv) / (fabs(divv) + cm + 1e-4 * c / H);
+}
+
+int orc_hydro_force_improved(const orc_params *p, const orc_improved *q, int64_t n, const float *pos, const float *vel,
+                             const float *u, const float *mass, double mass_scalar, const float *h, const float *rho,
+                             const float *omega, const float *alpha, const float *divv, const float *curlv,
+                             const int32_t *active, int64_t n_active, double *acc, double *dudt, double *vsig,
+                             double *dalpha, double *asum, double *dusum, double *asq, double *dusq, double *ducond)
+{
+    int64_t na = active ? n_active : n;
+    double L = p->box, gm1 = p->gamma - 1.0, sg = k_sigma(p->kernel);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        double Hi = (double)h[i], rhoi = (double)rho[i], ui = (double)u[i];
+        double ci = sqrt(p->gamma * gm1 * ui), Pi_ = gm1 * rhoi * ui;
+        double Ai = gm1 * ui / ((double)omega[i] * rhoi);
+        double fi = q->balsara ? balsara_f((double)divv[i], curlv + 3 * i, ci, Hi) : 1.0;
+        double ax = 0, ay = 0, az = 0, du = 0, vs = 0, as = 0, dus = 0, a2 = 0, du2 = 0, duc = 0;
+        for (int64_t j = 0; j < n; j++) { /* plain definition: all j (brute force) */
+            if (j == i) continue;
+            double d[3];
+            for (int k = 0; k < 3; k++) d[k] = min_image((double)pos[3 * i + k] - (double)pos[3 * j + k], L);
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            double Hj = (double)h[j], Hm = Hi > Hj ? Hi : Hj;
+            if (!(r2 < Hm * Hm)) continue;
+            double uj = (double)u[j], rhoj = (double)rho[j];
+            double cj = sqrt(p->gamma * gm1 * uj);
+            if (r2 == 0.0) { if (ci + cj > vs) vs = ci + cj; continue; }
+            double r = sqrt(r2);
+            double Aj = gm1 * uj / ((double)omega[j] * rhoj);
+            double mj = mass ? (double)mass[j] : mass_scalar;
+            double Fi = r < Hi ? sg / (Hi * Hi * Hi * Hi) * k_dw(p->kernel, r / Hi) : 0.0;
+            double Fj = r < Hj ? sg / (Hj * Hj * Hj * Hj) * k_dw(p->kernel, r / Hj) : 0.0;
+            double vr = 0.0;
+            for (int k = 0; k < 3; k++) vr += ((double)vel[3 * i + k] - (double)vel[3 * j + k]) * d[k] / r;
+            double mu = vr < 0.0 ? vr : 0.0;
+            double vsij = ci + cj - 3.0 * mu;
+            double rb = 0.5 * (rhoi + rhoj);
+            double aij = 0.5 * ((double)alpha[i] + (double)alpha[j]);                                       /* R19 */
+            double fj = q->balsara ? balsara_f((double)divv[j], curlv + 3 * j, cj, Hj) : 1.0;
+            double PI = -0.5 * aij * vsij * mu / rb * 0.5 * (fi + fj);                                       /* R9, R18 */
+            double Fbar = 0.5 * (Fi + Fj);
+            double t = mj * (Ai * Fi + Aj * Fj + PI * Fbar);
+            ax -= t * d[0] / r; ay -= t * d[1] / r; az -= t * d[2] / r;
+            as += fabs(t); a2 += t * t;
+            double e = mj * (Ai * Fi + 0.5 * PI * Fbar) * vr;
+            double Pj_ = gm1 * rhoj * uj;
+            double ec = mj * q->alpha_cond * sqrt(fabs(Pi_ - Pj_) / rb) * (ui - uj) * Fbar / rb;             /* R20 */
+            du += e + ec; duc += ec;
+            dus += fabs(e) + fabs(ec); du2 += e * e + ec * ec;
+            if (vsij > vs) vs = vsij;
+        }
+        acc[3 * a] = ax; acc[3 * a + 1] = ay; acc[3 * a + 2] = az;
+        dudt[a] = du; vsig[a] = vs;
+        double tau = Hi / (2.0 * q->decay_l * ci);
+        double S = ((double)divv[i] < 0.0 ? -(double)divv[i] : 0.0) * (q->alpha_max - (double)alpha[i]);
+        dalpha[a] = -((double)alpha[i] - q->alpha_min) / tau + S;                                            /* R19 */
+        if (asum) asum[a] = as;
+        if (dusum) dusum[a] = dus;
+        if (asq) asq[a] = a2;
+        if (dusq) dusq[a] = du2;
+        if (ducond) ducond[a] = duc;
+    }
+    return 0;
+}

@@ -172,3 +172,46 @@ def hydro_force(pos, vel, u, h, rho, omega, *, kernel, box=1.0, gamma=5.0 / 3.0,
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv))
+
+
+# ---------------------------------------------------------------- improved-SPH extension (R17-R20)
+class _Improved(C.Structure):
+    _fields_ = [("alpha_min", C.c_double), ("alpha_max", C.c_double), ("decay_l", C.c_double), ("alpha_cond", C.c_double),
+                ("balsara", C.c_int)]
+
+
+def velocity_gradients(pos, vel, h, rho, *, kernel, box=1.0, mass=None, mass_scalar=1.0, active=None):
+    """R17: div v and curl v with the particle's own support radius (brute force over all j). Returns dict divv (na), curlv (na,3)."""
+    pos_, ppos = _p(pos, np.float32)
+    vel_, pvel = _p(vel, np.float32)
+    h_, ph = _p(h, np.float32)
+    rho_, prho = _p(rho, np.float32)
+    m_, pm = _p(mass, np.float32)
+    act_, pact = _p(active, np.int32)
+    n = pos_.shape[0]
+    na = n if act_ is None else act_.shape[0]
+    out = {"divv": np.zeros(na, np.float64), "curlv": np.zeros((na, 3), np.float64)}
+    prm = _params(kernel, box, 5.0 / 3.0, 1.0, 0, 64)
+    lib().orc_velocity_gradients(C.byref(prm), C.c_int64(n), ppos, pvel, pm, C.c_double(mass_scalar), ph, prho, pact,
+                                 C.c_int64(na), out["divv"].ctypes.data_as(C.c_void_p), out["curlv"].ctypes.data_as(C.c_void_p))
+    return out
+
+
+def hydro_force_improved(pos, vel, u, h, rho, omega, alpha, divv, curlv, *, kernel, box=1.0, gamma=5.0 / 3.0, mass=None,
+                         mass_scalar=1.0, active=None, alpha_min=0.02, alpha_max=3.0, decay_l=4.0, alpha_cond=0.25, balsara=True):
+    """R8-R12 with R18-R20 (brute force over all j). Returns dict acc (na,3), dudt, vsig, dalpha, asum, dusum, asq, dusq, ducond."""
+    arrs = [_p(a, np.float32) for a in (pos, vel, u, h, rho, omega, alpha, divv, curlv)]
+    m_, pm = _p(mass, np.float32)
+    act_, pact = _p(active, np.int32)
+    n = arrs[0][0].shape[0]
+    na = n if act_ is None else act_.shape[0]
+    out = {"acc": np.zeros((na, 3), np.float64)}
+    for k in ("dudt", "vsig", "dalpha", "asum", "dusum", "asq", "dusq", "ducond"):
+        out[k] = np.zeros(na, np.float64)
+    prm = _params(kernel, box, gamma, 1.0, 0, 64)
+    q = _Improved(alpha_min, alpha_max, decay_l, alpha_cond, int(bool(balsara)))
+    (_, ppos), (_, pvel), (_, pu), (_, ph), (_, prho), (_, pom), (_, pal), (_, pdv), (_, pcv) = arrs
+    lib().orc_hydro_force_improved(C.byref(prm), C.byref(q), C.c_int64(n), ppos, pvel, pu, pm, C.c_double(mass_scalar), ph, prho,
+                                   pom, pal, pdv, pcv, pact, C.c_int64(na),
+                                   *[out[k].ctypes.data_as(C.c_void_p) for k in ("acc", "dudt", "vsig", "dalpha", "asum", "dusum", "asq", "dusq", "ducond")])
+    return out
