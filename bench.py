@@ -237,6 +237,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extension", action="store_true", help="skip the improved-SPH extension timing")
     ap.add_argument("--group-cap", type=int, default=0, help="actives per group (0 = library default)")
     ap.add_argument("--group-node", type=int, default=0, help="group-node capacity (0 = library default)")
     args = ap.parse_args()
@@ -334,6 +335,23 @@ def main():
     its = (stt & 0xff) if active is None else (stt.index_select(0, active.long()) & 0xff)
     eval_hist = torch.bincount(its.long(), minlength=2).cpu().tolist()
     launches = per[-1]["launches"] - l0
+    # improved-SPH extension, outside the timed region: cost of the velocity-gradient pass and of the
+    # force pass with per-particle alpha, shear limiter and conduction on the same converged state (CUDA events)
+    ext_ms = None
+    if not args.no_extension:
+        dvv, da = torch.zeros(n, device="cuda"), torch.zeros(n, device="cuda")
+        cvv = torch.zeros((n, 3), device="cuda")
+        alp = torch.full((n,), 1.0, device="cuda")
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        for rep in range(2):  # first round warms up
+            ev[0].record(stream)
+            sph.sph_velocity_gradients(vel, h, rho, dvv, cvv, active=active)
+            ev[1].record(stream)
+            sph.sph_hydro_force_improved(vel, u, h, rho, om, alp, dvv, cvv, acc, du, vs, da, active=active)
+            ev[2].record(stream)
+            torch.cuda.synchronize()
+        ext_ms = {"velocity_gradients": ev[0].elapsed_time(ev[1]), "hydro_force_improved": ev[1].elapsed_time(ev[2]),
+                  "note": "whole calls incl. the sorted-state preparation; base sph_hydro_force in phases_ms"}
     ms = max_over_ranks(ms, world, "cuda")
     value = whole_job_value(world, n_active, args.steps, ms)
 
@@ -418,6 +436,7 @@ def main():
             "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
             "e2e": e2e, "gpu_launches": int(launches), "roofline": roof,
             "phases_ms": {"index": ti, "density_kernel": tk, "force_prep": tp, "force_kernel": tf},
+            "improved_sph_extension_ms": ext_ms,
             "pairs": {"density_evals_per_particle": st["dens_evals"] / n_active,
                       "density_true_pairs": st["dens_pairs"], "density_candidates": st["dens_candidates"],
                       "force_true_pairs": st["force_pairs"], "force_candidates": st["force_candidates"],

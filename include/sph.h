@@ -159,6 +159,40 @@ int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const
                     float *vsig_max);
 
 /*
+ * Improved-SPH extension: the SPH flavour the paper's runs use is "the improved SPH
+ * of ref [6]" (PAPER.md:25 §1, :209), which the paper only cites; readings R17-R20.
+ *
+ * sph_velocity_gradients -- R17, a third gather over the same index: for every active particle i, over
+ * j != i with r_ij < H_i (its own support),
+ *   divv[id]       = (1/rho_i) sum_j m_j (v_j - v_i) . grad_i W_ij(H_i)
+ *   curlv[id*3..]  = (1/rho_i) sum_j m_j (v_i - v_j) x grad_i W_ij(H_i),  grad_i W_ij = dW/dr(r_ij, H_i) rhat_ij.
+ * vel [n*3], h [n], rho [n] device, valid for all particles; divv [n], curlv [n*3] written for active
+ * particles only.  Asynchronous; preconditions and error reporting as sph_hydro_force.
+ *
+ * sph_hydro_force_improved -- sph_hydro_force with
+ *   R19 a per-particle viscosity coefficient: Pi_ij uses (alpha_i + alpha_j)/2 in place of alpha_visc, and
+ *       dalpha_dt[id] = -(alpha_i - alpha_min) 2 l c_i / H_i + max(0, -div v_i)(alpha_max - alpha_i);
+ *   R18 the shear limiter f_i = |div v_i| / (|div v_i| + |curl v_i| + 1e-4 c_i / H_i) (if balsara != 0):
+ *       Pi_ij is multiplied by (f_i + f_j)/2;
+ *   R20 artificial conduction: dudt += sum_j m_j alpha_cond sqrt(|P_i - P_j| / rho_ij) (u_i - u_j) Fbar_ij / rho_ij.
+ * alpha [n], divv [n], curlv [n*3]: device, valid for ALL particles (neighbours contribute with theirs).
+ */
+typedef struct {
+    float alpha_min;   /* floor of the viscosity coefficient (0.02) */
+    float alpha_max;   /* its ceiling (3.0) */
+    float decay_l;     /* decay length l of R19 (4.0) */
+    float alpha_cond;  /* artificial conduction coefficient (0.25); 0 switches conduction off */
+    int balsara;       /* shear limiter on / off */
+} sph_improved_params;
+
+int sph_velocity_gradients(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *h,
+                           const float *rho, float *divv, float *curlv);
+int sph_hydro_force_improved(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
+                             const float *h, const float *rho, const float *omega, const float *alpha, const float *divv,
+                             const float *curlv, const sph_improved_params *ip, float *acc, float *dudt, float *vsig_max,
+                             float *dalpha_dt);
+
+/*
  * One whole pass of the hot path with HOST buffers (used for the end-to-end measurement): copies
  * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
  * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries

@@ -19,7 +19,7 @@ ST_CONVERGED, ST_BRACKET, ST_NOTCONV, ST_STALLED = 1 << 8, 1 << 9, 1 << 10, 1 <<
 KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
-           "sph_get_stats", "sph_last_error", "sph_version"]
+           "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -32,6 +32,11 @@ class SphStats(C.Structure):
                                          "dens_pairs", "force_candidates", "force_pairs")] + \
                [(k, C.c_float) for k in ("t_index_ms", "t_density_kernel_ms", "t_force_prep_ms", "t_force_kernel_ms")] + \
                [("node_pool_overflow", C.c_int64)]
+
+
+class SphImprovedParams(C.Structure):
+    _fields_ = [("alpha_min", C.c_float), ("alpha_max", C.c_float), ("decay_l", C.c_float), ("alpha_cond", C.c_float),
+                ("balsara", C.c_int)]
 
 
 class SphError(RuntimeError):
@@ -63,7 +68,10 @@ def load():
         lib.sph_last_error.argtypes = [C.c_void_p]
         lib.sph_last_error.restype = C.c_char_p
         lib.sph_version.restype = C.c_char_p
-        for name in EXPORTS[:7]:
+        lib.sph_velocity_gradients.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 5
+        lib.sph_hydro_force_improved.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 8 + \
+                                                [C.POINTER(SphImprovedParams)] + [C.c_void_p] * 4
+        for name in EXPORTS[:9]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -150,6 +158,27 @@ class Sph:
                                               _dev(acc, torch.float32, "acc", 3 * n),
                                               _dev(dudt, torch.float32, "dudt", n),
                                               _dev(vsig_max, torch.float32, "vsig_max", n)))
+
+    # -- improved-SPH extension (R17-R20) ----------------------------------------------
+    def sph_velocity_gradients(self, vel, h, rho, divv, curlv, active=None):
+        n = self.n
+        na = -1 if active is None else active.numel()
+        self._check(self._lib.sph_velocity_gradients(self._h, _dev(active, torch.int32, "active"), na,
+                                                     _dev(vel, torch.float32, "vel", 3 * n), _dev(h, torch.float32, "h", n),
+                                                     _dev(rho, torch.float32, "rho", n), _dev(divv, torch.float32, "divv", n),
+                                                     _dev(curlv, torch.float32, "curlv", 3 * n)))
+
+    def sph_hydro_force_improved(self, vel, u, h, rho, omega, alpha, divv, curlv, acc, dudt, vsig_max, dalpha_dt, active=None,
+                                 alpha_min=0.02, alpha_max=3.0, decay_l=4.0, alpha_cond=0.25, balsara=True):
+        n = self.n
+        na = -1 if active is None else active.numel()
+        ip = SphImprovedParams(alpha_min, alpha_max, decay_l, alpha_cond, int(bool(balsara)))
+        f32 = torch.float32
+        self._check(self._lib.sph_hydro_force_improved(
+            self._h, _dev(active, torch.int32, "active"), na, _dev(vel, f32, "vel", 3 * n), _dev(u, f32, "u", n),
+            _dev(h, f32, "h", n), _dev(rho, f32, "rho", n), _dev(omega, f32, "omega", n), _dev(alpha, f32, "alpha", n),
+            _dev(divv, f32, "divv", n), _dev(curlv, f32, "curlv", 3 * n), C.byref(ip), _dev(acc, f32, "acc", 3 * n),
+            _dev(dudt, f32, "dudt", n), _dev(vsig_max, f32, "vsig_max", n), _dev(dalpha_dt, f32, "dalpha_dt", n)))
 
     def sph_step_host(self, pos, vel, u, mass_scalar, h, rho, omega, ngb_count, acc, dudt, vsig, n_ngb_target,
                       n_ngb_tol, active=None):

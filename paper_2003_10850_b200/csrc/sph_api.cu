@@ -113,7 +113,7 @@ int sph_destroy(sph_ctx *ctx)
     cudaStreamSynchronize(ctx->stream);
     dfree(ctx->keys); dfree(ctx->keys_alt); dfree(ctx->perm); dfree(ctx->perm_alt); dfree(ctx->inv);
     dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->grp_start);
-    dfree(ctx->cnt); dfree(ctx->sort_hist); dfree(ctx->scan_bsum); dfree(ctx->f_xyzh); dfree(ctx->f_vc);
+    dfree(ctx->cnt); dfree(ctx->sort_hist); dfree(ctx->scan_bsum); dfree(ctx->f_xyzh); dfree(ctx->f_vc); dfree(ctx->f_ext);
     dfree(ctx->node_hmax); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
@@ -185,7 +185,49 @@ int sph_hydro_force(sph_ctx *ctx, const int32_t *active, int64_t n_active, const
     int rc = check_sticky(ctx);
     if (rc) return rc;
     if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
-    return sph_force_launch(ctx, active != nullptr, items, vel, u, h, rho, omega, acc, dudt, vsig_max);
+    return sph_force_launch(ctx, SPH_MODE_BASE, active != nullptr, items, vel, u, h, rho, omega, acc, dudt, vsig_max, nullptr, nullptr,
+                            nullptr, nullptr, nullptr, nullptr, nullptr);
+}
+
+int sph_velocity_gradients(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *h,
+                           const float *rho, float *divv, float *curlv)
+{
+    if (!ctx) return SPH_E_ARG;
+    Range nv("sph_velocity_gradients");
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_velocity_gradients before sph_build_index");
+    const bool subset = active != nullptr || n_active == 0;
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_velocity_gradients: n_active < 0");
+    int64_t items = subset ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!vel || !h || !rho || !divv || !curlv) return sph_fail(ctx, SPH_E_ARG, "sph_velocity_gradients: NULL array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    return sph_force_launch(ctx, SPH_MODE_GRADV, active != nullptr, items, vel, nullptr, h, rho, nullptr, nullptr, nullptr, nullptr,
+                            nullptr, nullptr, nullptr, nullptr, nullptr, divv, curlv);
+}
+
+int sph_hydro_force_improved(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
+                             const float *h, const float *rho, const float *omega, const float *alpha, const float *divv,
+                             const float *curlv, const sph_improved_params *ip, float *acc, float *dudt, float *vsig_max,
+                             float *dalpha_dt)
+{
+    if (!ctx) return SPH_E_ARG;
+    Range nv("sph_hydro_force_improved");
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_hydro_force_improved before sph_build_index");
+    if (!ip || !(ip->alpha_min >= 0.f) || !(ip->alpha_max >= ip->alpha_min) || !(ip->decay_l > 0.f) || !(ip->alpha_cond >= 0.f))
+        return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force_improved: bad sph_improved_params");
+    const bool subset = active != nullptr || n_active == 0;
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force_improved: n_active < 0");
+    int64_t items = subset ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!vel || !u || !h || !rho || !omega || !alpha || !divv || !curlv || !acc || !dudt || !vsig_max || !dalpha_dt)
+        return sph_fail(ctx, SPH_E_ARG, "sph_hydro_force_improved: NULL array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    return sph_force_launch(ctx, SPH_MODE_IMPROVED, active != nullptr, items, vel, u, h, rho, omega, acc, dudt, vsig_max, alpha, divv,
+                            curlv, ip, dalpha_dt, nullptr, nullptr);
 }
 
 int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *vel_host, const float *u_host,

@@ -26,7 +26,17 @@ struct ForceArgs {
     SphCounters *cnt;
     float L, alpha;
     float *acc, *dudt, *vsig;
+    // improved-SPH extension (MODE_IMPROVED, MODE_GRADV; R17-R20)
+    const float4 *ext;                 // sorted: (alpha, shear limiter f, u, -) per particle
+    float gm1;                         // gamma - 1
+    float alpha_cond, alpha_min, alpha_max, decay_l;
+    float *dalpha;                     // d alpha / dt of the active particles
+    float *divv, *curlv;               // MODE_GRADV outputs
 };
+
+// pair physics of the gather kernel: the base hydro force (R8-R12), the same with the improved-SPH terms
+// (per-particle alpha, shear limiter, artificial conduction: R18-R20), or the velocity-gradient sums (R17)
+enum { MODE_BASE = SPH_MODE_BASE, MODE_IMPROVED = SPH_MODE_IMPROVED, MODE_GRADV = SPH_MODE_GRADV };
 
 // w'(q) for the two arguments of a pair, (r / H_i, r / H_j), in one packed f32x2 chain
 template <int KERNEL>
@@ -63,8 +73,10 @@ struct ForceWarp {
 struct ForceLane {
     float xi, yi, zi, h2, hinv, f4;  // position, H^2, 1/H, sigma/H^4
     float vx, vy, vz, c, rho, A;
+    float al, fb, u, P;     // MODE_IMPROVED: alpha_i, limiter f_i, u_i, P_i
     uint32_t slot;
-    double px, py, pz, pdu; // fp64 accumulators of a and du/dt (R15: "fp64 accumulation where needed")
+    double px, py, pz, pdu; // fp64 accumulators of a and du/dt (R15: "fp64 accumulation where needed");
+                            // MODE_GRADV: of the curl (3) and the divergence sums
     float pvs;
     int cn, cnt;
 };
@@ -78,7 +90,7 @@ struct Frame {
 
 // evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
 // WRAP: 0 raw coordinate differences, 1 recentred frame, 2 per-pair nearest image
-template <int KERNEL, int WRAP>
+template <int KERNEL, int WRAP, int MODE>
 __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
                                       const Frame &fr)
 {
@@ -108,6 +120,18 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             float rinv = rsqrtf(r2c);
             rinv = rinv * fmaf(-0.5f * r2c, rinv * rinv, 1.5f);
             const float r = r2 * rinv;
+            const bool other = j != A.slot; // j == i: no self force, no self signal velocity
+            if (MODE == MODE_GRADV) {
+                // R17: m_j dW/dr(r, H_i) / r times (v_j - v_i) . d and (v_i - v_j) x d
+                const float2 dw = kern_dw2<KERNEL>(make_float2(r * A.hinv, 1.f));
+                const float g = other ? P2.z * A.f4 * dw.x * rinv : 0.f;
+                const float wx = P1.x - A.vx, wy = P1.y - A.vy, wz = P1.z - A.vz;
+                A.pdu += (double)(g * fmaf(wz, dz, fmaf(wy, dy, wx * dx)));
+                A.px -= (double)(g * (wy * dz - wz * dy));
+                A.py -= (double)(g * (wz * dx - wx * dz));
+                A.pz -= (double)(g * (wx * dy - wy * dx));
+                continue;
+            }
             const float hinv_j = P2.w; // 1 / H_j, correctly rounded once per particle (k_force_prep)
             const float hj2 = hinv_j * hinv_j;
             const float2 dw = kern_dw2<KERNEL>(__fmul2_rn(make_float2(r, r), make_float2(A.hinv, hinv_j)));
@@ -117,14 +141,22 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             const float vr = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx)) * rinv;
             const float mu = fminf(vr, 0.f);
             const float vs = A.c + P1.w - 3.f * mu;
-            const float Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
             const float Fbar = 0.5f * (Fi + Fj);
+            float Pi, cond = 0.f;
+            if (MODE == MODE_IMPROVED) {
+                const float4 E = __ldg(a.ext + j);                         // alpha_j, f_j, u_j
+                const float rbi = 2.f / (A.rho + P2.x);                    // 1 / rho_bar
+                Pi = -0.25f * (A.al + E.x) * vs * mu * rbi * 0.5f * (A.fb + E.y);               // R9 with R18, R19
+                const float Pj = a.gm1 * P2.x * E.z;
+                cond = a.alpha_cond * sqrtf(fabsf(A.P - Pj) * rbi) * (A.u - E.z) * Fbar * rbi;   // R20
+            } else {
+                Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
+            }
             const float AiFi = A.A * Fi;
             const float pv = Pi * Fbar;
-            const bool other = j != A.slot; // j == i: no self force, no self signal velocity
             // select, not multiply by zero: a lone particle has Omega = 0, hence A = inf
             const float tr = other ? P2.z * (AiFi + fmaf(P2.y, Fj, pv)) * rinv : 0.f;
-            const float du = other ? P2.z * fmaf(0.5f, pv, AiFi) * vr : 0.f;
+            const float du = other ? P2.z * (fmaf(0.5f, pv, AiFi) * vr + cond) : 0.f;
             A.px -= (double)(tr * dx);
             A.py -= (double)(tr * dy);
             A.pz -= (double)(tr * dz);
@@ -136,18 +168,18 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
     A.cnt = base;
 }
 
-template <int KERNEL>
+template <int KERNEL, int MODE>
 __device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
                                           const Frame &fr)
 {
-    if (fr.pairwrap) drain<KERNEL, 2>(a, qp, A, n, fr);
-    else if (fr.rec) drain<KERNEL, 1>(a, qp, A, n, fr);
-    else drain<KERNEL, 0>(a, qp, A, n, fr);
+    if (fr.pairwrap) drain<KERNEL, 2, MODE>(a, qp, A, n, fr);
+    else if (fr.rec) drain<KERNEL, 1, MODE>(a, qp, A, n, fr);
+    else drain<KERNEL, 0, MODE>(a, qp, A, n, fr);
 }
 
 // Test the candidate pairs of the gathered chunk against this lane's active (symmetric set, R10):
 // hit if r^2 < max(H_i, H_j)^2; a hit pushes the candidate's sorted slot onto the lane's queue.
-template <int KERNEL, bool PAIRWRAP>
+template <int KERNEL, bool PAIRWRAP, int MODE>
 __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,
                                               const uint32_t *__restrict__ gp, uint32_t *__restrict__ qp, ForceLane &A,
                                               int s, int f, bool live, const Frame &fr)
@@ -165,7 +197,7 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
         if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain_any<KERNEL>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
+            drain_any<KERNEL, MODE>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
         }
         const uint32_t q0 = smem_u32(qp);
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
@@ -185,11 +217,12 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
                 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
             }
             const float2 hj2 = make_float2(c1.z, c1.w); // H_j^2 (squared once per candidate by the gather)
-            if (r2.x < fmaxf(A.h2, hj2.x)) {
+            // symmetric set r < max(H_i, H_j) (R10); the velocity gradients gather over the own support only (R17)
+            if (r2.x < (MODE == MODE_GRADV ? A.h2 : fmaxf(A.h2, hj2.x))) {
                 sts_u32(qw, lds_u32(ga));
                 qw += 128u;
             }
-            if (r2.y < fmaxf(A.h2, hj2.y)) {
+            if (r2.y < (MODE == MODE_GRADV ? A.h2 : fmaxf(A.h2, hj2.y))) {
                 sts_u32(qw, lds_u32(ga + 4u));
                 qw += 128u;
             }
@@ -199,8 +232,8 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
     }
 }
 
-template <int KERNEL>
-__global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs a)
+template <int KERNEL, int MODE>
+__global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_FORCE - 1 : SPH_CTAS_FORCE) k_force(ForceArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -239,6 +272,12 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
             A.f4 = kern_sigma<KERNEL>() * h2i * h2i;
             A.vx = p1.x; A.vy = p1.y; A.vz = p1.z; A.c = p1.w;
             A.rho = p2.x; A.A = p2.y;
+            A.al = A.fb = A.u = A.P = 0.f;
+            if (MODE == MODE_IMPROVED) {
+                const float4 e = a.ext[slot];
+                A.al = e.x; A.fb = e.y; A.u = e.z;
+                A.P = a.gm1 * p2.x * e.z;
+            }
             A.px = A.py = A.pz = A.pdu = 0.0;
             A.pvs = 0.f;
             A.cn = A.cnt = 0;
@@ -260,11 +299,11 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
             fr.pairwrap = false;
             fr.rec = false;
             do {
-                walk_batch<true>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
+                walk_batch<MODE != MODE_GRADV>(W.ws, ctl, a.nodes, a.node_hmax, L, gcx, gcy, gcz, ghx, ghy, ghz, hg);
                 cands += ctl.total;
                 // queued hits of an earlier batch are evaluated in the frame they were found in
                 if (ctl.pairwrap != fr.pairwrap || ctl.thx != fr.thx || ctl.thy != fr.thy || ctl.thz != fr.thz) {
-                    drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+                    drain_any<KERNEL, MODE>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
                     fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
                     fr.rec = ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f;
                 }
@@ -276,11 +315,11 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
                     GatherRegs G;
                     gather_load(W.ws, ctl, gc, c, G, a.xyzh);
                     gather_store<true, true>(ctl, G, W.slot, W.gidx, L);
-                    if (fr.pairwrap) consume_chunk<KERNEL, true>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
-                    else consume_chunk<KERNEL, false>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true, MODE>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false, MODE>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
                 }
             } while (ctl.sp > 0);
-            drain_any<KERNEL>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+            drain_any<KERNEL, MODE>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
             // cross-stream totals
             double X = A.px, Y = A.py, Z = A.pz, U = A.pdu;
             float V = A.pvs;
@@ -297,11 +336,23 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
             // a11: scatter to the caller's particle id
             if (lane < g) {
                 const uint32_t id = a.perm[slot];
-                a.acc[3 * (size_t)id] = (float)X;
-                a.acc[3 * (size_t)id + 1] = (float)Y;
-                a.acc[3 * (size_t)id + 2] = (float)Z;
-                a.dudt[id] = (float)U;
-                a.vsig[id] = V;
+                if (MODE == MODE_GRADV) {
+                    const double ir = 1.0 / (double)A.rho;
+                    a.divv[id] = (float)(U * ir);
+                    a.curlv[3 * (size_t)id] = (float)(X * ir);
+                    a.curlv[3 * (size_t)id + 1] = (float)(Y * ir);
+                    a.curlv[3 * (size_t)id + 2] = (float)(Z * ir);
+                } else {
+                    a.acc[3 * (size_t)id] = (float)X;
+                    a.acc[3 * (size_t)id + 1] = (float)Y;
+                    a.acc[3 * (size_t)id + 2] = (float)Z;
+                    a.dudt[id] = (float)U;
+                    a.vsig[id] = V;
+                }
+                if (MODE == MODE_IMPROVED) { // R19: d alpha/dt = -(alpha - alpha_min) 2 l c / H + max(0, -div v)(alpha_max - alpha)
+                    const float dv = a.divv[id];
+                    a.dalpha[id] = -(A.al - a.alpha_min) * 2.f * a.decay_l * A.c * A.hinv + fmaxf(-dv, 0.f) * (a.alpha_max - A.al);
+                }
             }
             unsigned long long pr = (lane < g) ? (unsigned long long)(cn - 1) : 0ull; // minus self
 #pragma unroll
@@ -320,28 +371,41 @@ __global__ void __launch_bounds__(SPH_THREADS, SPH_CTAS_FORCE) k_force(ForceArgs
 __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const float4 *__restrict__ xyzm,
                              const float *__restrict__ vel, const float *__restrict__ u, const float *__restrict__ h,
                              const float *__restrict__ rho, const float *__restrict__ omega, float gamma, float half_box,
-                             float4 *__restrict__ xyzh, float4 *__restrict__ vc, SphCounters *cnt)
+                             float4 *__restrict__ xyzh, float4 *__restrict__ vc, SphCounters *cnt,
+                             const float *__restrict__ alpha, const float *__restrict__ divv, const float *__restrict__ curlv,
+                             int balsara, float4 *__restrict__ ext)
 {
+    // u, omega may be NULL (velocity-gradient pass: only positions, h, velocities, rho and masses are used);
+    // alpha != NULL: improved-SPH state record (alpha, shear limiter f of R18, u) per particle
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     uint32_t id = perm[i];
     float4 p = xyzm[i];
-    float ui = u[id], ri = rho[id];
+    float ui = u ? u[id] : 0.f, ri = rho[id];
     // preconditions on the state of ALL particles (inactive neighbours contribute, R12): 0 < H < box / 2, rho > 0,
     // u >= 0, everything finite (a comparison with NaN is false)
     {
         const float inf = __int_as_float(0x7f800000);
-        const float H = h[id], om = omega[id];
+        const float H = h[id], om = omega ? omega[id] : 1.f;
         const float v2 = fabsf(vel[3 * (int64_t)id]) + fabsf(vel[3 * (int64_t)id + 1]) + fabsf(vel[3 * (int64_t)id + 2]);
         if (!(H > 0.f) || !(H < inf)) atomicOr(&cnt->err, SPH_ERR_H);
         else if (!(H < half_box)) atomicOr(&cnt->err, SPH_ERR_HRANGE);
         if (!(ri > 0.f) || !(ri < inf) || !(ui >= 0.f) || !(ui < inf) || !(fabsf(om) < inf) || !(v2 < inf)) atomicOr(&cnt->err, SPH_ERR_STATE);
     }
     float c = sqrtf(gamma * (gamma - 1.f) * ui);
-    float A = (gamma - 1.f) * ui / (omega[id] * ri); // P/(Omega rho^2), P = (gamma-1) rho u
+    float A = omega ? (gamma - 1.f) * ui / (omega[id] * ri) : 0.f; // P/(Omega rho^2), P = (gamma-1) rho u
     xyzh[i] = make_float4(p.x, p.y, p.z, h[id]);
     vc[2 * i] = make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c);
     vc[2 * i + 1] = make_float4(ri, A, p.w, 1.f / h[id]);
+    if (alpha) {
+        const float inf = __int_as_float(0x7f800000);
+        const float al = alpha[id], dv = divv[id];
+        const float cx = curlv[3 * (int64_t)id], cy = curlv[3 * (int64_t)id + 1], cz = curlv[3 * (int64_t)id + 2];
+        const float cm = sqrtf(fmaf(cz, cz, fmaf(cy, cy, cx * cx)));
+        if (!(al >= 0.f) || !(al < inf) || !(fabsf(dv) < inf) || !(cm < inf)) atomicOr(&cnt->err, SPH_ERR_STATE);
+        const float fb = balsara ? fabsf(dv) / (fabsf(dv) + cm + 1e-4f * c / h[id]) : 1.f; // R18
+        ext[i] = make_float4(al, fb, ui, 0.f);
+    }
 }
 
 // largest support radius inside every octree node: leaves scan their particles, then push the value
@@ -371,11 +435,11 @@ __global__ void k_node_hmax(const SphCounters *cnt, const SphNode *__restrict__ 
     }
 }
 
-template <int KERNEL>
+template <int KERNEL, int MODE>
 int launch(sph_ctx *ctx, const ForceArgs &a, int64_t est_groups)
 {
     size_t dyn = sizeof(ForceWarp) * SPH_WARPS;
-    auto kfn = k_force<KERNEL>;
+    auto kfn = k_force<KERNEL, MODE>;
     SPH_CUDA(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
     int per_sm = 1;
     SPH_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kfn, SPH_THREADS, dyn));
@@ -390,19 +454,30 @@ int launch(sph_ctx *ctx, const ForceArgs &a, int64_t est_groups)
 
 } // namespace
 
-int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
-                     const float *rho, const float *omega, float *acc, float *dudt, float *vsig)
+// mode: MODE_BASE (sph_hydro_force), MODE_IMPROVED (sph_hydro_force_improved), MODE_GRADV (sph_velocity_gradients)
+int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
+                     const float *rho, const float *omega, float *acc, float *dudt, float *vsig, const float *alpha,
+                     const float *divv, const float *curlv, const sph_improved_params *ip, float *dalpha, float *divv_out,
+                     float *curlv_out)
 {
     cudaStream_t st = ctx->stream;
     const int64_t n = ctx->n;
     const int T = 256;
+    if (mode == MODE_IMPROVED && !ctx->f_ext) {
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->f_ext, sizeof(float4) * (size_t)ctx->cap_n));
+    }
     cudaEventRecord(ctx->ev[4], st);
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
-                                                       0.5f * ctx->prm.box, ctx->f_xyzh, ctx->f_vc, ctx->cnt);
-    k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
-    k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
+                                                       0.5f * ctx->prm.box, ctx->f_xyzh, ctx->f_vc, ctx->cnt,
+                                                       mode == MODE_IMPROVED ? alpha : nullptr, divv, curlv,
+                                                       ip ? ip->balsara : 0, ctx->f_ext);
+    ctx->launches++;
+    if (mode != MODE_GRADV) { // the symmetric pair set needs the largest support radius inside every node
+        k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
+        k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
+        ctx->launches += 2;
+    }
     sph_reset_counters(ctx, 1, subset);
-    ctx->launches += 4;
     cudaEventRecord(ctx->ev[5], st);
     ctx->ev_set[2] = true;
 
@@ -419,9 +494,22 @@ int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *ve
     a.L = ctx->prm.box;
     a.alpha = ctx->prm.alpha_visc;
     a.acc = acc; a.dudt = dudt; a.vsig = vsig;
+    a.ext = ctx->f_ext;
+    a.gm1 = ctx->prm.gamma - 1.f;
+    a.alpha_cond = ip ? ip->alpha_cond : 0.f;
+    a.alpha_min = ip ? ip->alpha_min : 0.f;
+    a.alpha_max = ip ? ip->alpha_max : 0.f;
+    a.decay_l = ip ? ip->decay_l : 0.f;
+    a.dalpha = dalpha;
+    a.divv = mode == MODE_GRADV ? divv_out : const_cast<float *>(divv);
+    a.curlv = curlv_out;
     int64_t est_groups = n_items; // (an upper bound: the group count stays on the device)
     cudaEventRecord(ctx->ev[6], st);
-    int rc = ctx->prm.kernel == SPH_KERNEL_CUBIC ? launch<SPH_KERNEL_CUBIC>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6>(ctx, a, est_groups);
+    int rc;
+    const bool cubic = ctx->prm.kernel == SPH_KERNEL_CUBIC;
+    if (mode == MODE_BASE) rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_BASE>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_BASE>(ctx, a, est_groups);
+    else if (mode == MODE_IMPROVED) rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_IMPROVED>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_IMPROVED>(ctx, a, est_groups);
+    else rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_GRADV>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_GRADV>(ctx, a, est_groups);
     cudaEventRecord(ctx->ev[7], st);
     ctx->ev_set[3] = true;
     ctx->launches++;

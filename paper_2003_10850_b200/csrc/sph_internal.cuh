@@ -112,7 +112,7 @@ struct sph_ctx {
     size_t scan_cap;
 
     // force pass (device)
-    float4 *f_xyzh, *f_vc;
+    float4 *f_xyzh, *f_vc, *f_ext; // f_ext: improved-SPH record (alpha, f, u), allocated on first use
     float *node_hmax;
 
     // active subset scratch (device)
@@ -141,6 +141,9 @@ int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
                             "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);    \
     } while (0)
 
+// pair physics of the force gather kernel (sph_force_launch)
+enum { SPH_MODE_BASE = 0, SPH_MODE_IMPROVED = 1, SPH_MODE_GRADV = 2 };
+
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
 // stable LSD radix sort on the low `bits` key bits; *in_alt = 1 if the result ended up in the *_alt buffers
@@ -153,5 +156,7 @@ void sph_reset_counters(sph_ctx *ctx, int which, bool subset); // 0: density, 1:
 int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t n_active);
 int sph_density_launch(sph_ctx *ctx, const int32_t *active, int64_t n_items, float n_target, float n_tol, float *h,
                        float *rho, float *omega, int32_t *ngb, int32_t *status);
-int sph_force_launch(sph_ctx *ctx, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
-                     const float *rho, const float *omega, float *acc, float *dudt, float *vsig);
+int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
+                     const float *rho, const float *omega, float *acc, float *dudt, float *vsig, const float *alpha,
+                     const float *divv, const float *curlv, const sph_improved_params *ip, float *dalpha, float *divv_out,
+                     float *curlv_out);

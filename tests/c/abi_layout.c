@@ -18,6 +18,9 @@ int main(void)
     F(sph_stats, force_candidates); F(sph_stats, force_pairs);
     F(sph_stats, t_index_ms); F(sph_stats, t_density_kernel_ms); F(sph_stats, t_force_prep_ms);
     F(sph_stats, t_force_kernel_ms); F(sph_stats, node_pool_overflow);
+    printf("sph_improved_params %zu\n", sizeof(sph_improved_params));
+    F(sph_improved_params, alpha_min); F(sph_improved_params, alpha_max); F(sph_improved_params, decay_l);
+    F(sph_improved_params, alpha_cond); F(sph_improved_params, balsara);
     printf("status %d %d %d %d %d %d %d %d\n", SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL,
            SPH_E_HRANGE, SPH_W_NOCONV);
     printf("flags %d %d %d %d\n", SPH_ST_CONVERGED, SPH_ST_BRACKET, SPH_ST_NOTCONV, SPH_ST_STALLED);
