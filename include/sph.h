@@ -193,6 +193,18 @@ int sph_hydro_force_improved(sph_ctx *ctx, const int32_t *active, int64_t n_acti
                              float *dalpha_dt);
 
 /*
+ * Thermal conduction: the paper's third module of the same pattern (PAPER.md:27 §1, :41, :102
+ * §2.4, :156 §3.3; no equations given) as a further pair pass over the same index; reading R21.  For every
+ * active particle i, over j != i with r_ij < max(H_i, H_j),
+ *   dudt_cond[id] = sum_j m_j / (rho_i rho_j) * [4 k_i k_j / (k_i + k_j)] * (u_i - u_j) * Fbar_ij / r_ij,
+ *   k = kappa0 * u^kappa_exp   (kappa_exp = 2.5: Spitzer; 0: constant conductivity; T = u up to constants in kappa0).
+ * u [n], h [n], rho [n]: device, valid for all particles; dudt_cond [n] written for active particles only.
+ * Asynchronous; preconditions and error reporting as sph_hydro_force.
+ */
+int sph_thermal_conduction(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *u, const float *h,
+                           const float *rho, float kappa0, float kappa_exp, float *dudt_cond);
+
+/*
  * One whole pass of the hot path with HOST buffers (used for the end-to-end measurement): copies
  * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
  * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries

@@ -615,3 +615,48 @@ int orc_hydro_force_improved(const orc_params *p, const orc_improved *q, int64_t
     }
     return 0;
 }
+
+/* ================================================================ thermal conduction
+ * The paper ports "thermal conduction" as a third module of the same pattern (PAPER.md:27 §1, :41: ~14 % of the
+ * run time, :102 §2.4, :156 §3.3) and gives no equation.  READING R21, the isotropic SPH heat
+ * conduction estimate of the published lineage (second-derivative form of Brookshaw with the harmonic mean of the
+ * conductivities of Cleary & Monaghan, as used for conduction in the Gadget lineage), over the symmetric pair set
+ * r_ij < max(H_i, H_j) of the force pass:
+ *   du_i/dt = sum_j m_j / (rho_i rho_j) * [4 kappa_i kappa_j / (kappa_i + kappa_j)] * (T_i - T_j) * Fbar_ij / r_ij,
+ *   Fbar_ij = (F_ij(H_i) + F_ij(H_j))/2 <= 0,  T = u (the constants of the temperature scale are absorbed in
+ *   kappa_0),  kappa_i = kappa_0 T_i^e  (e = 5/2: Spitzer; e = 0: constant conductivity).
+ * Heat flows from hot to cold; the pair term is antisymmetric in i <-> j (energy is conserved pair by pair).
+ */
+int orc_thermal_conduction(const orc_params *p, int64_t n, const float *pos, const float *u, const float *mass,
+                           double mass_scalar, const float *h, const float *rho, double kappa0, double kappa_exp,
+                           const int32_t *active, int64_t n_active, double *dudt, double *dusum, double *dusq)
+{
+    int64_t na = active ? n_active : n;
+    double L = p->box, sg = k_sigma(p->kernel);
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        double Hi = (double)h[i], Ti = (double)u[i], ki = kappa0 * pow(Ti, kappa_exp);
+        double du = 0.0, s1 = 0.0, s2 = 0.0;
+        for (int64_t j = 0; j < n; j++) { /* plain definition: all j (brute force) */
+            if (j == i) continue;
+            double d[3];
+            for (int k = 0; k < 3; k++) d[k] = min_image((double)pos[3 * i + k] - (double)pos[3 * j + k], L);
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            double Hj = (double)h[j], Hm = Hi > Hj ? Hi : Hj;
+            if (!(r2 < Hm * Hm) || r2 == 0.0) continue;
+            double r = sqrt(r2);
+            double Fi = r < Hi ? sg / (Hi * Hi * Hi * Hi) * k_dw(p->kernel, r / Hi) : 0.0;
+            double Fj = r < Hj ? sg / (Hj * Hj * Hj * Hj) * k_dw(p->kernel, r / Hj) : 0.0;
+            double Tj = (double)u[j], kj = kappa0 * pow(Tj, kappa_exp);
+            double mj = mass ? (double)mass[j] : mass_scalar;
+            double kij = (ki + kj) > 0.0 ? 4.0 * ki * kj / (ki + kj) : 0.0;
+            double e = mj / ((double)rho[i] * (double)rho[j]) * kij * (Ti - Tj) * 0.5 * (Fi + Fj) / r;
+            du += e; s1 += fabs(e); s2 += e * e;
+        }
+        dudt[a] = du;
+        if (dusum) dusum[a] = s1;
+        if (dusq) dusq[a] = s2;
+    }
+    return 0;
+}

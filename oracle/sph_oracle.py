@@ -215,3 +215,21 @@ def hydro_force_improved(pos, vel, u, h, rho, omega, alpha, divv, curlv, *, kern
                                    pom, pal, pdv, pcv, pact, C.c_int64(na),
                                    *[out[k].ctypes.data_as(C.c_void_p) for k in ("acc", "dudt", "vsig", "dalpha", "asum", "dusum", "asq", "dusq", "ducond")])
     return out
+
+
+def thermal_conduction(pos, u, h, rho, *, kernel, kappa0, kappa_exp=2.5, box=1.0, mass=None, mass_scalar=1.0, active=None):
+    """R21: isotropic heat conduction pair sum (brute force over all j). Returns dict dudt, dusum, dusq (fp64, per active)."""
+    pos_, ppos = _p(pos, np.float32)
+    u_, pu = _p(u, np.float32)
+    h_, ph = _p(h, np.float32)
+    rho_, prho = _p(rho, np.float32)
+    m_, pm = _p(mass, np.float32)
+    act_, pact = _p(active, np.int32)
+    n = pos_.shape[0]
+    na = n if act_ is None else act_.shape[0]
+    out = {k: np.zeros(na, np.float64) for k in ("dudt", "dusum", "dusq")}
+    prm = _params(kernel, box, 5.0 / 3.0, 1.0, 0, 64)
+    lib().orc_thermal_conduction(C.byref(prm), C.c_int64(n), ppos, pu, pm, C.c_double(mass_scalar), ph, prho,
+                                 C.c_double(kappa0), C.c_double(kappa_exp), pact, C.c_int64(na),
+                                 *[out[k].ctypes.data_as(C.c_void_p) for k in ("dudt", "dusum", "dusq")])
+    return out

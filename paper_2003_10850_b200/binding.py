@@ -19,7 +19,8 @@ ST_CONVERGED, ST_BRACKET, ST_NOTCONV, ST_STALLED = 1 << 8, 1 << 9, 1 << 10, 1 <<
 KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
-           "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_last_error", "sph_version"]
+           "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_thermal_conduction",
+           "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -71,7 +72,8 @@ def load():
         lib.sph_velocity_gradients.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 5
         lib.sph_hydro_force_improved.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 8 + \
                                                 [C.POINTER(SphImprovedParams)] + [C.c_void_p] * 4
-        for name in EXPORTS[:9]:
+        lib.sph_thermal_conduction.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 3 + [C.c_float, C.c_float, C.c_void_p]
+        for name in EXPORTS[:10]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -179,6 +181,15 @@ class Sph:
             _dev(h, f32, "h", n), _dev(rho, f32, "rho", n), _dev(omega, f32, "omega", n), _dev(alpha, f32, "alpha", n),
             _dev(divv, f32, "divv", n), _dev(curlv, f32, "curlv", 3 * n), C.byref(ip), _dev(acc, f32, "acc", 3 * n),
             _dev(dudt, f32, "dudt", n), _dev(vsig_max, f32, "vsig_max", n), _dev(dalpha_dt, f32, "dalpha_dt", n)))
+
+    def sph_thermal_conduction(self, u, h, rho, dudt_cond, kappa0, kappa_exp=2.5, active=None):
+        """R21: isotropic heat conduction as a further pair pass over the index."""
+        n = self.n
+        na = -1 if active is None else active.numel()
+        f32 = torch.float32
+        self._check(self._lib.sph_thermal_conduction(self._h, _dev(active, torch.int32, "active"), na, _dev(u, f32, "u", n),
+                                                     _dev(h, f32, "h", n), _dev(rho, f32, "rho", n), float(kappa0), float(kappa_exp),
+                                                     _dev(dudt_cond, f32, "dudt_cond", n)))
 
     def sph_step_host(self, pos, vel, u, mass_scalar, h, rho, omega, ngb_count, acc, dudt, vsig, n_ngb_target,
                       n_ngb_tol, active=None):

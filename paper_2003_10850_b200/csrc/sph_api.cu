@@ -207,6 +207,25 @@ int sph_velocity_gradients(sph_ctx *ctx, const int32_t *active, int64_t n_active
                             nullptr, nullptr, nullptr, nullptr, nullptr, divv, curlv);
 }
 
+int sph_thermal_conduction(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *u, const float *h,
+                           const float *rho, float kappa0, float kappa_exp, float *dudt_cond)
+{
+    if (!ctx) return SPH_E_ARG;
+    Range nv("sph_thermal_conduction");
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_thermal_conduction before sph_build_index");
+    if (!(kappa0 >= 0.f) || !(kappa_exp >= 0.f)) return sph_fail(ctx, SPH_E_ARG, "sph_thermal_conduction: bad kappa0 / kappa_exp");
+    const bool subset = active != nullptr || n_active == 0;
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_thermal_conduction: n_active < 0");
+    int64_t items = subset ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!u || !h || !rho || !dudt_cond) return sph_fail(ctx, SPH_E_ARG, "sph_thermal_conduction: NULL array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    return sph_force_launch(ctx, SPH_MODE_CONDUCT, active != nullptr, items, nullptr, u, h, rho, nullptr, nullptr, dudt_cond, nullptr,
+                            nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, kappa0, kappa_exp);
+}
+
 int sph_hydro_force_improved(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *vel, const float *u,
                              const float *h, const float *rho, const float *omega, const float *alpha, const float *divv,
                              const float *curlv, const sph_improved_params *ip, float *acc, float *dudt, float *vsig_max,

@@ -27,7 +27,7 @@ struct ForceArgs {
     float L, alpha;
     float *acc, *dudt, *vsig;
     // improved-SPH extension (MODE_IMPROVED, MODE_GRADV; R17-R20)
-    const float4 *ext;                 // sorted: (alpha, shear limiter f, u, -) per particle
+    const float4 *ext;                 // sorted: (alpha, shear limiter f, u, -) per particle; MODE_CONDUCT: (kappa, T = u, -, -)
     float gm1;                         // gamma - 1
     float alpha_cond, alpha_min, alpha_max, decay_l;
     float *dalpha;                     // d alpha / dt of the active particles
@@ -35,8 +35,9 @@ struct ForceArgs {
 };
 
 // pair physics of the gather kernel: the base hydro force (R8-R12), the same with the improved-SPH terms
-// (per-particle alpha, shear limiter, artificial conduction: R18-R20), or the velocity-gradient sums (R17)
-enum { MODE_BASE = SPH_MODE_BASE, MODE_IMPROVED = SPH_MODE_IMPROVED, MODE_GRADV = SPH_MODE_GRADV };
+// (per-particle alpha, shear limiter, artificial conduction: R18-R20), the velocity-gradient sums (R17), or the
+// thermal-conduction pair sum (R21)
+enum { MODE_BASE = SPH_MODE_BASE, MODE_IMPROVED = SPH_MODE_IMPROVED, MODE_GRADV = SPH_MODE_GRADV, MODE_CONDUCT = SPH_MODE_CONDUCT };
 
 // w'(q) for the two arguments of a pair, (r / H_i, r / H_j), in one packed f32x2 chain
 template <int KERNEL>
@@ -142,6 +143,15 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             const float mu = fminf(vr, 0.f);
             const float vs = A.c + P1.w - 3.f * mu;
             const float Fbar = 0.5f * (Fi + Fj);
+            if (MODE == MODE_CONDUCT) {
+                // R21: m_j / (rho_i rho_j) * 4 k_i k_j / (k_i + k_j) * (T_i - T_j) * Fbar / r
+                const float4 E = __ldg(a.ext + j); // kappa_j, T_j
+                const float ks = A.al + E.x;
+                const float kij = ks > 0.f ? 4.f * A.al * E.x / ks : 0.f;
+                const float e = other ? P2.z / (A.rho * P2.x) * kij * (A.u - E.y) * Fbar * rinv : 0.f;
+                A.pdu += (double)e;
+                continue;
+            }
             float Pi, cond = 0.f;
             if (MODE == MODE_IMPROVED) {
                 const float4 E = __ldg(a.ext + j);                         // alpha_j, f_j, u_j
@@ -278,6 +288,10 @@ __global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_
                 A.al = e.x; A.fb = e.y; A.u = e.z;
                 A.P = a.gm1 * p2.x * e.z;
             }
+            if (MODE == MODE_CONDUCT) {
+                const float4 e = a.ext[slot];
+                A.al = e.x; A.u = e.y; // kappa_i, T_i
+            }
             A.px = A.py = A.pz = A.pdu = 0.0;
             A.pvs = 0.f;
             A.cn = A.cnt = 0;
@@ -342,6 +356,8 @@ __global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_
                     a.curlv[3 * (size_t)id] = (float)(X * ir);
                     a.curlv[3 * (size_t)id + 1] = (float)(Y * ir);
                     a.curlv[3 * (size_t)id + 2] = (float)(Z * ir);
+                } else if (MODE == MODE_CONDUCT) {
+                    a.dudt[id] = (float)U;
                 } else {
                     a.acc[3 * (size_t)id] = (float)X;
                     a.acc[3 * (size_t)id + 1] = (float)Y;
@@ -373,7 +389,7 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
                              const float *__restrict__ rho, const float *__restrict__ omega, float gamma, float half_box,
                              float4 *__restrict__ xyzh, float4 *__restrict__ vc, SphCounters *cnt,
                              const float *__restrict__ alpha, const float *__restrict__ divv, const float *__restrict__ curlv,
-                             int balsara, float4 *__restrict__ ext)
+                             int balsara, float4 *__restrict__ ext, float kappa0, float kappa_exp, int conduct)
 {
     // u, omega may be NULL (velocity-gradient pass: only positions, h, velocities, rho and masses are used);
     // alpha != NULL: improved-SPH state record (alpha, shear limiter f of R18, u) per particle
@@ -387,7 +403,7 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
     {
         const float inf = __int_as_float(0x7f800000);
         const float H = h[id], om = omega ? omega[id] : 1.f;
-        const float v2 = fabsf(vel[3 * (int64_t)id]) + fabsf(vel[3 * (int64_t)id + 1]) + fabsf(vel[3 * (int64_t)id + 2]);
+        const float v2 = vel ? fabsf(vel[3 * (int64_t)id]) + fabsf(vel[3 * (int64_t)id + 1]) + fabsf(vel[3 * (int64_t)id + 2]) : 0.f;
         if (!(H > 0.f) || !(H < inf)) atomicOr(&cnt->err, SPH_ERR_H);
         else if (!(H < half_box)) atomicOr(&cnt->err, SPH_ERR_HRANGE);
         if (!(ri > 0.f) || !(ri < inf) || !(ui >= 0.f) || !(ui < inf) || !(fabsf(om) < inf) || !(v2 < inf)) atomicOr(&cnt->err, SPH_ERR_STATE);
@@ -395,7 +411,8 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
     float c = sqrtf(gamma * (gamma - 1.f) * ui);
     float A = omega ? (gamma - 1.f) * ui / (omega[id] * ri) : 0.f; // P/(Omega rho^2), P = (gamma-1) rho u
     xyzh[i] = make_float4(p.x, p.y, p.z, h[id]);
-    vc[2 * i] = make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c);
+    vc[2 * i] = vel ? make_float4(vel[3 * (int64_t)id], vel[3 * (int64_t)id + 1], vel[3 * (int64_t)id + 2], c) : make_float4(0.f, 0.f, 0.f, c);
+    if (conduct) ext[i] = make_float4(kappa0 * powf(ui, kappa_exp), ui, 0.f, 0.f); // R21: kappa = kappa_0 T^e, T = u
     vc[2 * i + 1] = make_float4(ri, A, p.w, 1.f / h[id]);
     if (alpha) {
         const float inf = __int_as_float(0x7f800000);
@@ -458,19 +475,19 @@ int launch(sph_ctx *ctx, const ForceArgs &a, int64_t est_groups)
 int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
                      const float *rho, const float *omega, float *acc, float *dudt, float *vsig, const float *alpha,
                      const float *divv, const float *curlv, const sph_improved_params *ip, float *dalpha, float *divv_out,
-                     float *curlv_out)
+                     float *curlv_out, float kappa0, float kappa_exp)
 {
     cudaStream_t st = ctx->stream;
     const int64_t n = ctx->n;
     const int T = 256;
-    if (mode == MODE_IMPROVED && !ctx->f_ext) {
+    if ((mode == MODE_IMPROVED || mode == MODE_CONDUCT) && !ctx->f_ext) {
         SPH_CUDA(ctx, cudaMalloc((void **)&ctx->f_ext, sizeof(float4) * (size_t)ctx->cap_n));
     }
     cudaEventRecord(ctx->ev[4], st);
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
                                                        0.5f * ctx->prm.box, ctx->f_xyzh, ctx->f_vc, ctx->cnt,
                                                        mode == MODE_IMPROVED ? alpha : nullptr, divv, curlv,
-                                                       ip ? ip->balsara : 0, ctx->f_ext);
+                                                       ip ? ip->balsara : 0, ctx->f_ext, kappa0, kappa_exp, mode == MODE_CONDUCT);
     ctx->launches++;
     if (mode != MODE_GRADV) { // the symmetric pair set needs the largest support radius inside every node
         k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
@@ -509,7 +526,8 @@ int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const
     const bool cubic = ctx->prm.kernel == SPH_KERNEL_CUBIC;
     if (mode == MODE_BASE) rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_BASE>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_BASE>(ctx, a, est_groups);
     else if (mode == MODE_IMPROVED) rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_IMPROVED>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_IMPROVED>(ctx, a, est_groups);
-    else rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_GRADV>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_GRADV>(ctx, a, est_groups);
+    else if (mode == MODE_GRADV) rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_GRADV>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_GRADV>(ctx, a, est_groups);
+    else rc = cubic ? launch<SPH_KERNEL_CUBIC, MODE_CONDUCT>(ctx, a, est_groups) : launch<SPH_KERNEL_WC6, MODE_CONDUCT>(ctx, a, est_groups);
     cudaEventRecord(ctx->ev[7], st);
     ctx->ev_set[3] = true;
     ctx->launches++;

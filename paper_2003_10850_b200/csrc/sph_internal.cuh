@@ -142,7 +142,7 @@ int sph_fail(sph_ctx *ctx, int code, const char *fmt, ...);
     } while (0)
 
 // pair physics of the force gather kernel (sph_force_launch)
-enum { SPH_MODE_BASE = 0, SPH_MODE_IMPROVED = 1, SPH_MODE_GRADV = 2 };
+enum { SPH_MODE_BASE = 0, SPH_MODE_IMPROVED = 1, SPH_MODE_GRADV = 2, SPH_MODE_CONDUCT = 3 };
 
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
@@ -159,4 +159,4 @@ int sph_density_launch(sph_ctx *ctx, const int32_t *active, int64_t n_items, flo
 int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const float *vel, const float *u, const float *h,
                      const float *rho, const float *omega, float *acc, float *dudt, float *vsig, const float *alpha,
                      const float *divv, const float *curlv, const sph_improved_params *ip, float *dalpha, float *divv_out,
-                     float *curlv_out);
+                     float *curlv_out, float kappa0 = 0.f, float kappa_exp = 0.f);

@@ -78,3 +78,34 @@ def test_improved_sph_against_the_oracle(shape):
     assert np.array_equal(vs.cpu().numpy(), base["vsig"])
     print(shape, "improved: acc err/tol", float(np.max(err_a / tol_a)), "dudt err/tol", float(np.max(err_d / tol_d)))
     g.close()
+
+
+@pytest.mark.parametrize("shape,kexp", [("C2", 2.5), ("C4", 2.5), ("C2", 0.0)])
+def test_thermal_conduction_against_the_oracle(shape, kexp):
+    """the conduction pair pass on the GPU against the oracle's brute-force sum."""
+    ps = I.config2(20) if shape == "C2" else I.config4(24000, 6, m_lo=320, m_hi=8000)
+    H, rho, om = _state(ps)
+    n = ps.n
+    rng = np.random.default_rng(6)
+    sample = np.sort(rng.choice(n, 1500, replace=False)).astype(np.int32)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    f32 = torch.float32
+    out = torch.full((n,), 7.0, device="cuda")
+    g.sph.sph_thermal_conduction(dev(ps.u, f32), dev(H, f32), dev(rho, f32), out, 0.8, kexp)
+    torch.cuda.synchronize()
+    o = O.thermal_conduction(ps.pos, ps.u, H, rho, kernel=ps.kernel, kappa0=0.8, kappa_exp=kexp, mass_scalar=ps.mass, active=sample)
+    gd = out.cpu().numpy().astype(np.float64)
+    tol = RTOL_FORCE * np.maximum(np.abs(o["dudt"]), FLOOR * o["dusum"]) + ULPS * 2.0 ** -24 * np.sqrt(o["dusq"])
+    err = np.abs(gd[sample] - o["dudt"])
+    assert np.all(err <= tol), float(np.max(err / tol))
+    # energy: all particles active, equal masses -> sum du/dt = 0 to rounding
+    assert abs(gd.sum()) < 1e-5 * np.abs(gd).sum()
+    # active subset: only those entries are written
+    out2 = torch.full((n,), 7.0, device="cuda")
+    g.sph.sph_thermal_conduction(dev(ps.u, f32), dev(H, f32), dev(rho, f32), out2, 0.8, kexp, active=dev(sample, torch.int32))
+    torch.cuda.synchronize()
+    o2 = out2.cpu().numpy()
+    inact = np.ones(n, bool); inact[sample] = False
+    assert np.array_equal(o2[sample], out.cpu().numpy()[sample]) and np.all(o2[inact] == 7.0)
+    print(shape, kexp, "conduction err/tol", float(np.max(err / tol)))
+    g.close()

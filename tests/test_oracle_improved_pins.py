@@ -147,3 +147,40 @@ def test_improved_force_conserves_momentum_and_energy(k):
     one = np.ones(n, np.float32)
     s = O.hydro_force_improved(pos, vel0, us, np.full(n, 0.2, np.float32), one, one, al, dv, cv, kernel=k, mass_scalar=m)
     assert np.all(s["ducond"][us > 1.5] <= 0) and np.all(s["ducond"][us < 1.5] >= 0) and s["ducond"].min() < 0
+
+
+# ------------------------------------------------------------------ thermal conduction (R21)
+def test_thermal_conduction_closed_forms_on_a_lattice():
+    """R21 with a constant conductivity on a cubic lattice (rho = 1): a uniform temperature conducts nothing, a linear
+    one neither (inversion symmetry: exactly), and T = x^2 gives du/dt = kappa lap(T) / rho = 2 kappa times the SAME
+    isotropy factor t of the lattice that the velocity-gradient estimator has (R17 pin) -- two routines, one number.
+    (16^3 lattice: coordinates, T and the velocities are dyadic rationals, exact in fp32.)"""
+    pos, H, rho, act = _lattice(16)
+    n = len(pos)
+    m = 1.0 / n
+    x = pos[:, 0].astype(np.float64) - 0.5
+    kw = dict(kernel=1, kappa0=0.3, kappa_exp=0.0, mass_scalar=m, active=act)
+    assert np.all(O.thermal_conduction(pos, np.full(n, 1.7, np.float32), H, rho, **kw)["dudt"] == 0.0)
+    lin = O.thermal_conduction(pos, (2.0 + 0.5 * x).astype(np.float32), H, rho, **kw)
+    assert np.max(np.abs(lin["dudt"])) < 1e-13 * lin["dusum"].max()
+    quad = O.thermal_conduction(pos, (1.0 + x * x).astype(np.float32), H, rho, **kw)
+    A = np.diag([1.0, 2.0, -0.5])
+    t = O.velocity_gradients(pos, ((pos.astype(np.float64) - 0.5) @ A.T).astype(np.float32), H, rho, kernel=1, mass_scalar=m,
+                             active=act)["divv"] / np.trace(A)
+    assert np.max(np.abs(quad["dudt"] / (2 * 0.3) - t)) < 1e-7 and abs(t.mean() - 1) < 0.01  # (kappa0 = 0.3 is not dyadic)
+
+
+def test_thermal_conduction_two_particles_and_conservation():
+    r, h1, h2 = 0.1, 0.25, 0.2
+    pos, vel, u, H = I.two_particles(r, h1, h2, u1=2.0, u2=0.5)
+    rho = np.array([1.2, 0.9], np.float32)
+    m, k0 = 0.3, 0.7
+    o = O.thermal_conduction(pos, u, H, rho, kernel=1, kappa0=k0, kappa_exp=2.5, mass_scalar=m)
+    rr = float(pos[1, 0]) - float(pos[0, 0])
+    k = [k0 * 2.0 ** 2.5, k0 * 0.5 ** 2.5]
+    Fb = 0.5 * (O.dWdr(1, rr, float(H[0])) + O.dWdr(1, rr, float(H[1])))
+    e0 = m / (float(rho[0]) * float(rho[1])) * 4 * k[0] * k[1] / (k[0] + k[1]) * (2.0 - 0.5) * Fb / rr
+    assert e0 < 0 and abs(o["dudt"][0] - e0) < 1e-12 * abs(e0) and abs(o["dudt"][1] + e0) < 1e-12 * abs(e0)  # hot cools, cold heats
+    pos, vel, u, H, rho, om, m = _random_state(500, 4)
+    o = O.thermal_conduction(pos, u, H, rho, kernel=0, kappa0=1.0, mass_scalar=m)
+    assert abs(o["dudt"].sum()) < 1e-12 * o["dusum"].sum() and o["dusum"].sum() > 0  # equal masses: sum m du/dt = 0
