@@ -43,10 +43,12 @@ def test_improved_sph_against_the_oracle(shape):
     scale = np.abs(ps.vel).max() * 3.0 / H[sample]
     assert np.max(np.abs(dv[sample] - og["divv"]) / np.maximum(np.abs(og["divv"]), 1e-3 * scale)) < 1e-4
     assert np.max(np.abs(cv[sample] - og["curlv"]).max(1) / np.maximum(np.abs(og["curlv"]).max(1), 1e-3 * scale)) < 1e-4
-    # the subset call writes the active entries only, with the same values
+    # the subset call writes the active entries only, with the same values (other groups, hence another summation order)
     dv2, cv2 = _gradients(g, ps, H, rho, active=sample)
     inact = np.ones(n, bool); inact[sample] = False
-    assert np.array_equal(dv2[sample], dv[sample]) and np.array_equal(cv2[sample], cv[sample]) and np.all(dv2[inact] == 9.0)
+    tiny = 1e-5 * np.abs(dv).max()
+    assert np.allclose(dv2[sample], dv[sample], rtol=1e-4, atol=tiny) and np.allclose(cv2[sample], cv[sample], rtol=1e-4, atol=tiny)
+    assert np.all(dv2[inact] == 9.0) and np.all(cv2[inact] == 9.0)
     # R18-R20: the force pass with the GPU's own gradients as the common input of both sides
     alpha = rng.uniform(0.02, 3.0, n).astype(np.float32)
     kw = dict(alpha_min=0.02, alpha_max=3.0, decay_l=4.0, alpha_cond=0.25, balsara=True)
@@ -106,6 +108,7 @@ def test_thermal_conduction_against_the_oracle(shape, kexp):
     torch.cuda.synchronize()
     o2 = out2.cpu().numpy()
     inact = np.ones(n, bool); inact[sample] = False
-    assert np.array_equal(o2[sample], out.cpu().numpy()[sample]) and np.all(o2[inact] == 7.0)
+    o1 = out.cpu().numpy()
+    assert np.allclose(o2[sample], o1[sample], rtol=1e-4, atol=1e-5 * np.abs(o1).max()) and np.all(o2[inact] == 7.0)
     print(shape, kexp, "conduction err/tol", float(np.max(err / tol)))
     g.close()
