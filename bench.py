@@ -238,6 +238,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extension", action="store_true", help="skip the improved-SPH extension timing")
+    ap.add_argument("--kdk-steps", type=int, default=0,
+                    help="after the timed region, run this many steps of the kick-drift-kick driver (SURVEY.md 8(f)-3) on the "
+                         "workload and report active counts and times per step")
     ap.add_argument("--group-cap", type=int, default=0, help="actives per group (0 = library default)")
     ap.add_argument("--group-node", type=int, default=0, help="group-node capacity (0 = library default)")
     args = ap.parse_args()
@@ -355,6 +358,32 @@ def main():
     ms = max_over_ranks(ms, world, "cuda")
     value = whole_job_value(world, n_active, args.steps, ms)
 
+    kdk = None
+    if args.kdk_steps > 0:
+        # the time-bin driver on this set: real active lists step after step; dt_max = 4 x the median
+        # Courant step so that several bins are occupied
+        vs0 = float(torch.median(vs).item()) if float(vs.max().item()) > 0 else 1.0
+        dt_med = 0.3 * float(torch.median(h).item()) / max(vs0, 1e-30)
+        stt_ = dict(pos=pos.clone(), vel=vel.clone(), u=u.clone(), h=h.clone(), rho=rho.clone(), omega=om.clone(), ngb=ngb.clone(),
+                    acc=torch.zeros((n, 3), device="cuda"), dudt=torch.zeros(n, device="cuda"), vsig=torch.zeros(n, device="cuda"),
+                    vpred=torch.zeros((n, 3), device="cuda"), upred=torch.zeros(n, device="cuda"),
+                    bin=torch.zeros(n, device="cuda", dtype=torch.int32), tbegin=torch.zeros(n, device="cuda", dtype=torch.int32),
+                    active=torch.zeros(n, device="cuda", dtype=torch.int32))
+        sph.sph_kdk_init(stt_, ps.mass, 4.0 * dt_med, 12, ps.n_ngb, ps.n_tol)
+        torch.cuda.synchronize()
+        rows = []
+        for _ in range(args.kdk_steps):
+            k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            k0.record(stream)
+            tick, na = sph.sph_kdk_step(stt_, ps.mass)
+            k1.record(stream)
+            torch.cuda.synchronize()
+            rows.append((tick, na, k0.elapsed_time(k1)))
+        tot_a, tot_ms = sum(r[1] for r in rows), sum(r[2] for r in rows)
+        kdk = {"steps": len(rows), "dt_max": 4.0 * dt_med, "n_bins": 12, "active_per_step": [r[1] for r in rows],
+               "ms_per_step": [round(r[2], 3) for r in rows], "updates_per_s": tot_a / (tot_ms * 1e-3),
+               "bins_occupied": sorted(set(torch.unique(stt_["bin"]).cpu().tolist()))}
+
     # e2e: the same step through sph_step_host, pinned host buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -436,7 +465,7 @@ def main():
             "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
             "e2e": e2e, "gpu_launches": int(launches), "roofline": roof,
             "phases_ms": {"index": ti, "density_kernel": tk, "force_prep": tp, "force_kernel": tf},
-            "improved_sph_extension_ms": ext_ms,
+            "improved_sph_extension_ms": ext_ms, "kdk_driver": kdk,
             "pairs": {"density_evals_per_particle": st["dens_evals"] / n_active,
                       "density_true_pairs": st["dens_pairs"], "density_candidates": st["dens_candidates"],
                       "force_true_pairs": st["force_pairs"], "force_candidates": st["force_candidates"],

@@ -205,6 +205,46 @@ int sph_thermal_conduction(sph_ctx *ctx, const int32_t *active, int64_t n_active
                            const float *rho, float kappa0, float kappa_exp, float *dudt_cond);
 
 /*
+ * Kick-drift-kick time integration with power-of-two time bins (SURVEY.md §8(f)-3; PAPER.md:37 §1, :84-86 §2.2, :114
+ * §3: the scheme that produces the paper's active lists, down to "one or very few" particles per step; no formulas in
+ * the paper: DESIGN.md reading R22).  Timeline of T = 2^(n_bins-1) ticks per dt_max; a particle of bin b steps
+ * dt_max / 2^b.  Time-step criterion dt_i = min(courant * H_i / vsig_i, sqrt(2 eta H_i / |a_i|)), bin = smallest b with
+ * dt_max / 2^b <= dt_i; a particle may move to a longer step one bin at a time and only where the timeline is aligned.
+ *   sph_kdk_init: tick 0 -- index, density and force for all particles, bins, first half kick (vel, u become
+ *                 kick-centred).  h is the guess on entry.
+ *   sph_kdk_step: advance to the next tick at which a step ends; drift ALL particles there (pos, periodic wrap;
+ *                 vpred, upred = velocity and energy extrapolated to that time with the stored acc, dudt); the
+ *                 particles whose step ends are active: sph_build_index, sph_density (last h as the guess),
+ *                 sph_hydro_force (with vpred, upred) on them; second half kick, new bin, first half kick.
+ *                 *tick_host = the new tick, *n_active_host = number of active particles (their ids, ascending,
+ *                 are left in state->active).  Synchronises.
+ * All arrays of sph_kdk_state are DEVICE arrays owned by the caller.
+ */
+typedef struct {
+    float dt_max;       /* length of the longest step (bin 0) */
+    int n_bins;         /* 1..24 */
+    float courant;      /* 0.3 */
+    float eta;          /* 0.025 */
+    float n_ngb_target, n_ngb_tol;
+} sph_kdk_params;
+
+typedef struct {
+    float *pos;         /* n*3 */
+    float *vel;         /* n*3, kick-centred after sph_kdk_init */
+    float *u, *h, *rho, *omega; /* n each */
+    int32_t *ngb;       /* n */
+    float *acc;         /* n*3 */
+    float *dudt, *vsig; /* n each */
+    float *vpred;       /* n*3 */
+    float *upred;       /* n */
+    int32_t *bin, *tbegin, *active; /* n each: time bin, tick at which the current step began, active list */
+} sph_kdk_state;
+
+int sph_kdk_init(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_params *p, const sph_kdk_state *state);
+int sph_kdk_step(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_params *p, const sph_kdk_state *state,
+                 int64_t *tick_host, int64_t *n_active_host);
+
+/*
  * One whole pass of the hot path with HOST buffers (used for the end-to-end measurement): copies
  * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
  * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries

@@ -20,7 +20,7 @@ KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
            "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_thermal_conduction",
-           "sph_last_error", "sph_version"]
+           "sph_kdk_init", "sph_kdk_step", "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -38,6 +38,20 @@ class SphStats(C.Structure):
 class SphImprovedParams(C.Structure):
     _fields_ = [("alpha_min", C.c_float), ("alpha_max", C.c_float), ("decay_l", C.c_float), ("alpha_cond", C.c_float),
                 ("balsara", C.c_int)]
+
+
+class SphKdkParams(C.Structure):
+    _fields_ = [("dt_max", C.c_float), ("n_bins", C.c_int), ("courant", C.c_float), ("eta", C.c_float),
+                ("n_ngb_target", C.c_float), ("n_ngb_tol", C.c_float)]
+
+
+KDK_F32 = ("pos", "vel", "u", "h", "rho", "omega")
+KDK_FIELDS = (("pos", 3), ("vel", 3), ("u", 1), ("h", 1), ("rho", 1), ("omega", 1), ("ngb", 1), ("acc", 3), ("dudt", 1), ("vsig", 1),
+              ("vpred", 3), ("upred", 1), ("bin", 1), ("tbegin", 1), ("active", 1))
+
+
+class SphKdkState(C.Structure):
+    _fields_ = [(k, C.c_void_p) for k, _ in KDK_FIELDS]
 
 
 class SphError(RuntimeError):
@@ -73,7 +87,10 @@ def load():
         lib.sph_hydro_force_improved.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 8 + \
                                                 [C.POINTER(SphImprovedParams)] + [C.c_void_p] * 4
         lib.sph_thermal_conduction.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 3 + [C.c_float, C.c_float, C.c_void_p]
-        for name in EXPORTS[:10]:
+        lib.sph_kdk_init.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.POINTER(SphKdkParams), C.POINTER(SphKdkState)]
+        lib.sph_kdk_step.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.POINTER(SphKdkParams), C.POINTER(SphKdkState),
+                                     C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+        for name in EXPORTS[:12]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -190,6 +207,31 @@ class Sph:
         self._check(self._lib.sph_thermal_conduction(self._h, _dev(active, torch.int32, "active"), na, _dev(u, f32, "u", n),
                                                      _dev(h, f32, "h", n), _dev(rho, f32, "rho", n), float(kappa0), float(kappa_exp),
                                                      _dev(dudt_cond, f32, "dudt_cond", n)))
+
+    # -- kick-drift-kick driver with power-of-two time bins (R22) ---------------------------
+    @staticmethod
+    def _kdk_state(state: dict, n: int) -> "SphKdkState":
+        st = SphKdkState()
+        for k, w in KDK_FIELDS:
+            dt = torch.int32 if k in ("ngb", "bin", "tbegin", "active") else torch.float32
+            setattr(st, k, _dev(state[k], dt, k, w * n))
+        return st
+
+    def sph_kdk_init(self, state: dict, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025):
+        n = state["pos"].shape[0]
+        self._kdk_p = SphKdkParams(dt_max, n_bins, courant, eta, n_ngb_target, n_ngb_tol)
+        st = self._kdk_state(state, n)
+        self._check(self._lib.sph_kdk_init(self._h, n, float(mass_scalar), C.byref(self._kdk_p), C.byref(st)), allow=(SPH_OK, SPH_W_NOCONV))
+        self.n = n
+
+    def sph_kdk_step(self, state: dict, mass_scalar):
+        """One step of the driver; returns (tick, n_active)."""
+        n = state["pos"].shape[0]
+        st = self._kdk_state(state, n)
+        tick, na = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.sph_kdk_step(self._h, n, float(mass_scalar), C.byref(self._kdk_p), C.byref(st), C.byref(tick), C.byref(na)),
+                    allow=(SPH_OK, SPH_W_NOCONV))
+        return int(tick.value), int(na.value)
 
     def sph_step_host(self, pos, vel, u, mass_scalar, h, rho, omega, ngb_count, acc, dudt, vsig, n_ngb_target,
                       n_ngb_tol, active=None):

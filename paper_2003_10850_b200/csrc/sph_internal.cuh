@@ -125,6 +125,7 @@ struct sph_ctx {
     int32_t *d_ngb, *d_active;
 
     int64_t launches;
+    int64_t kdk_tick;  // sph_kdk_*: current tick of the integer timeline
 
     // phase timing: events recorded on the stream around the phases named in sph_stats
     cudaEvent_t ev[8]; // 0,1 index  2,3 density kernel  4,5 force prep  6,7 force kernel

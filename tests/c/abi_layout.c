@@ -21,6 +21,13 @@ int main(void)
     printf("sph_improved_params %zu\n", sizeof(sph_improved_params));
     F(sph_improved_params, alpha_min); F(sph_improved_params, alpha_max); F(sph_improved_params, decay_l);
     F(sph_improved_params, alpha_cond); F(sph_improved_params, balsara);
+    printf("sph_kdk_params %zu\n", sizeof(sph_kdk_params));
+    F(sph_kdk_params, dt_max); F(sph_kdk_params, n_bins); F(sph_kdk_params, courant); F(sph_kdk_params, eta);
+    F(sph_kdk_params, n_ngb_target); F(sph_kdk_params, n_ngb_tol);
+    printf("sph_kdk_state %zu\n", sizeof(sph_kdk_state));
+    F(sph_kdk_state, pos); F(sph_kdk_state, vel); F(sph_kdk_state, u); F(sph_kdk_state, h); F(sph_kdk_state, rho);
+    F(sph_kdk_state, omega); F(sph_kdk_state, ngb); F(sph_kdk_state, acc); F(sph_kdk_state, dudt); F(sph_kdk_state, vsig);
+    F(sph_kdk_state, vpred); F(sph_kdk_state, upred); F(sph_kdk_state, bin); F(sph_kdk_state, tbegin); F(sph_kdk_state, active);
     printf("status %d %d %d %d %d %d %d %d\n", SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL,
            SPH_E_HRANGE, SPH_W_NOCONV);
     printf("flags %d %d %d %d\n", SPH_ST_CONVERGED, SPH_ST_BRACKET, SPH_ST_NOTCONV, SPH_ST_STALLED);

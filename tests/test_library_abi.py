@@ -44,7 +44,8 @@ def test_struct_layout_matches_the_c_header(tmp_path):
     subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-o", exe, os.path.join(ROOT, "tests", "c", "abi_layout.c"),
                            "-I", os.path.join(ROOT, "include")])
     out = dict(l.split(None, 1) for l in subprocess.check_output([exe], text=True).splitlines())
-    for name, cls in (("sph_params", B.SphParams), ("sph_stats", B.SphStats), ("sph_improved_params", B.SphImprovedParams)):
+    for name, cls in (("sph_params", B.SphParams), ("sph_stats", B.SphStats), ("sph_improved_params", B.SphImprovedParams),
+                      ("sph_kdk_params", B.SphKdkParams), ("sph_kdk_state", B.SphKdkState)):
         assert int(out[name]) == ctypes.sizeof(cls)
         fields = [f for f, _ in cls._fields_]
         assert sorted(k.split(".")[1] for k in out if k.startswith(name + ".")) == sorted(fields)
