@@ -660,3 +660,42 @@ int orc_thermal_conduction(const orc_params *p, int64_t n, const float *pos, con
     }
     return 0;
 }
+
+/* ================================================================ short-range gravity
+ * The paper's gravity is "Barnes-Hut + Particle-Mesh" (§1), i.e. a TreePM split: the tree walk
+ * computes the SHORT-range part (PAPER.md:41 ~15 % of the time, :102-104 §2.4: "particles interact with distant
+ * tree nodes as they were point-like pseudo particles"); no formulas are given.  READING R23, the
+ * short-range force of the TreePM split of the Gadget lineage [2], with Plummer softening, minimum image, and an
+ * explicit truncation radius (the factor is 2e-3 at 4.5 r_s and the lineage stops the walk there):
+ *   a_i = - G sum_{j != i, r_ij < r_cut} m_j d_ij / (r_ij^2 + eps^2)^(3/2) * [erfc(r_ij / 2 r_s) + r_ij / (r_s sqrt(pi)) exp(-r_ij^2 / 4 r_s^2)]
+ * This is the exact definition (direct summation).  The tree code on the GPU reaches it up to the multipole
+ * error of its opening criterion (exactly, for an opening angle of zero).
+ */
+int orc_gravity_short(const orc_params *p, int64_t n, const float *pos, const float *mass, double mass_scalar, double G,
+                      double r_s, double r_cut, double eps, const int32_t *active, int64_t n_active, double *acc,
+                      double *asum)
+{
+    int64_t na = active ? n_active : n;
+    double L = p->box;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t a = 0; a < na; a++) {
+        int64_t i = active ? active[a] : a;
+        double ax = 0, ay = 0, az = 0, s = 0;
+        for (int64_t j = 0; j < n; j++) {
+            if (j == i) continue;
+            double d[3];
+            for (int k = 0; k < 3; k++) d[k] = min_image((double)pos[3 * i + k] - (double)pos[3 * j + k], L);
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            if (!(r2 < r_cut * r_cut)) continue;
+            double r = sqrt(r2), x = r / (2.0 * r_s);
+            double fac = erfc(x) + r / (r_s * sqrt(M_PI)) * exp(-x * x);
+            double mj = mass ? (double)mass[j] : mass_scalar;
+            double t = G * mj * fac / ((r2 + eps * eps) * sqrt(r2 + eps * eps));
+            ax -= t * d[0]; ay -= t * d[1]; az -= t * d[2];
+            s += t * r;
+        }
+        acc[3 * a] = ax; acc[3 * a + 1] = ay; acc[3 * a + 2] = az;
+        if (asum) asum[a] = s;
+    }
+    return 0;
+}

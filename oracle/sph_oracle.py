@@ -233,3 +233,18 @@ def thermal_conduction(pos, u, h, rho, *, kernel, kappa0, kappa_exp=2.5, box=1.0
                                  C.c_double(kappa0), C.c_double(kappa_exp), pact, C.c_int64(na),
                                  *[out[k].ctypes.data_as(C.c_void_p) for k in ("dudt", "dusum", "dusq")])
     return out
+
+
+def gravity_short(pos, *, G, r_s, r_cut, eps, box=1.0, mass=None, mass_scalar=1.0, active=None):
+    """R23: short-range (TreePM) gravity by direct summation. Returns dict acc (na,3), asum (sum of |pair terms|)."""
+    pos_, ppos = _p(pos, np.float32)
+    m_, pm = _p(mass, np.float32)
+    act_, pact = _p(active, np.int32)
+    n = pos_.shape[0]
+    na = n if act_ is None else act_.shape[0]
+    out = {"acc": np.zeros((na, 3), np.float64), "asum": np.zeros(na, np.float64)}
+    prm = _params(0, box, 5.0 / 3.0, 1.0, 0, 64)
+    lib().orc_gravity_short(C.byref(prm), C.c_int64(n), ppos, pm, C.c_double(mass_scalar), C.c_double(G), C.c_double(r_s),
+                            C.c_double(r_cut), C.c_double(eps), pact, C.c_int64(na), out["acc"].ctypes.data_as(C.c_void_p),
+                            out["asum"].ctypes.data_as(C.c_void_p))
+    return out

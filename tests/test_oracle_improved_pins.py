@@ -184,3 +184,42 @@ def test_thermal_conduction_two_particles_and_conservation():
     pos, vel, u, H, rho, om, m = _random_state(500, 4)
     o = O.thermal_conduction(pos, u, H, rho, kernel=0, kappa0=1.0, mass_scalar=m)
     assert abs(o["dudt"].sum()) < 1e-12 * o["dusum"].sum() and o["dusum"].sum() > 0  # equal masses: sum m du/dt = 0
+
+
+# ------------------------------------------------------------------ short-range gravity (R23)
+def test_gravity_short_two_particles_and_potential():
+    """R23: two particles -- the closed form with math.erfc, its Newtonian limit for r << r_s, the force as minus the
+    derivative of the short-range potential -G m erfc(r / 2 r_s) / r (finite difference), truncation at r_cut, and the
+    pair through the periodic wall."""
+    G, rs, m = 2.0, 0.05, 0.3
+    for r in (0.003, 0.02, 0.07, 0.15):
+        pos = np.array([[0.25, 0.5, 0.5], [0.25 + r, 0.5, 0.5]], np.float32)
+        rr = float(pos[1, 0]) - float(pos[0, 0])
+        o = O.gravity_short(pos, G=G, r_s=rs, r_cut=0.2, eps=0.0, mass_scalar=m)
+        x = rr / (2 * rs)
+        F = G * m / rr ** 2 * (math.erfc(x) + rr / (rs * math.sqrt(math.pi)) * math.exp(-x * x))
+        assert abs(o["acc"][0, 0] - F) < 1e-12 * F and abs(o["acc"][1, 0] + F) < 1e-12 * F  # attraction, antisymmetric
+        phi = lambda q: -G * m * math.erfc(q / (2 * rs)) / q
+        h = 1e-6 * rr
+        assert abs((phi(rr + h) - phi(rr - h)) / (2 * h) - F) < 1e-6 * F                      # F = -dPhi/dr (on particle 0: +x)
+        if r == 0.003:
+            assert abs(F / (G * m / rr ** 2) - 1) < 1e-4                                       # Newtonian for r << r_s
+    far = np.array([[0.1, 0.5, 0.5], [0.35, 0.5, 0.5]], np.float32)
+    assert np.all(O.gravity_short(far, G=G, r_s=rs, r_cut=0.2, eps=0.0, mass_scalar=m)["acc"] == 0)  # beyond r_cut
+    wall = np.array([[0.02, 0.5, 0.5], [0.97, 0.5, 0.5]], np.float32)
+    assert O.gravity_short(wall, G=G, r_s=rs, r_cut=0.2, eps=0.0, mass_scalar=m)["acc"][0, 0] < 0   # pulled through the wall
+    soft = O.gravity_short(np.array([[0.5, 0.5, 0.5], [0.51, 0.5, 0.5]], np.float32), G=G, r_s=rs, r_cut=0.2, eps=0.02, mass_scalar=m)
+    rr = float(np.float32(0.51)) - 0.5
+    x = rr / (2 * rs)
+    Fs = G * m * rr / (rr ** 2 + 0.02 ** 2) ** 1.5 * (math.erfc(x) + rr / (rs * math.sqrt(math.pi)) * math.exp(-x * x))
+    assert abs(soft["acc"][0, 0] - Fs) < 1e-12 * Fs
+
+
+def test_gravity_short_symmetries():
+    """Momentum: sum m a = 0 to rounding (all active); a perfect lattice feels nothing (inversion symmetry)."""
+    pos, vel, u, H, rho, om, m = _random_state(500, 12)
+    o = O.gravity_short(pos, G=1.0, r_s=0.04, r_cut=0.18, eps=0.005, mass_scalar=m)
+    assert np.all(np.abs(o["acc"].sum(0)) < 1e-12 * np.abs(o["acc"]).sum(0))
+    lat = I.perfect_lattice(8)
+    ol = O.gravity_short(lat, G=1.0, r_s=0.04, r_cut=0.18, eps=0.0, mass_scalar=1.0 / len(lat))
+    assert np.max(np.abs(ol["acc"])) < 1e-12 * ol["asum"].max()
