@@ -355,6 +355,16 @@ def main():
             torch.cuda.synchronize()
         ext_ms = {"velocity_gradients": ev[0].elapsed_time(ev[1]), "hydro_force_improved": ev[1].elapsed_time(ev[2]),
                   "note": "whole calls incl. the sorted-state preparation; base sph_hydro_force in phases_ms"}
+        # short-range Barnes-Hut gravity with TreePM-like parameters: mesh cell = half the mean particle
+        # spacing, r_s = 1.25 cells, r_cut = 4.5 r_s, softening = spacing / 40, opening angle 0.5
+        cell = 0.5 / n ** (1.0 / 3.0)
+        gk = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        for rep in range(2):
+            gk[0].record(stream)
+            sph.sph_gravity_short(acc, 1.0, 1.25 * cell, 4.5 * 1.25 * cell, 2.0 * cell / 40.0, 0.5, active=active)
+            gk[1].record(stream)
+            torch.cuda.synchronize()
+        ext_ms["gravity_short_theta0.5"] = gk[0].elapsed_time(gk[1])
     ms = max_over_ranks(ms, world, "cuda")
     value = whole_job_value(world, n_active, args.steps, ms)
 

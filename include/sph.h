@@ -205,6 +205,19 @@ int sph_thermal_conduction(sph_ctx *ctx, const int32_t *active, int64_t n_active
                            const float *rho, float kappa0, float kappa_exp, float *dudt_cond);
 
 /*
+ * Short-range Barnes-Hut gravity on the octree of the index (SURVEY.md §8(f)-4; PAPER.md:25 §1, :41, :102-104 §2.4;
+ * DESIGN.md reading R23): for every active particle i
+ *   acc_grav[id*3..] = - G sum_{j != i, r < r_cut} m_j d_ij / (r^2 + eps^2)^(3/2) [erfc(r / 2 r_s) + r / (r_s sqrt(pi)) exp(-r^2 / 4 r_s^2)],
+ * the short-range force of a TreePM split, evaluated with a grouped tree walk: a cell whose edge is smaller than theta
+ * times the distance from the group's bounding box to the cell's centre of mass enters as ONE pseudo-particle
+ * (monopole), closer cells are opened down to their particles.  theta = 0 opens everything: the exact direct sum.
+ * Uses the positions and masses of the index only.  r_cut < box/2.  acc_grav [n*3] device, written for active particles.
+ * Asynchronous.
+ */
+int sph_gravity_short(sph_ctx *ctx, const int32_t *active, int64_t n_active, float G, float r_s, float r_cut, float eps,
+                      float theta, float *acc_grav);
+
+/*
  * Kick-drift-kick time integration with power-of-two time bins (SURVEY.md §8(f)-3; PAPER.md:37 §1, :84-86 §2.2, :114
  * §3: the scheme that produces the paper's active lists, down to "one or very few" particles per step; no formulas in
  * the paper: DESIGN.md reading R22).  Timeline of T = 2^(n_bins-1) ticks per dt_max; a particle of bin b steps

@@ -20,7 +20,7 @@ KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
            "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_thermal_conduction",
-           "sph_kdk_init", "sph_kdk_step", "sph_last_error", "sph_version"]
+           "sph_kdk_init", "sph_kdk_step", "sph_gravity_short", "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -90,7 +90,8 @@ def load():
         lib.sph_kdk_init.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.POINTER(SphKdkParams), C.POINTER(SphKdkState)]
         lib.sph_kdk_step.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.POINTER(SphKdkParams), C.POINTER(SphKdkState),
                                      C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
-        for name in EXPORTS[:12]:
+        lib.sph_gravity_short.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_float] * 5 + [C.c_void_p]
+        for name in EXPORTS[:13]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -207,6 +208,13 @@ class Sph:
         self._check(self._lib.sph_thermal_conduction(self._h, _dev(active, torch.int32, "active"), na, _dev(u, f32, "u", n),
                                                      _dev(h, f32, "h", n), _dev(rho, f32, "rho", n), float(kappa0), float(kappa_exp),
                                                      _dev(dudt_cond, f32, "dudt_cond", n)))
+
+    def sph_gravity_short(self, acc_grav, G, r_s, r_cut, eps, theta, active=None):
+        """R23: short-range Barnes-Hut gravity on the octree of the index (theta = 0: exact direct sum)."""
+        n = self.n
+        na = -1 if active is None else active.numel()
+        self._check(self._lib.sph_gravity_short(self._h, _dev(active, torch.int32, "active"), na, float(G), float(r_s), float(r_cut),
+                                                float(eps), float(theta), _dev(acc_grav, torch.float32, "acc_grav", 3 * n)))
 
     # -- kick-drift-kick driver with power-of-two time bins (DESIGN.md R22) ---------------------------
     @staticmethod

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsph.so")
-SOURCES = ["sph_api.cu", "sph_index.cu", "sph_sort.cu", "sph_density.cu", "sph_force.cu", "sph_kdk.cu"]
+SOURCES = ["sph_api.cu", "sph_index.cu", "sph_sort.cu", "sph_density.cu", "sph_force.cu", "sph_kdk.cu", "sph_gravity.cu"]
 HEADERS = ["sph_internal.cuh", "sph_warp.cuh", os.path.join(ROOT, "include", "sph.h")]
 
 

@@ -114,7 +114,7 @@ int sph_destroy(sph_ctx *ctx)
     dfree(ctx->keys); dfree(ctx->keys_alt); dfree(ctx->perm); dfree(ctx->perm_alt); dfree(ctx->inv);
     dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->grp_start);
     dfree(ctx->cnt); dfree(ctx->sort_hist); dfree(ctx->scan_bsum); dfree(ctx->f_xyzh); dfree(ctx->f_vc); dfree(ctx->f_ext);
-    dfree(ctx->node_hmax); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
+    dfree(ctx->node_hmax); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
     dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
@@ -205,6 +205,25 @@ int sph_velocity_gradients(sph_ctx *ctx, const int32_t *active, int64_t n_active
     if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
     return sph_force_launch(ctx, SPH_MODE_GRADV, active != nullptr, items, vel, nullptr, h, rho, nullptr, nullptr, nullptr, nullptr,
                             nullptr, nullptr, nullptr, nullptr, nullptr, divv, curlv);
+}
+
+int sph_gravity_short(sph_ctx *ctx, const int32_t *active, int64_t n_active, float G, float r_s, float r_cut, float eps, float theta,
+                      float *acc_grav)
+{
+    if (!ctx) return SPH_E_ARG;
+    Range nv("sph_gravity_short");
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_gravity_short before sph_build_index");
+    if (!(G >= 0.f) || !(r_s > 0.f) || !(r_cut > 0.f) || !(r_cut < 0.5f * ctx->prm.box) || !(eps >= 0.f) || !(theta >= 0.f))
+        return sph_fail(ctx, SPH_E_ARG, "sph_gravity_short: bad G, r_s, r_cut (must be < box/2), eps or theta");
+    const bool subset = active != nullptr || n_active == 0;
+    if (active && n_active < 0) return sph_fail(ctx, SPH_E_ARG, "sph_gravity_short: n_active < 0");
+    int64_t items = subset ? n_active : ctx->n;
+    if (ctx->n == 0 || items == 0) return SPH_OK;
+    if (!acc_grav) return sph_fail(ctx, SPH_E_ARG, "sph_gravity_short: NULL array");
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    if (active && (rc = sph_active_groups(ctx, active, n_active))) return rc;
+    return sph_gravity_launch(ctx, active != nullptr, items, G, r_s, r_cut, eps, theta, acc_grav);
 }
 
 int sph_thermal_conduction(sph_ctx *ctx, const int32_t *active, int64_t n_active, const float *u, const float *h,

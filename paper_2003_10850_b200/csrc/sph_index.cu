@@ -205,6 +205,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
         if ((rc = ensure(ctx, &ctx->f_xyzh, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->f_vc, 2 * cap))) return rc; // 32-byte records (v,c | rho,A,m,1/H)
         if (ctx->f_ext) { cudaFree(ctx->f_ext); ctx->f_ext = nullptr; } // (re-allocated on first use)
+        if (ctx->node_mom) { cudaFree(ctx->node_mom); ctx->node_mom = nullptr; ctx->node_mom_cap = 0; }
         // node pool: internal nodes hold > B particles each; 8 children per internal node.
         // Typical use is ~ 8 n / (3 B); the pool is sized generously and overflow degrades gracefully.
         int64_t ncap = 64 + 8 * (2 * cap / (int64_t)(B > 4 ? B / 4 : 1) + 8);

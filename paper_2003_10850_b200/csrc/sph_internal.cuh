@@ -114,6 +114,8 @@ struct sph_ctx {
     // force pass (device)
     float4 *f_xyzh, *f_vc, *f_ext; // f_ext: improved-SPH record (alpha, f, u), allocated on first use
     float *node_hmax;
+    float4 *node_mom;     // short-range gravity: centre of mass and mass of every node (allocated on first use)
+    int64_t node_mom_cap;
 
     // active subset scratch (device)
     int64_t cap_act;
@@ -147,6 +149,7 @@ enum { SPH_MODE_BASE = 0, SPH_MODE_IMPROVED = 1, SPH_MODE_GRADV = 2, SPH_MODE_CO
 
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
+int sph_gravity_launch(sph_ctx *ctx, bool subset, int64_t n_items, float G, float r_s, float r_cut, float eps, float theta, float *acc);
 // stable LSD radix sort on the low `bits` key bits; *in_alt = 1 if the result ended up in the *_alt buffers
 int sph_sort_pairs_u64(sph_ctx *ctx, uint64_t *keys, uint64_t *keys_alt, uint32_t *vals, uint32_t *vals_alt, int64_t n, int bits,
                        int *in_alt);
