@@ -241,6 +241,8 @@ def main():
     ap.add_argument("--kdk-steps", type=int, default=0,
                     help="after the timed region, run this many steps of the kick-drift-kick driver (SURVEY.md 8(f)-3) on the "
                          "workload and report active counts and times per step")
+    ap.add_argument("--kdk-refresh-max", type=int, default=16,
+                    help="sph_kdk_params.refresh_max: steps in a row that refresh the index instead of rebuilding it (0 = never)")
     ap.add_argument("--group-cap", type=int, default=0, help="actives per group (0 = library default)")
     ap.add_argument("--group-node", type=int, default=0, help="group-node capacity (0 = library default)")
     args = ap.parse_args()
@@ -379,7 +381,7 @@ def main():
                     vpred=torch.zeros((n, 3), device="cuda"), upred=torch.zeros(n, device="cuda"),
                     bin=torch.zeros(n, device="cuda", dtype=torch.int32), tbegin=torch.zeros(n, device="cuda", dtype=torch.int32),
                     active=torch.zeros(n, device="cuda", dtype=torch.int32))
-        sph.sph_kdk_init(stt_, ps.mass, 4.0 * dt_med, 12, ps.n_ngb, ps.n_tol)
+        sph.sph_kdk_init(stt_, ps.mass, 4.0 * dt_med, 12, ps.n_ngb, ps.n_tol, refresh_max=args.kdk_refresh_max)
         torch.cuda.synchronize()
         rows = []
         for _ in range(args.kdk_steps):
@@ -390,7 +392,7 @@ def main():
             torch.cuda.synchronize()
             rows.append((tick, na, k0.elapsed_time(k1)))
         tot_a, tot_ms = sum(r[1] for r in rows), sum(r[2] for r in rows)
-        kdk = {"steps": len(rows), "dt_max": 4.0 * dt_med, "n_bins": 12, "active_per_step": [r[1] for r in rows],
+        kdk = {"steps": len(rows), "dt_max": 4.0 * dt_med, "n_bins": 12, "refresh_max": args.kdk_refresh_max, "active_per_step": [r[1] for r in rows],
                "ms_per_step": [round(r[2], 3) for r in rows], "updates_per_s": tot_a / (tot_ms * 1e-3),
                "bins_occupied": sorted(set(torch.unique(stt_["bin"]).cpu().tolist()))}
 

@@ -118,6 +118,18 @@ int sph_destroy(sph_ctx *ctx);
 int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar);
 
 /*
+ * Refresh the index after the particles have MOVED A LITTLE (same n, same ids): the sorted order, the octree and the
+ * groups of the last sph_build_index are kept, the sorted positions are replaced by the new ones and every octree cell
+ * is enlarged by the distance its farthest particle now lies outside it.  Results of the later calls are exactly those
+ * of a fresh build (the neighbour search only prunes more conservatively), at about a fifth of its cost; the pruning
+ * degrades as particles stray from their cells, so rebuild once displacements become comparable to the support radii.
+ * This is what keeps time-steps with few active particles cheap (PAPER.md:57 §2, :86 §2.2, :160 §3.3: the paper's weak
+ * point; SURVEY.md §8(f)-3 "incremental index refresh instead of full rebuild").  pos [n*3] device, 0 <= x < box
+ * (checked on the device).  Asynchronous.
+ */
+int sph_refresh_index(sph_ctx *ctx, int64_t n, const float *pos);
+
+/*
  * SPH density with the smoothing-length iteration (steps a5-a9; R1-R7):
  * for every active particle, starting from h[id], iterate the safeguarded Newton rule of R7 on the
  * support radius until the neighbour number N (kernel-weighted, or integer with count_mode 1)
@@ -227,8 +239,10 @@ int sph_gravity_short(sph_ctx *ctx, const int32_t *active, int64_t n_active, flo
  *                 kick-centred).  h is the guess on entry.
  *   sph_kdk_step: advance to the next tick at which a step ends; drift ALL particles there (pos, periodic wrap;
  *                 vpred, upred = velocity and energy extrapolated to that time with the stored acc, dudt); the
- *                 particles whose step ends are active: sph_build_index, sph_density (last h as the guess),
- *                 sph_hydro_force (with vpred, upred) on them; second half kick, new bin, first half kick.
+ *                 particles whose step ends are active: sph_build_index -- or, for a step with fewer than
+ *                 rebuild_fraction * n active particles and at most refresh_max times in a row, sph_refresh_index (the
+ *                 same results, see there) --, sph_density (last h as the guess), sph_hydro_force (with vpred, upred)
+ *                 on them; second half kick, new bin, first half kick.
  *                 *tick_host = the new tick, *n_active_host = number of active particles (their ids, ascending,
  *                 are left in state->active).  Synchronises.
  * All arrays of sph_kdk_state are DEVICE arrays owned by the caller.
@@ -239,6 +253,8 @@ typedef struct {
     float courant;      /* 0.3 */
     float eta;          /* 0.025 */
     float n_ngb_target, n_ngb_tol;
+    int refresh_max;    /* steps in a row that may refresh the index instead of rebuilding it; 0 = always rebuild */
+    float rebuild_fraction; /* rebuild whenever n_active >= rebuild_fraction * n (1/16) */
 } sph_kdk_params;
 
 typedef struct {

@@ -20,7 +20,7 @@ KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
            "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_thermal_conduction",
-           "sph_kdk_init", "sph_kdk_step", "sph_gravity_short", "sph_last_error", "sph_version"]
+           "sph_kdk_init", "sph_kdk_step", "sph_gravity_short", "sph_refresh_index", "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -42,7 +42,7 @@ class SphImprovedParams(C.Structure):
 
 class SphKdkParams(C.Structure):
     _fields_ = [("dt_max", C.c_float), ("n_bins", C.c_int), ("courant", C.c_float), ("eta", C.c_float),
-                ("n_ngb_target", C.c_float), ("n_ngb_tol", C.c_float)]
+                ("n_ngb_target", C.c_float), ("n_ngb_tol", C.c_float), ("refresh_max", C.c_int), ("rebuild_fraction", C.c_float)]
 
 
 KDK_F32 = ("pos", "vel", "u", "h", "rho", "omega")
@@ -91,7 +91,8 @@ def load():
         lib.sph_kdk_step.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.POINTER(SphKdkParams), C.POINTER(SphKdkState),
                                      C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         lib.sph_gravity_short.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_float] * 5 + [C.c_void_p]
-        for name in EXPORTS[:13]:
+        lib.sph_refresh_index.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
+        for name in EXPORTS[:14]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -154,6 +155,11 @@ class Sph:
         self._check(self._lib.sph_build_index(self._h, n, _dev(pos, torch.float32, "pos", 3 * n),
                                               _dev(mass, torch.float32, "mass", n), float(mass_scalar)))
         self.n = n
+
+    def sph_refresh_index(self, pos):
+        """Positions moved a little since sph_build_index: keep the tree, refresh the sorted positions, enlarge the cells."""
+        n = pos.shape[0]
+        self._check(self._lib.sph_refresh_index(self._h, n, _dev(pos, torch.float32, "pos", 3 * n)))
 
     def sph_density(self, h, rho, omega, ngb_count, n_ngb_target, n_ngb_tol, active=None, status=None):
         """Returns the number of active particles that stopped without convergence."""
@@ -225,9 +231,10 @@ class Sph:
             setattr(st, k, _dev(state[k], dt, k, w * n))
         return st
 
-    def sph_kdk_init(self, state: dict, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025):
+    def sph_kdk_init(self, state: dict, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025,
+                     refresh_max=16, rebuild_fraction=1.0 / 16):
         n = state["pos"].shape[0]
-        self._kdk_p = SphKdkParams(dt_max, n_bins, courant, eta, n_ngb_target, n_ngb_tol)
+        self._kdk_p = SphKdkParams(dt_max, n_bins, courant, eta, n_ngb_target, n_ngb_tol, refresh_max, rebuild_fraction)
         st = self._kdk_state(state, n)
         self._check(self._lib.sph_kdk_init(self._h, n, float(mass_scalar), C.byref(self._kdk_p), C.byref(st)), allow=(SPH_OK, SPH_W_NOCONV))
         self.n = n

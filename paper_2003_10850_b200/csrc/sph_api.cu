@@ -112,9 +112,9 @@ int sph_destroy(sph_ctx *ctx)
     if (!ctx) return SPH_E_ARG;
     cudaStreamSynchronize(ctx->stream);
     dfree(ctx->keys); dfree(ctx->keys_alt); dfree(ctx->perm); dfree(ctx->perm_alt); dfree(ctx->inv);
-    dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->grp_start);
+    dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->slot_leaf); dfree(ctx->grp_start);
     dfree(ctx->cnt); dfree(ctx->sort_hist); dfree(ctx->scan_bsum); dfree(ctx->f_xyzh); dfree(ctx->f_vc); dfree(ctx->f_ext);
-    dfree(ctx->node_hmax); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
+    dfree(ctx->node_hmax); dfree(ctx->node_slack); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
     dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
@@ -141,6 +141,18 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
     cudaEventRecord(ctx->ev[1], ctx->stream);
     ctx->ev_set[0] = true;
     return rc;
+}
+
+int sph_refresh_index(sph_ctx *ctx, int64_t n, const float *pos)
+{
+    if (!ctx) return SPH_E_ARG;
+    Range nv("sph_refresh_index");
+    if (!ctx->have_index) return sph_fail(ctx, SPH_E_NOINDEX, "sph_refresh_index before sph_build_index");
+    if (n != ctx->n || (n > 0 && !pos)) return sph_fail(ctx, SPH_E_ARG, "sph_refresh_index: n differs from the index or pos is NULL");
+    if (n == 0) return SPH_OK;
+    int rc = check_sticky(ctx);
+    if (rc) return rc;
+    return sph_index_refresh(ctx, pos);
 }
 
 int sph_density(sph_ctx *ctx, const int32_t *active, int64_t n_active, float n_ngb_target, float n_ngb_tol, float *h,
@@ -318,8 +330,10 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
     int rcd = sph_density(ctx, act, n_active, n_ngb_target, n_ngb_tol, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_ngb,
                           nullptr, n_unconverged_host);
     if (rcd != SPH_OK && rcd != SPH_W_NOCONV) return rcd;
+    ctx->act_keep = true; // the same active list: its groups are those of the density pass
     rc = sph_hydro_force(ctx, act, n_active, ctx->d_vel, ctx->d_u, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_acc,
                          ctx->d_dudt, ctx->d_vsig);
+    ctx->act_keep = false;
     if (rc) return rc;
     SPH_CUDA(ctx, cudaMemcpyAsync(h_host, ctx->d_h, c * sizeof(float), cudaMemcpyDeviceToHost, st));
     SPH_CUDA(ctx, cudaMemcpyAsync(rho_host, ctx->d_rho, c * sizeof(float), cudaMemcpyDeviceToHost, st));

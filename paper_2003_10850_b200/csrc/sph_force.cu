@@ -393,11 +393,29 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
                              const float *__restrict__ rho, const float *__restrict__ omega, float gamma, float half_box,
                              float4 *__restrict__ xyzh, float4 *__restrict__ vc, SphCounters *cnt,
                              const float *__restrict__ alpha, const float *__restrict__ divv, const float *__restrict__ curlv,
-                             int balsara, float4 *__restrict__ ext, float kappa0, float kappa_exp, int conduct)
+                             int balsara, float4 *__restrict__ ext, float kappa0, float kappa_exp, int conduct,
+                             const SphNode *__restrict__ nodes, const uint32_t *__restrict__ slot_leaf, float *__restrict__ hmax)
 {
     // u, omega may be NULL (velocity-gradient pass: only positions, h, velocities, rho and masses are used);
     // alpha != NULL: improved-SPH state record (alpha, shear limiter f of R18, u) per particle
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // largest support radius inside every octree node (hmax != NULL; zeroed before): the lanes that share a leaf send
+    // one value up the parent chain with integer atomicMax (H > 0: the float bit patterns order like integers)
+    if (hmax) {
+        const uint32_t leaf = i < n ? slot_leaf[i] : 0xffffffffu;
+        const float H = i < n ? h[perm[i]] : 0.f;
+        const unsigned grp = __match_any_sync(0xffffffffu, leaf);
+        const int mb = __reduce_max_sync(grp, H > 0.f ? __float_as_int(H) : 0);
+        if (i < n && (threadIdx.x & 31) == __ffs(grp) - 1 && mb > 0) {
+            uint32_t cur = leaf;
+            for (;;) {
+                if (__float_as_int(__ldcg(hmax + cur)) >= mb) break;
+                const int old = atomicMax(reinterpret_cast<int *>(hmax) + cur, mb);
+                if (cur == 0 || old >= mb) break;
+                cur = nodes[cur].parent;
+            }
+        }
+    }
     if (i >= n) return;
     uint32_t id = perm[i];
     float4 p = xyzm[i];
@@ -429,31 +447,10 @@ __global__ void k_force_prep(int64_t n, const uint32_t *__restrict__ perm, const
     }
 }
 
-// largest support radius inside every octree node: leaves scan their particles, then push the value
-// up the parent chain with integer atomicMax (H > 0, so the float bit patterns order like integers)
 __global__ void k_zero_hmax(const SphCounters *cnt, float *__restrict__ hmax)
 {
     uint32_t nn = cnt->n_nodes;
     for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) hmax[nd] = 0.f;
-}
-
-__global__ void k_node_hmax(const SphCounters *cnt, const SphNode *__restrict__ nodes, const float4 *__restrict__ xyzh,
-                            float *__restrict__ hmax)
-{
-    uint32_t nn = cnt->n_nodes;
-    for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) {
-        SphNode p = nodes[nd];
-        if (p.child != 0 || p.count == 0) continue;
-        float m = 0.f;
-        for (uint32_t s = 0; s < p.count; s++) m = fmaxf(m, xyzh[p.start + s].w);
-        int mb = __float_as_int(m);
-        uint32_t cur = nd;
-        for (;;) {
-            int old = atomicMax(reinterpret_cast<int *>(hmax) + cur, mb);
-            if (cur == 0 || old >= mb) break;
-            cur = nodes[cur].parent;
-        }
-    }
 }
 
 template <int KERNEL, int MODE>
@@ -488,16 +485,17 @@ int sph_force_launch(sph_ctx *ctx, int mode, bool subset, int64_t n_items, const
         SPH_CUDA(ctx, cudaMalloc((void **)&ctx->f_ext, sizeof(float4) * (size_t)ctx->cap_n));
     }
     cudaEventRecord(ctx->ev[4], st);
+    const bool need_hmax = mode != MODE_GRADV; // the symmetric pair set needs the largest support radius inside every node
+    if (need_hmax) {
+        k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
+        ctx->launches++;
+    }
     k_force_prep<<<(int)((n + T - 1) / T), T, 0, st>>>(n, ctx->perm, ctx->xyzm, vel, u, h, rho, omega, ctx->prm.gamma,
                                                        0.5f * ctx->prm.box, ctx->f_xyzh, ctx->f_vc, ctx->cnt,
                                                        mode == MODE_IMPROVED ? alpha : nullptr, divv, curlv,
-                                                       ip ? ip->balsara : 0, ctx->f_ext, kappa0, kappa_exp, mode == MODE_CONDUCT);
+                                                       ip ? ip->balsara : 0, ctx->f_ext, kappa0, kappa_exp, mode == MODE_CONDUCT,
+                                                       ctx->nodes, ctx->slot_leaf, need_hmax ? ctx->node_hmax : nullptr);
     ctx->launches++;
-    if (mode != MODE_GRADV) { // the symmetric pair set needs the largest support radius inside every node
-        k_zero_hmax<<<ctx->device_sms * 4, 256, 0, st>>>(ctx->cnt, ctx->node_hmax);
-        k_node_hmax<<<ctx->device_sms * 4, 128, 0, st>>>(ctx->cnt, ctx->nodes, ctx->f_xyzh, ctx->node_hmax);
-        ctx->launches += 2;
-    }
     sph_reset_counters(ctx, 1, subset);
     cudaEventRecord(ctx->ev[5], st);
     ctx->ev_set[2] = true;

@@ -137,12 +137,15 @@ __global__ void k_tree_split(SphCounters *cnt, SphNode *nodes, const uint64_t *_
 // (a leaf that holds more, e.g. coincident particles, is its own group node); every group node is cut
 // into ceil(count / grp_cap) balanced runs of consecutive sorted slots; a run is a group (consecutive
 // Morton order inside a small cell keeps a run spatially compact)
+// (+ the leaf of every sorted slot, for the per-particle passes that feed per-node maxima: k_force_prep, k_refresh_slots)
 __global__ void k_mark_groups(const SphCounters *cnt, const SphNode *__restrict__ nodes, uint32_t grp_cap,
-                              uint32_t node_cap, uint32_t *__restrict__ mark)
+                              uint32_t node_cap, uint32_t *__restrict__ mark, uint32_t *__restrict__ slot_leaf)
 {
     uint32_t nn = cnt->n_nodes;
     for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) {
         SphNode p = nodes[nd];
+        if (p.child == 0)
+            for (uint32_t s = 0; s < p.count; s++) slot_leaf[p.start + s] = nd;
         if (p.count == 0 || (p.count > node_cap && p.child != 0)) continue;
         if (nd != 0 && nodes[p.parent].count <= node_cap) continue; // an ancestor is the group node
         const uint32_t ns = (p.count + grp_cap - 1) / grp_cap;
@@ -169,6 +172,66 @@ __global__ void k_act_flags(int64_t na, const uint32_t *__restrict__ slot, const
     flag[k] = (k == 0 || gid[slot[k]] != gid[slot[k - 1]]) ? 1u : 0u;
     // an id listed twice sits next to itself in the sorted slots (and would make a group larger than a warp)
     if (k > 0 && slot[k] == slot[k - 1] && !(cnt->err & SPH_ERR_IDS)) atomicOr(&cnt->err, SPH_ERR_DUP);
+}
+
+// ---- sph_refresh_index: the particles moved a little since the build; keep the tree, make every cell large enough ----
+__device__ __forceinline__ int level_of(const SphCounters *cnt, uint32_t nd)
+{
+    int l = 0;
+    while (l < SPH_LMAX && nd >= cnt->lvl_begin[l + 1]) l++;
+    return l;
+}
+
+// every sorted slot: fetch the particle's new position into the sorted copy; slack of its leaf = how far the farthest of
+// the leaf's particles now lies outside the leaf's cell (periodic), handed up the parent chain (a particle outside a
+// cell by s is outside each ancestor's cell by at most s).  The lanes of a warp that share a leaf send one value.
+__global__ void k_refresh_slots(int64_t n, SphCounters *cnt, const SphNode *__restrict__ nodes, const uint32_t *__restrict__ perm,
+                                const uint32_t *__restrict__ slot_leaf, const float *__restrict__ pos, float box,
+                                float4 *__restrict__ xyzm, float *__restrict__ slack)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool in = i < n;
+    uint32_t leaf = 0xffffffffu;
+    float d = 0.f;
+    if (in) {
+        const uint32_t id = perm[i];
+        const float x = pos[3 * (size_t)id], y = pos[3 * (size_t)id + 1], z = pos[3 * (size_t)id + 2];
+        if (!(x >= 0.f && x < box && y >= 0.f && y < box && z >= 0.f && z < box)) atomicOr(&cnt->idx_err, SPH_ERR_POS);
+        float4 q = xyzm[i];
+        q.x = x; q.y = y; q.z = z;
+        xyzm[i] = q;
+        leaf = slot_leaf[i];
+        const SphNode p = nodes[leaf];
+        float dx = fabsf(x - p.cx), dy = fabsf(y - p.cy), dz = fabsf(z - p.cz);
+        dx = fminf(dx, box - dx); dy = fminf(dy, box - dy); dz = fminf(dz, box - dz);
+        d = fmaxf(fmaxf(dx, dy), dz); // >= 0 (NaN -> 0: the position error is already recorded)
+    }
+    const unsigned grp = __match_any_sync(0xffffffffu, leaf);
+    const int db = __reduce_max_sync(grp, __float_as_int(d));
+    if (!in || (threadIdx.x & 31) != __ffs(grp) - 1) return;
+    const float m = __int_as_float(db) - ldexpf(box, -(level_of(cnt, leaf) + 1));
+    if (!(m > 0.f)) return;
+    const int mb = __float_as_int(m);
+    uint32_t cur = leaf;
+    for (;;) {
+        const int old = atomicMax(reinterpret_cast<int *>(slack) + cur, mb);
+        if (cur == 0 || old >= mb) break;
+        cur = nodes[cur].parent;
+    }
+}
+
+__global__ void k_refresh_zero(const SphCounters *cnt, float *__restrict__ slack)
+{
+    const uint32_t nn = cnt->n_nodes;
+    for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x) slack[nd] = 0.f;
+}
+
+// half edge of every cell = its geometric half edge + its slack
+__global__ void k_refresh_apply(const SphCounters *cnt, SphNode *__restrict__ nodes, const float *__restrict__ slack, float box)
+{
+    const uint32_t nn = cnt->n_nodes;
+    for (uint32_t nd = blockIdx.x * blockDim.x + threadIdx.x; nd < nn; nd += gridDim.x * blockDim.x)
+        nodes[nd].half = ldexpf(box, -(level_of(cnt, nd) + 1)) + slack[nd] * (1.f + 1e-6f);
 }
 
 template <typename T>
@@ -201,6 +264,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
         if ((rc = ensure(ctx, &ctx->xyzm, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->grp_mark, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->gid_of_slot, cap))) return rc;
+        if ((rc = ensure(ctx, &ctx->slot_leaf, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->grp_start, cap + 1))) return rc;
         if ((rc = ensure(ctx, &ctx->f_xyzh, cap))) return rc;
         if ((rc = ensure(ctx, &ctx->f_vc, 2 * cap))) return rc; // 32-byte records (v,c | rho,A,m,1/H)
@@ -213,6 +277,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
         ncap = 1 + 8 * ((ncap - 1) / 8);
         if ((rc = ensure(ctx, &ctx->nodes, ncap))) return rc;
         if ((rc = ensure(ctx, &ctx->node_hmax, ncap))) return rc;
+        if ((rc = ensure(ctx, &ctx->node_slack, ncap))) return rc;
         ctx->node_cap = ncap;
         ctx->cap_n = cap;
     }
@@ -254,7 +319,7 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     // a5: group starts in sorted order + group id of every slot
     SPH_CUDA(ctx, cudaMemsetAsync(ctx->grp_mark, 0, sizeof(uint32_t) * n, st));
     k_mark_groups<<<grid, 128, 0, st>>>(ctx->cnt, ctx->nodes, (uint32_t)ctx->grp_cap,
-                                        (uint32_t)(ctx->grp_node > SPH_LEAF ? ctx->grp_node : SPH_LEAF), ctx->grp_mark);
+                                        (uint32_t)(ctx->grp_node > SPH_LEAF ? ctx->grp_node : SPH_LEAF), ctx->grp_mark, ctx->slot_leaf);
     ctx->launches++;
     if ((rc = sph_scan_marks(ctx, ctx->grp_mark, n, ctx->gid_of_slot, ctx->grp_start, &ctx->cnt->n_groups))) return rc;
 
@@ -265,20 +330,27 @@ int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass)
     return SPH_OK;
 }
 
+// room for active lists of up to cap entries (a time-bin driver reserves n once instead of growing step by step)
+int sph_active_reserve(sph_ctx *ctx, int64_t cap)
+{
+    int rc;
+    if (cap <= ctx->cap_act) return SPH_OK;
+    ctx->cap_act = 0;
+    if ((rc = ensure(ctx, &ctx->act_slot, cap))) return rc;
+    if ((rc = ensure(ctx, &ctx->act_slot_alt, cap))) return rc;
+    if ((rc = ensure(ctx, &ctx->act_flag, cap))) return rc;
+    if ((rc = ensure(ctx, &ctx->agrp_start, cap + 1))) return rc;
+    ctx->cap_act = cap;
+    return SPH_OK;
+}
+
 // a5 (active subset): ids -> sorted slots -> sort -> groups = runs sharing an all-active group
 int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
 {
     cudaStream_t st = ctx->stream;
     int rc;
-    if (na > ctx->cap_act) {
-        int64_t cap = na + na / 8 + 1024;
-        ctx->cap_act = 0;
-        if ((rc = ensure(ctx, &ctx->act_slot, cap))) return rc;
-        if ((rc = ensure(ctx, &ctx->act_slot_alt, cap))) return rc;
-        if ((rc = ensure(ctx, &ctx->act_flag, cap))) return rc;
-        if ((rc = ensure(ctx, &ctx->agrp_start, cap + 1))) return rc;
-        ctx->cap_act = cap;
-    }
+    if (ctx->act_keep) return SPH_OK; // the caller (a driver inside the library) vouches: same list, same index as the last call
+    if (na > ctx->cap_act && (rc = sph_active_reserve(ctx, na + na / 8 + 1024))) return rc;
     const int T = 256;
     k_act_slots<<<nblocks(na, T), T, 0, st>>>(na, ctx->n, active, ctx->inv, ctx->act_slot_alt, ctx->cnt);
     int bits = 1;
@@ -289,5 +361,19 @@ int sph_active_groups(sph_ctx *ctx, const int32_t *active, int64_t na)
     k_act_flags<<<nblocks(na, T), T, 0, st>>>(na, ctx->act_slot, ctx->gid_of_slot, ctx->act_flag, ctx->cnt);
     if ((rc = sph_scan_marks(ctx, ctx->act_flag, na, nullptr, ctx->agrp_start, &ctx->cnt->n_agroups))) return rc;
     ctx->launches += 2;
+    return SPH_OK;
+}
+
+// positions moved since sph_index_build: same tree, same sorted order, cells inflated to hold their particles
+int sph_index_refresh(sph_ctx *ctx, const float *pos)
+{
+    cudaStream_t st = ctx->stream;
+    const int grid = ctx->device_sms * 4;
+    k_refresh_zero<<<grid, 256, 0, st>>>(ctx->cnt, ctx->node_slack);
+    k_refresh_slots<<<nblocks(ctx->n, 256), 256, 0, st>>>(ctx->n, ctx->cnt, ctx->nodes, ctx->perm, ctx->slot_leaf, pos, ctx->prm.box, ctx->xyzm,
+                                                          ctx->node_slack);
+    k_refresh_apply<<<grid, 256, 0, st>>>(ctx->cnt, ctx->nodes, ctx->node_slack, ctx->prm.box);
+    ctx->launches += 3;
+    SPH_CUDA(ctx, cudaGetLastError());
     return SPH_OK;
 }

@@ -44,12 +44,8 @@
 #ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
 #endif
-#ifndef SPH_NA
-#define SPH_NA 1            // actives per lane of the density gather (1 or 2)
-#endif
-#ifndef SPH_GBLOCK
-#define SPH_GBLOCK 1         // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
-#endif
+#define SPH_NA 1            // actives per lane of the density gather (2 measured slower: profiles/r1j_gather.md)
+#define SPH_GBLOCK 1        // consecutive groups a warp takes per work-counter increment (1: shortest tail, measured)
 
 // device-side precondition failures (SphCounters::err / idx_err)
 #define SPH_ERR_IDS 1u      // an active id outside [0, n)
@@ -105,6 +101,7 @@ struct sph_ctx {
     SphNode *nodes;
     int64_t node_cap;
     uint32_t *grp_mark, *gid_of_slot, *grp_start;
+    uint32_t *slot_leaf;  // octree leaf of every sorted slot
     SphCounters *cnt;
     uint32_t *sort_hist;   // radix sort: per-tile digit histograms + digit bases
     size_t sort_cap;
@@ -114,6 +111,9 @@ struct sph_ctx {
     // force pass (device)
     float4 *f_xyzh, *f_vc, *f_ext; // f_ext: improved-SPH record (alpha, f, u), allocated on first use
     float *node_hmax;
+    bool act_keep;        // sph_active_groups: keep the groups of the last call (set by sph_kdk_step / sph_step_* between density and force)
+    int kdk_refreshed;    // steps of sph_kdk_step since the last full build
+    float *node_slack;    // sph_refresh_index: how far particles have left their cells (per node)
     float4 *node_mom;     // short-range gravity: centre of mass and mass of every node (allocated on first use)
     int64_t node_mom_cap;
 
@@ -149,6 +149,8 @@ enum { SPH_MODE_BASE = 0, SPH_MODE_IMPROVED = 1, SPH_MODE_GRADV = 2, SPH_MODE_CO
 
 // stages (each returns sph_status) --------------------------------------------------------------
 int sph_index_build(sph_ctx *ctx, const float *pos, const float *mass);
+int sph_index_refresh(sph_ctx *ctx, const float *pos);
+int sph_active_reserve(sph_ctx *ctx, int64_t cap);
 int sph_gravity_launch(sph_ctx *ctx, bool subset, int64_t n_items, float G, float r_s, float r_cut, float eps, float theta, float *acc);
 // stable LSD radix sort on the low `bits` key bits; *in_alt = 1 if the result ended up in the *_alt buffers
 int sph_sort_pairs_u64(sph_ctx *ctx, uint64_t *keys, uint64_t *keys_alt, uint32_t *vals, uint32_t *vals_alt, int64_t n, int bits,

@@ -145,10 +145,12 @@ int sph_kdk_init(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
     int rc = check(ctx, n, p, s, k);
     if (rc) return rc;
     ctx->kdk_tick = 0;
+    ctx->kdk_refreshed = 0;
     if (n == 0) return SPH_OK;
     cudaStream_t st = ctx->stream;
     const int T = 256, G = (int)((n + T - 1) / T);
     if ((rc = sph_build_index(ctx, n, s->pos, nullptr, mass_scalar))) return rc;
+    if ((rc = sph_active_reserve(ctx, n))) return rc; // active lists of any length without reallocation later
     int64_t unconv = 0;
     rc = sph_density(ctx, nullptr, -1, p->n_ngb_target, p->n_ngb_tol, s->h, s->rho, s->omega, s->ngb, nullptr, &unconv);
     if (rc != SPH_OK && rc != SPH_W_NOCONV) return rc;
@@ -190,16 +192,26 @@ int sph_kdk_step(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
     SPH_CUDA(ctx, cudaStreamSynchronize(st));
     ctx->launches += 2;
     // the hot path for the active particles at their new positions
-    if ((rc = sph_build_index(ctx, n, s->pos, nullptr, mass_scalar))) return rc;
+    // (few active particles: keep the tree and refresh it; the rebuild would be most of the step)
+    const bool refresh = ctx->have_index && ctx->n == n && ctx->kdk_refreshed < p->refresh_max && (double)na < (double)p->rebuild_fraction * (double)n;
+    if (refresh) {
+        if ((rc = sph_refresh_index(ctx, n, s->pos))) return rc;
+        ctx->kdk_refreshed++;
+    } else {
+        if ((rc = sph_build_index(ctx, n, s->pos, nullptr, mass_scalar))) return rc;
+        ctx->kdk_refreshed = 0;
+    }
     int64_t unconv = 0;
     const bool all = (int64_t)na == n;
     rc = sph_density(ctx, all ? nullptr : s->active, all ? -1 : (int64_t)na, p->n_ngb_target, p->n_ngb_tol, s->h, s->rho, s->omega, s->ngb,
                      nullptr, &unconv);
     if (rc != SPH_OK && rc != SPH_W_NOCONV) return rc;
     const int rcd = rc;
-    if ((rc = sph_hydro_force(ctx, all ? nullptr : s->active, all ? -1 : (int64_t)na, s->vpred, s->upred, s->h, s->rho, s->omega, s->acc,
-                              s->dudt, s->vsig)))
-        return rc;
+    ctx->act_keep = true; // the same active list: its groups are those of the density pass
+    rc = sph_hydro_force(ctx, all ? nullptr : s->active, all ? -1 : (int64_t)na, s->vpred, s->upred, s->h, s->rho, s->omega, s->acc, s->dudt,
+                         s->vsig);
+    ctx->act_keep = false;
+    if (rc) return rc;
     if (all) k_iota<<<G, T, 0, st>>>(n, s->active);
     if (na) k_kdk_close_open<<<(int)((na + T - 1) / T), T, 0, st>>>((int64_t)na, k, t1, s->active, s->h, s->vsig, s->acc, s->dudt, s->vel, s->u,
                                                                    s->bin, s->tbegin);

@@ -35,8 +35,10 @@ def _close(a, b, rtol, scale, what):
     assert np.all(err <= tol), f"{what}: worst err/tol {np.max(err / tol):.3f}"
 
 
-@pytest.mark.parametrize("shape", ["C1", "C3"])
-def test_kdk_driver_in_lock_step_with_the_oracle(shape):
+# refresh_max = 0: an index build every step; 4 with rebuild_fraction 2: four refreshed steps (sph_refresh_index: the old
+# tree with enlarged cells), then a rebuild, whatever the number of active particles -- the same results either way
+@pytest.mark.parametrize("shape,refresh_max", [("C1", 0), ("C1", 4), ("C3", 0), ("C3", 4)])
+def test_kdk_driver_in_lock_step_with_the_oracle(shape, refresh_max):
     if shape == "C1":
         ps = I.config1(12)
         rng = np.random.default_rng(9)
@@ -50,7 +52,8 @@ def test_kdk_driver_in_lock_step_with_the_oracle(shape):
     n = ps.n
     sph = B.Sph(kernel=0)
     st = _alloc(ps, h0)
-    sph.sph_kdk_init(st, ps.mass, kw["dt_max"], kw["n_bins"], kw["n_ngb_target"], kw["n_ngb_tol"])
+    sph.sph_kdk_init(st, ps.mass, kw["dt_max"], kw["n_bins"], kw["n_ngb_target"], kw["n_ngb_tol"], refresh_max=refresh_max,
+                     rebuild_fraction=2.0)
     torch.cuda.synchronize()
     g = _np(st, 0)
     o = K.init(dict(pos=ps.pos, vel=ps.vel, u=ps.u, h=h0), **kw)
