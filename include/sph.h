@@ -278,8 +278,11 @@ int sph_kdk_step(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
  * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
  * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries
  * of inactive particles of the outputs rho..vsig_max are unspecified unless the caller pre-filled the
- * device state through an earlier call), and synchronises.  All pointers are HOST pointers (pinned
- * memory makes the copies asynchronous); `active_host` may be NULL (all active).
+ * device state through an earlier call), and synchronises.  All pointers are HOST pointers;
+ * `active_host` may be NULL (all active).  With PINNED host memory the copies overlap the kernels on a
+ * second stream of the context: h, vel and u go up while the index is built and the density runs, h, rho,
+ * omega and ngb_count come down while the force pass runs; only pos (up) and acc, dudt, vsig_max (down)
+ * are exposed.  With pageable memory the copies are staged by the driver and the call is merely slower.
  */
 int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *vel_host, const float *u_host,
                   float mass_scalar, const int32_t *active_host, int64_t n_active, float n_ngb_target,

@@ -131,6 +131,8 @@ struct sph_ctx {
 
     // phase timing: events recorded on the stream around the phases named in sph_stats
     cudaEvent_t ev[8]; // 0,1 index  2,3 density kernel  4,5 force prep  6,7 force kernel
+    cudaStream_t copy_stream; // sph_step_host: host copies that overlap the kernels (created at first use)
+    cudaEvent_t cev[4];       // sph_step_host: positions up / velocities, energies up / density results final / h up
     bool ev_set[4];
 };
 
