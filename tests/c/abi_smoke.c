@@ -81,6 +81,15 @@ int main(void)
     CHECK(fabs(mean - 1.0) < 0.05);  /* density = m n within the lattice bound */
     CHECK(fabs(px) < 1e-4 * pa);     /* momentum: all active, pair terms antisymmetric */
 
+    /* the same positions through sph_refresh_index: the same tree, hence the same integers */
+    static int32_t ngb2[N];
+    CHECK(sph_refresh_index(ctx, N - 1, d_pos) == SPH_E_ARG);
+    CHECK(sph_refresh_index(ctx, N, d_pos) == SPH_OK);
+    CHECK(cudaMemcpy(d_h, h, sizeof h, cudaMemcpyHostToDevice) == cudaSuccess);
+    CHECK(sph_density(ctx, NULL, -1, 64.f, 2.f, d_h, d_rho, d_om, d_ngb, d_st, &unconv) == SPH_OK && unconv == 0);
+    CHECK(cudaMemcpy(ngb2, d_ngb, sizeof ngb2, cudaMemcpyDeviceToHost) == cudaSuccess);
+    for (int i = 0; i < N; i++) CHECK(ngb2[i] == ngb[i]);
+
     /* a support radius >= box / 2 among the guesses: nothing is computed, SPH_E_HRANGE */
     h[7] = 0.75f;
     CHECK(cudaMemcpy(d_h, h, sizeof h, cudaMemcpyHostToDevice) == cudaSuccess);

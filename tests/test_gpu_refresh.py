@@ -58,6 +58,29 @@ def test_refreshed_index_against_the_oracle(shape, frac):
         x.close()
 
 
+def test_gravity_on_a_refreshed_index():
+    """The tree walk of sph_gravity_short reads the enlarged cells: the opening criterion only gets more conservative, the
+    node moments are recomputed from the new positions."""
+    ps = I.config3(8000, 4)
+    pos1 = _moved(ps, 0.7, 5)
+    kw = dict(G=1.0, r_s=0.03, r_cut=0.135, eps=0.002)
+    g = GpuRun(ps.pos, ps.kernel, ps.mass)
+    g.pos.copy_(torch.from_numpy(pos1))
+    g.sph.sph_refresh_index(g.pos)
+    o = O.gravity_short(pos1, mass_scalar=ps.mass, **kw)
+    amag = np.sqrt((o["acc"] ** 2).sum(1))
+    acc = torch.zeros((ps.n, 3), device="cuda")
+    g.sph.sph_gravity_short(acc, kw["G"], kw["r_s"], kw["r_cut"], kw["eps"], 0.0)
+    a0 = acc.cpu().numpy().astype(np.float64)
+    err = np.sqrt(((a0 - o["acc"]) ** 2).sum(1))
+    tol = 1e-4 * np.maximum(amag, 1e-3 * o["asum"])
+    assert np.all(err <= tol), float(np.max(err / tol))
+    g.sph.sph_gravity_short(acc, kw["G"], kw["r_s"], kw["r_cut"], kw["eps"], 0.5)
+    rel = np.sqrt(((acc.cpu().numpy() - o["acc"]) ** 2).sum(1)) / np.maximum(amag, np.median(amag))
+    assert np.median(rel) < 5e-3 and np.percentile(rel, 99) < 3e-2 and rel.max() < 0.1
+    g.close()
+
+
 def test_refresh_preconditions():
     ps = I.config1(8)
     s = B.Sph(kernel=ps.kernel)
