@@ -24,7 +24,7 @@ struct GravArgs {
     const uint32_t *item_slot;
     uint32_t n_items;
     SphCounters *cnt;
-    float L, G, rs, rcut, eps2, theta2;
+    float L, G, hrs, rcut, rcut2, eps2, theta2;  // hrs = 1 / (2 r_s)
     float *acc;
 };
 
@@ -34,14 +34,19 @@ struct GravWarp {
     uint32_t stack[SPH_STK];
 };
 
-// G m_j * [erfc(r / 2 r_s) + r / (r_s sqrt(pi)) exp(-r^2 / 4 r_s^2)] / (r^2 + eps^2)^(3/2) for r < r_cut, else 0  (R23)
+// G m_j * [erfc(r / 2 r_s) + r / (r_s sqrt(pi)) exp(-r^2 / 4 r_s^2)] / (r^2 + eps^2)^(3/2) for r < r_cut, else 0  (R23).
+// With x = r / 2 r_s the bracket is exp(-x^2) * (P(t) + 2 x / sqrt(pi)), t = 1 / (1 + p x): erfc by the rational
+// approximation 7.1.26 of Abramowitz & Stegun (|error| <= 1.5e-7, i.e. <= 1e-5 of the bracket at x = 2.25 where it is
+// smallest), which shares the exponential with the second term -- one ex2, one rcp and six FMAs instead of erfcf + expf.
 __device__ __forceinline__ float grav_pair(const GravArgs &a, float r2, float m)
 {
-    const float r = sqrtf(r2), x = r * (0.5f / a.rs);
-    const float fac = erfcf(x) + r * (0.5641895835477563f / a.rs) * __expf(-x * x);
     const float s2 = r2 + a.eps2;
     const float ri = rsqrtf(s2);
-    return r2 < a.rcut * a.rcut ? a.G * m * fac * ri * ri * ri : 0.f;
+    const float r = r2 * rsqrtf(fmaxf(r2, 1e-37f)), x = r * a.hrs;
+    const float t = __fdividef(1.f, fmaf(0.3275911f, x, 1.f));
+    const float P = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.061405429f, -1.453152027f), 1.421413741f), -0.284496736f), 0.254829592f);
+    const float fac = __expf(-x * x) * fmaf(1.1283791670955126f, x, P);
+    return r2 < a.rcut2 ? a.G * m * fac * ri * ri * ri : 0.f;
 }
 
 __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
@@ -122,25 +127,40 @@ __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
                 nseg += __popc(me); nmono += __popc(ma); sp += __popc(mp);
                 __syncwarp();
             }
-            // evaluate: lane = (active, stream); the streams split the items
+            // evaluate: lane = (active, stream); the streams split the accepted nodes and the flat sequence of the leaf
+            // runs' particles; 16 terms at a time are summed in fp32, those sums in fp64
             if (live) {
+                float bx = 0.f, by = 0.f, bz = 0.f;
                 for (int i = s; i < nmono; i += f) {
                     const float4 q = W.mono[i];
                     const float ddx = image_diff(pi.x, q.x, L), ddy = image_diff(pi.y, q.y, L), ddz = image_diff(pi.z, q.z, L);
                     const float t = grav_pair(a, fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)), q.w);
-                    ax -= (double)(t * ddx); ay -= (double)(t * ddy); az -= (double)(t * ddz);
+                    bx = fmaf(-t, ddx, bx); by = fmaf(-t, ddy, by); bz = fmaf(-t, ddz, bz);
                 }
-            }
-            for (int k = 0; k < nseg; k++) {
-                const uint32_t b = W.seg_start[k], e = W.seg_end[k];
-                if (live) {
-                    for (uint32_t j = b + s; j < e; j += f) {
+                ax += (double)bx; ay += (double)by; az += (double)bz;
+                bx = by = bz = 0.f;
+                if (nseg > 0) {
+                    int k = 0, since = 0;
+                    uint32_t j = W.seg_start[0] + (uint32_t)s, e = W.seg_end[0];
+                    for (;;) {
+                        while (j >= e && ++k < nseg) { // step over the ends of the runs
+                            j = W.seg_start[k] + (j - e);
+                            e = W.seg_end[k];
+                        }
+                        if (k >= nseg) break;
                         const float4 q = __ldg(a.xyzm + j);
                         const float ddx = image_diff(pi.x, q.x, L), ddy = image_diff(pi.y, q.y, L), ddz = image_diff(pi.z, q.z, L);
                         const float t = j != slot ? grav_pair(a, fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)), q.w) : 0.f;
-                        ax -= (double)(t * ddx); ay -= (double)(t * ddy); az -= (double)(t * ddz);
+                        bx = fmaf(-t, ddx, bx); by = fmaf(-t, ddy, by); bz = fmaf(-t, ddz, bz);
+                        j += (uint32_t)f;
+                        if (++since == 16) { // (fp32 partial sums stay short: DESIGN.md R15's argument for the force pass)
+                            ax += (double)bx; ay += (double)by; az += (double)bz;
+                            bx = by = bz = 0.f;
+                            since = 0;
+                        }
                     }
                 }
+                ax += (double)bx; ay += (double)by; az += (double)bz;
             }
             nseg = nmono = 0;
             __syncwarp();
@@ -206,7 +226,7 @@ int sph_gravity_launch(sph_ctx *ctx, bool subset, int64_t n_items, float G, floa
     a.item_slot = subset ? ctx->act_slot : nullptr;
     a.n_items = (uint32_t)n_items;
     a.cnt = ctx->cnt;
-    a.L = ctx->prm.box; a.G = G; a.rs = r_s; a.rcut = r_cut; a.eps2 = eps * eps; a.theta2 = theta * theta;
+    a.L = ctx->prm.box; a.G = G; a.hrs = 0.5f / r_s; a.rcut = r_cut; a.rcut2 = r_cut * r_cut; a.eps2 = eps * eps; a.theta2 = theta * theta;
     a.acc = acc;
     const size_t dyn = sizeof(GravWarp) * SPH_WARPS;
     SPH_CUDA(ctx, cudaFuncSetAttribute(k_gravity, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn));
