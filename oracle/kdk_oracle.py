@@ -14,6 +14,8 @@ kick-drift-kick integrator of the Gadget lineage [2], restated from its publishe
             drifted v, u of everybody for the force pass: v + a tau, u + du/dt tau, tau = time since the middle of
             the particle's step; active = {i : t1 - tbegin_i == s_i}; density (last h as the guess) and force for the
             active particles; second half kick of the old step, new bin, first half kick of the new step.
+  gravity   (optional, gravity = dict(G, r_s, r_cut, eps)): a_i = hydro force + the short-range gravity of R23 (direct
+            sum) wherever the hydro force is evaluated; the time-step criterion sees the total acceleration.
 
 Only tests/ may import this module; it imports nothing of the CUDA path.
 """
@@ -40,7 +42,17 @@ def new_bin(dt_max, n_bins, courant, eta, H, vsig, acc):
     return np.clip(b, 0, n_bins - 1).astype(np.int32), edge
 
 
-def init(state, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025, box=1.0):
+def _grav(pos32, gravity, mass_scalar, box, active=None):
+    """(acc, asum) of the short-range gravity for the active particles; zeros without gravity."""
+    na = len(pos32) if active is None else len(active)
+    if not gravity:
+        return np.zeros((na, 3)), np.zeros(na)
+    g = O.gravity_short(pos32, G=gravity["G"], r_s=gravity["r_s"], r_cut=gravity["r_cut"], eps=gravity["eps"], box=box,
+                        mass_scalar=mass_scalar, active=active)
+    return g["acc"], g["asum"]
+
+
+def init(state, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025, box=1.0, gravity=None):
     """state: dict with pos (n,3), vel (n,3), u, h (guess) as float arrays.  Returns the full state at tick 0 (fp64)."""
     pos = np.asarray(state["pos"], F32)
     n = len(pos)
@@ -49,6 +61,8 @@ def init(state, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol,
                       d["omega"].astype(F32), kernel=kernel, mass_scalar=mass_scalar, box=box)
     T = 1 << (n_bins - 1)
     delta = dt_max / T
+    ga, _ = _grav(pos, gravity, mass_scalar, box)
+    f["acc"] = f["acc"] + ga
     b, edge = new_bin(dt_max, n_bins, courant, eta, d["H"], f["vsig"], f["acc"])
     hk = 0.5 * (T >> b) * delta
     out = dict(pos=pos.astype(np.float64), vel=np.asarray(state["vel"], np.float64) + f["acc"] * hk[:, None],
@@ -57,7 +71,7 @@ def init(state, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol,
     return out
 
 
-def step(s, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025, box=1.0):
+def step(s, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025, box=1.0, gravity=None):
     """One step from state s (as returned by init/step, or the GPU's state converted to numpy).  Returns the new state
     plus active (ids), vpred, upred, edge (bin decision within 1e-4 of switching, active particles only)."""
     T = 1 << (n_bins - 1)
@@ -87,7 +101,8 @@ def step(s, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, cou
     acc = np.asarray(s["acc"], np.float64).copy()
     dudt = np.asarray(s["dudt"], np.float64).copy()
     vsig = np.asarray(s["vsig"], np.float64).copy()
-    acc[active], dudt[active], vsig[active] = f["acc"], f["dudt"], f["vsig"]
+    ga, gsum = _grav(pos32, gravity, mass_scalar, box, active=active)
+    acc[active], dudt[active], vsig[active] = f["acc"] + ga, f["dudt"], f["vsig"]
     bn, edge = new_bin(dt_max, n_bins, courant, eta, h[active], vsig[active], acc[active])
     bo = b0[active]
     longer = bn < bo
@@ -103,5 +118,5 @@ def step(s, *, kernel, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, cou
     b[active] = bn
     tb[active] = t1
     return dict(pos=pos32.astype(np.float64), vel=vel, u=u, h=h, rho=rho, omega=om, ngb=ngb, acc=acc, dudt=dudt, vsig=vsig, bin=b,
-                tbegin=tb, tick=t1, active=active, vpred=vpred, upred=upred, edge=edge, dens_edge=d["edge"], asum=f["asum"], dusum=f["dusum"],
+                tbegin=tb, tick=t1, active=active, vpred=vpred, upred=upred, edge=edge, dens_edge=d["edge"], asum=f["asum"] + gsum, dusum=f["dusum"],
                 asq=f["asq"], dusq=f["dusq"])

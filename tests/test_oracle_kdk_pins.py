@@ -105,3 +105,57 @@ def test_time_bin_structure():
         assert np.array_equal(s["bin"][inact], b0[inact]) and np.array_equal(s["acc"][inact], s["acc"][inact])
         nact.append(len(a))
     assert min(nact) < ps.n // 2  # most steps update a part of the particles only (the paper's regime)
+
+
+GRAV = dict(G=1.0, r_s=0.05, r_cut=0.225, eps=0.01)
+
+
+def _grav_factor(r, g):
+    """Closed form of R23 for one pair: G fac(r) / (r^2 + eps^2)^(3/2), fac = erfc(r / 2 r_s) + r / (r_s sqrt(pi)) exp(-r^2 / 4 r_s^2)."""
+    x = r / (2 * g["r_s"])
+    return g["G"] * (math.erfc(x) + r / (g["r_s"] * math.sqrt(math.pi)) * math.exp(-x * x)) / (r * r + g["eps"] ** 2) ** 1.5
+
+
+def test_two_bodies_under_gravity_follow_the_leapfrog_by_hand():
+    """Two gas particles outside each other's SPH support but inside r_cut: the only force is the short-range gravity of
+    R23, known in closed form; with one bin the first step is x1 = x0 + v0 dt + a0 dt^2 / 2 exactly."""
+    r = 0.125
+    pos = np.array([[0.5 - r / 2, 0.5, 0.5], [0.5 + r / 2, 0.5, 0.5]], np.float32)
+    st = dict(pos=pos, vel=np.zeros((2, 3), np.float32), u=np.ones(2, np.float32), h=np.full(2, 0.03, np.float32))
+    m, dt = 0.25, 0.0625
+    kw = dict(kernel=0, mass_scalar=m, dt_max=dt, n_bins=1, n_ngb_target=1.0, n_ngb_tol=10.0, gravity=GRAV)
+    s = K.init(st, **kw)
+    a0 = m * _grav_factor(r, GRAV) * r  # towards each other
+    assert abs(s["acc"][0, 0] - a0) < 1e-12 * a0 and abs(s["acc"][1, 0] + a0) < 1e-12 * a0 and np.all(s["acc"][:, 1:] == 0)
+    assert np.all(s["vsig"] == 0) and np.all(s["dudt"] == 0)  # no SPH neighbour
+    s1 = K.step(s, **kw)
+    assert abs(s1["pos"][0, 0] - (pos[0, 0] + 0.5 * a0 * dt * dt)) < 1e-7
+    assert abs(s1["pos"][1, 0] - (pos[1, 0] - 0.5 * a0 * dt * dt)) < 1e-7
+    r1 = float(s1["pos"][1, 0] - s1["pos"][0, 0])
+    a1 = m * _grav_factor(r1, GRAV) * r1
+    assert abs(s1["acc"][0, 0] - a1) < 1e-10 * a1 and a1 > a0  # closer, stronger
+    # without the option nothing pulls
+    s0 = K.init(st, **{**kw, "gravity": None})
+    assert np.all(s0["acc"] == 0)
+
+
+def test_gravity_in_the_driver_conserves_momentum_and_vanishes_on_the_lattice():
+    ps = I.config1(6)
+    rng = np.random.default_rng(4)
+    vel = (0.05 * rng.normal(size=(ps.n, 3))).astype(np.float32)
+    kw = dict(kernel=0, mass_scalar=ps.mass, dt_max=0.01, n_bins=1, n_ngb_target=ps.n_ngb, n_ngb_tol=0.05, gravity=dict(GRAV, G=50.0))
+    s = K.init(dict(pos=ps.pos, vel=vel, u=ps.u, h=ps.h_guess), **kw)
+    s_h = K.init(dict(pos=ps.pos, vel=vel, u=ps.u, h=ps.h_guess), **{**kw, "gravity": None})
+    assert np.abs(s["acc"] - s_h["acc"]).max() > 0.05 * np.abs(s_h["acc"]).max()  # gravity takes part
+    _, p0 = _energy(s, ps.mass, 1, 0.01)
+    for _ in range(3):
+        s = K.step(s, **kw)
+        _, p = _energy(s, ps.mass, 1, 0.01)
+        assert np.all(np.abs(p - p0) < 1e-9 * ps.mass * np.abs(s["vel"]).sum())
+    # perfect lattice: every pair term has its mirror image, gravity cancels like the pressure force does
+    n_side = 8
+    pos = I.perfect_lattice(n_side)
+    n = len(pos)
+    st = dict(pos=pos, vel=np.zeros((n, 3), np.float32), u=np.ones(n, np.float32), h=np.full(n, 1.03 * 2.48232 / n_side, np.float32))
+    s = K.init(st, kernel=0, mass_scalar=1.0 / n, dt_max=0.05, n_bins=6, n_ngb_target=64.0, n_ngb_tol=1e-3, gravity=GRAV)
+    assert np.max(np.abs(s["acc"])) < 1e-9
