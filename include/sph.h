@@ -255,6 +255,9 @@ typedef struct {
     float n_ngb_target, n_ngb_tol;
     int refresh_max;    /* steps in a row that may refresh the index instead of rebuilding it; 0 = always rebuild */
     float rebuild_fraction; /* rebuild whenever n_active >= rebuild_fraction * n (1/16) */
+    /* grav_G > 0: the short-range gravity of sph_gravity_short (same parameters) is added to the hydro acceleration of
+     * the active particles; the time-step criterion sees the sum.  grav_G = 0: hydrodynamics only. */
+    float grav_G, grav_rs, grav_rcut, grav_eps, grav_theta;
 } sph_kdk_params;
 
 typedef struct {

@@ -42,7 +42,8 @@ class SphImprovedParams(C.Structure):
 
 class SphKdkParams(C.Structure):
     _fields_ = [("dt_max", C.c_float), ("n_bins", C.c_int), ("courant", C.c_float), ("eta", C.c_float),
-                ("n_ngb_target", C.c_float), ("n_ngb_tol", C.c_float), ("refresh_max", C.c_int), ("rebuild_fraction", C.c_float)]
+                ("n_ngb_target", C.c_float), ("n_ngb_tol", C.c_float), ("refresh_max", C.c_int), ("rebuild_fraction", C.c_float),
+                ("grav_G", C.c_float), ("grav_rs", C.c_float), ("grav_rcut", C.c_float), ("grav_eps", C.c_float), ("grav_theta", C.c_float)]
 
 
 KDK_F32 = ("pos", "vel", "u", "h", "rho", "omega")
@@ -232,9 +233,11 @@ class Sph:
         return st
 
     def sph_kdk_init(self, state: dict, mass_scalar, dt_max, n_bins, n_ngb_target, n_ngb_tol, courant=0.3, eta=0.025,
-                     refresh_max=16, rebuild_fraction=1.0 / 16):
+                     refresh_max=16, rebuild_fraction=1.0 / 16, gravity=None):
+        """gravity: None or dict(G, r_s, r_cut, eps, theta) -- short-range gravity added to the hydro acceleration."""
         n = state["pos"].shape[0]
-        self._kdk_p = SphKdkParams(dt_max, n_bins, courant, eta, n_ngb_target, n_ngb_tol, refresh_max, rebuild_fraction)
+        self._kdk_p = SphKdkParams(dt_max, n_bins, courant, eta, n_ngb_target, n_ngb_tol, refresh_max, rebuild_fraction,
+                                   *([gravity[k] for k in ("G", "r_s", "r_cut", "eps", "theta")] if gravity else [0.0] * 5))
         st = self._kdk_state(state, n)
         self._check(self._lib.sph_kdk_init(self._h, n, float(mass_scalar), C.byref(self._kdk_p), C.byref(st)), allow=(SPH_OK, SPH_W_NOCONV))
         self.n = n

@@ -114,7 +114,7 @@ int sph_destroy(sph_ctx *ctx)
     dfree(ctx->keys); dfree(ctx->keys_alt); dfree(ctx->perm); dfree(ctx->perm_alt); dfree(ctx->inv);
     dfree(ctx->xyzm); dfree(ctx->nodes); dfree(ctx->grp_mark); dfree(ctx->gid_of_slot); dfree(ctx->slot_leaf); dfree(ctx->grp_start);
     dfree(ctx->cnt); dfree(ctx->sort_hist); dfree(ctx->scan_bsum); dfree(ctx->f_xyzh); dfree(ctx->f_vc); dfree(ctx->f_ext);
-    dfree(ctx->node_hmax); dfree(ctx->node_slack); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
+    dfree(ctx->node_hmax); dfree(ctx->node_slack); dfree(ctx->kdk_grav); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
     dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);

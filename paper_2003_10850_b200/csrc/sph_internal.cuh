@@ -112,6 +112,8 @@ struct sph_ctx {
     float4 *f_xyzh, *f_vc, *f_ext; // f_ext: improved-SPH record (alpha, f, u), allocated on first use
     float *node_hmax;
     bool act_keep;        // sph_active_groups: keep the groups of the last call (set by sph_kdk_step / sph_step_* between density and force)
+    float *kdk_grav;      // sph_kdk_*: gravity of the active particles before it is added to acc
+    int64_t kdk_grav_cap;
     int kdk_refreshed;    // steps of sph_kdk_step since the last full build
     float *node_slack;    // sph_refresh_index: how far particles have left their cells (per node)
     float4 *node_mom;     // short-range gravity: centre of mass and mass of every node (allocated on first use)

@@ -101,6 +101,17 @@ __global__ void k_kdk_close_open(int64_t na, KdkConst k, int t1, const int32_t *
     tbegin[i] = t1;
 }
 
+// acc += gravity for the listed particles (active == NULL: all)
+__global__ void k_kdk_add_gravity(int64_t na, const int32_t *__restrict__ active, const float *__restrict__ grav, float *__restrict__ acc)
+{
+    const int64_t kk = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (kk >= na) return;
+    const int64_t i = active ? active[kk] : kk;
+    acc[3 * i] += grav[3 * i];
+    acc[3 * i + 1] += grav[3 * i + 1];
+    acc[3 * i + 2] += grav[3 * i + 2];
+}
+
 __global__ void k_kdk_bmax(int64_t n, const int32_t *__restrict__ bin, unsigned int *bmax)
 {
     unsigned int m = 0;
@@ -121,6 +132,8 @@ int check(sph_ctx *ctx, int64_t n, const sph_kdk_params *p, const sph_kdk_state 
     if (!(p->dt_max > 0.f) || p->n_bins < 1 || p->n_bins > 24 || !(p->courant > 0.f) || !(p->eta > 0.f) || !(p->n_ngb_target > 0.f) ||
         !(p->n_ngb_tol >= 0.f))
         return sph_fail(ctx, SPH_E_ARG, "sph_kdk: bad sph_kdk_params");
+    if (p->grav_G < 0.f || (p->grav_G > 0.f && (!(p->grav_rs > 0.f) || !(p->grav_rcut > 0.f) || !(p->grav_eps >= 0.f) || !(p->grav_theta >= 0.f))))
+        return sph_fail(ctx, SPH_E_ARG, "sph_kdk: bad gravity parameters in sph_kdk_params");
     if (n > 0 && (!s->pos || !s->vel || !s->u || !s->h || !s->rho || !s->omega || !s->ngb || !s->acc || !s->dudt || !s->vsig ||
                   !s->vpred || !s->upred || !s->bin || !s->tbegin || !s->active))
         return sph_fail(ctx, SPH_E_ARG, "sph_kdk: NULL array in sph_kdk_state");
@@ -131,6 +144,27 @@ int check(sph_ctx *ctx, int64_t n, const sph_kdk_params *p, const sph_kdk_state 
     k.dt_max = p->dt_max;
     k.courant = p->courant;
     k.eta = p->eta;
+    return SPH_OK;
+}
+
+// short-range gravity of the listed particles added to their hydro acceleration (grav_G > 0); the active groups of the
+// density pass are still valid (act_keep set by the caller)
+int add_gravity(sph_ctx *ctx, int64_t n, const sph_kdk_params *p, const sph_kdk_state *s, const int32_t *active, int64_t na)
+{
+    if (!(p->grav_G > 0.f)) return SPH_OK;
+    int rc;
+    if (ctx->kdk_grav_cap < n) {
+        ctx->kdk_grav_cap = 0;
+        if (ctx->kdk_grav) cudaFree(ctx->kdk_grav);
+        ctx->kdk_grav = nullptr;
+        SPH_CUDA(ctx, cudaMalloc((void **)&ctx->kdk_grav, sizeof(float) * 3 * (size_t)n));
+        ctx->kdk_grav_cap = n;
+    }
+    if ((rc = sph_gravity_short(ctx, active, active ? na : -1, p->grav_G, p->grav_rs, p->grav_rcut, p->grav_eps, p->grav_theta, ctx->kdk_grav)))
+        return rc;
+    const int64_t cnt = active ? na : n;
+    if (cnt > 0) k_kdk_add_gravity<<<(int)((cnt + 255) / 256), 256, 0, ctx->stream>>>(cnt, active, ctx->kdk_grav, s->acc);
+    ctx->launches++;
     return SPH_OK;
 }
 
@@ -156,6 +190,7 @@ int sph_kdk_init(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
     if (rc != SPH_OK && rc != SPH_W_NOCONV) return rc;
     const int rcd = rc;
     if ((rc = sph_hydro_force(ctx, nullptr, -1, s->vel, s->u, s->h, s->rho, s->omega, s->acc, s->dudt, s->vsig))) return rc;
+    if ((rc = add_gravity(ctx, n, p, s, nullptr, n))) return rc;
     SPH_CUDA(ctx, cudaMemsetAsync(&ctx->cnt->work, 0, sizeof(unsigned int), st)); // (reused as the bin maximum between calls of the gather kernels)
     k_kdk_open_all<<<G, T, 0, st>>>(n, k, s->h, s->vsig, s->acc, s->dudt, s->vel, s->u, s->bin, s->tbegin, &ctx->cnt->work);
     ctx->launches++;
@@ -210,6 +245,7 @@ int sph_kdk_step(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
     ctx->act_keep = true; // the same active list: its groups are those of the density pass
     rc = sph_hydro_force(ctx, all ? nullptr : s->active, all ? -1 : (int64_t)na, s->vpred, s->upred, s->h, s->rho, s->omega, s->acc, s->dudt,
                          s->vsig);
+    if (!rc) rc = add_gravity(ctx, n, p, s, all ? nullptr : s->active, (int64_t)na);
     ctx->act_keep = false;
     if (rc) return rc;
     if (all) k_iota<<<G, T, 0, st>>>(n, s->active);

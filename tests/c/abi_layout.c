@@ -24,6 +24,7 @@ int main(void)
     printf("sph_kdk_params %zu\n", sizeof(sph_kdk_params));
     F(sph_kdk_params, dt_max); F(sph_kdk_params, n_bins); F(sph_kdk_params, courant); F(sph_kdk_params, eta);
     F(sph_kdk_params, n_ngb_target); F(sph_kdk_params, n_ngb_tol); F(sph_kdk_params, refresh_max); F(sph_kdk_params, rebuild_fraction);
+    F(sph_kdk_params, grav_G); F(sph_kdk_params, grav_rs); F(sph_kdk_params, grav_rcut); F(sph_kdk_params, grav_eps); F(sph_kdk_params, grav_theta);
     printf("sph_kdk_state %zu\n", sizeof(sph_kdk_state));
     F(sph_kdk_state, pos); F(sph_kdk_state, vel); F(sph_kdk_state, u); F(sph_kdk_state, h); F(sph_kdk_state, rho);
     F(sph_kdk_state, omega); F(sph_kdk_state, ngb); F(sph_kdk_state, acc); F(sph_kdk_state, dudt); F(sph_kdk_state, vsig);

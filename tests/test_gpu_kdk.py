@@ -37,8 +37,13 @@ def _close(a, b, rtol, scale, what):
 
 # refresh_max = 0: an index build every step; 4 with rebuild_fraction 2: four refreshed steps (sph_refresh_index: the old
 # tree with enlarged cells), then a rebuild, whatever the number of active particles -- the same results either way
-@pytest.mark.parametrize("shape,refresh_max", [("C1", 0), ("C1", 4), ("C3", 0), ("C3", 4)])
-def test_kdk_driver_in_lock_step_with_the_oracle(shape, refresh_max):
+# gravity: the short-range gravity of R23 added to the hydro acceleration (opening angle 0: the oracle's direct sum)
+GRAV = dict(G=2.0, r_s=0.02, r_cut=0.09, eps=0.002, theta=0.0)
+
+
+@pytest.mark.parametrize("shape,refresh_max,gravity", [("C1", 0, None), ("C1", 4, None), ("C3", 0, None), ("C3", 4, None), ("C3", 4, GRAV),
+                                                       ("C1", 0, GRAV)])
+def test_kdk_driver_in_lock_step_with_the_oracle(shape, refresh_max, gravity):
     if shape == "C1":
         ps = I.config1(12)
         rng = np.random.default_rng(9)
@@ -53,12 +58,18 @@ def test_kdk_driver_in_lock_step_with_the_oracle(shape, refresh_max):
     sph = B.Sph(kernel=0)
     st = _alloc(ps, h0)
     sph.sph_kdk_init(st, ps.mass, kw["dt_max"], kw["n_bins"], kw["n_ngb_target"], kw["n_ngb_tol"], refresh_max=refresh_max,
-                     rebuild_fraction=2.0)
+                     rebuild_fraction=2.0, gravity=gravity)
+    if gravity:
+        kw["gravity"] = {k: gravity[k] for k in ("G", "r_s", "r_cut", "eps")}
     torch.cuda.synchronize()
     g = _np(st, 0)
     o = K.init(dict(pos=ps.pos, vel=ps.vel, u=ps.u, h=h0), **kw)
     ok = ~o["edge"]
     assert np.array_equal(g["bin"][ok], o["bin"][ok]) and o["edge"].mean() < 0.01
+    if gravity:  # gravity really takes part: the accelerations are those of the oracle with gravity, not without
+        o0 = K.init(dict(pos=ps.pos, vel=ps.vel, u=ps.u, h=h0), **{**kw, "gravity": None})
+        amax = np.abs(o["acc"]).max()
+        assert np.abs(g["acc"] - o0["acc"]).max() > 1e-2 * amax and np.abs(g["acc"] - o["acc"]).max() < 1e-4 * amax
     vs = np.abs(o["vel"]).max()
     _close(g["vel"], o["vel"], 2e-4, 1e-3 * vs, "init vel")
     _close(g["u"], o["u"], 1e-4, 1e-3, "init u")
