@@ -4,7 +4,7 @@
 // The paper keeps its particles in space-filling-curve order (§1); here that order is
 // produced on the device by sorting the 48-bit Morton keys.  One pass per 8-bit digit, three kernels per
 // pass -- (1) per-tile digit histograms, (2) an exclusive scan of the histogram matrix, (3) a scatter that
-// ranks the tile's keys stably (warp-wide match on the digit), orders the tile in shared memory and
+// ranks the tile's keys stably (warp-wide ballots on the digit bits), orders the tile in shared memory and
 // writes every digit's run of the tile to its place as one contiguous, coalesced piece.  HBM-bound:
 // a pass reads the keys twice and the values once and writes both once (32 bytes per record).
 #include "sph_internal.cuh"
@@ -142,11 +142,29 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINB) k_sort_scatter(const 
         key[r] = valid ? kin[t0 + o] : (K)0;
         if (HAS_VAL) val[r] = valid ? vin[t0 + o] : 0u;
     }
+    // the lanes holding the same digit, from eight ballots (one per digit bit) -- measured faster than __match_any_sync
+    // here (index build 1.54 instead of 1.63 ms at 10^7 keys: the match instruction's latency dominated the kernel);
+    // all rounds' masks are computed before the first counter update, which is ordered through shared memory
+    unsigned mm[SORT_ROUNDS];
 #pragma unroll
     for (int r = 0; r < SORT_ROUNDS; r++) {
         const bool valid = w0 + r * 32 + lane < tn;
-        const uint32_t d = valid ? digit_of(key[r], shift, mask) : 0xffffffffu; // (invalid lanes match one another only)
-        const unsigned m = __match_any_sync(FULL, d);
+        const uint32_t d = valid ? digit_of(key[r], shift, mask) : 0u;
+        const unsigned vm = __ballot_sync(FULL, valid);
+        unsigned m = valid ? vm : ~vm; // (invalid lanes match one another only)
+#pragma unroll
+        for (int b = 0; b < 8; b++) {
+            const bool bit = (d >> b) & 1u;
+            const unsigned bb = __ballot_sync(FULL, bit);
+            m &= bit ? bb : ~bb;
+        }
+        mm[r] = m;
+    }
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; r++) {
+        const bool valid = w0 + r * 32 + lane < tn;
+        const uint32_t d = valid ? digit_of(key[r], shift, mask) : 0xffffffffu;
+        const unsigned m = mm[r];
         const int leader = __ffs(m) - 1;
         uint32_t old = 0;
         if (lane == leader && valid) {
