@@ -60,27 +60,31 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort_scan(uint32_t *__restrict
     __shared__ bool last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     uint32_t *row = hist + (size_t)blockIdx.x * tiles;
-    const uint32_t per = (tiles + SORT_THREADS - 1) / SORT_THREADS, i0 = tid * per, i1 = min(i0 + per, tiles);
+    // warp w owns a contiguous piece of the row and walks it 32 entries at a time (coalesced): first its sum ...
+    const uint32_t per = ((tiles + SORT_WARPS - 1) / SORT_WARPS + 31u) & ~31u, i0 = warp * per, i1 = min(i0 + per, tiles);
     uint32_t s = 0;
-    for (uint32_t i = i0; i < i1; i++) s += row[i];
-    uint32_t inc = s;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(FULL, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) wt[warp] = inc;
+    for (uint32_t i = i0 + lane; i < i1; i += 32) s += row[i];
+    s = __reduce_add_sync(FULL, s);
+    if (lane == 0) wt[warp] = s;
     __syncthreads();
-    uint32_t run = inc - s, all = 0;
+    uint32_t run = 0, all = 0;
 #pragma unroll
     for (int w = 0; w < SORT_WARPS; w++) {
         run += w < warp ? wt[w] : 0u;
         all += wt[w];
     }
-    for (uint32_t i = i0; i < i1; i++) {
-        const uint32_t v = row[i];
-        row[i] = run;
-        run += v;
+    // ... then the exclusive prefix, chunk by chunk with a running carry
+    for (uint32_t b = i0; b < i1; b += 32) {
+        const uint32_t i = b + lane;
+        const uint32_t v = i < i1 ? row[i] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(FULL, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (i < i1) row[i] = run + inc - v;
+        run += __shfl_sync(FULL, inc, 31);
     }
     if (tid == 0) {
         tot[blockIdx.x] = all;
