@@ -132,10 +132,9 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINB) k_sort_scatter(const 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tile = blockIdx.x, t0 = tile * SORT_TILE;
     const uint32_t tn = min((uint32_t)SORT_TILE, n - t0);
-    for (int i = tid; i < SORT_WARPS * SORT_RADIX; i += SORT_THREADS) (&S.wcnt[0][0])[i] = 0;
-    __syncthreads();
     // rank inside the warp's chunk: the chunk is SORT_ROUNDS consecutive rows of 32 keys, row by row, lane by lane --
-    // the order of the input, so equal digits keep their order (stable)
+    // the order of the input, so equal digits keep their order (stable).  (All global loads of the block are issued
+    // first, so that their latency overlaps the clearing of the counters.)
     K key[SORT_ROUNDS];
     uint32_t val[SORT_ROUNDS], rank[SORT_ROUNDS];
     const uint32_t w0 = warp * (32 * SORT_ROUNDS);
@@ -146,6 +145,9 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINB) k_sort_scatter(const 
         key[r] = valid ? kin[t0 + o] : (K)0;
         if (HAS_VAL) val[r] = valid ? vin[t0 + o] : 0u;
     }
+    const uint32_t gbase = base[tid] + hist[(size_t)tid * tiles + tile]; // where this tile's run of digit tid starts
+    for (int i = tid; i < SORT_WARPS * SORT_RADIX; i += SORT_THREADS) (&S.wcnt[0][0])[i] = 0;
+    __syncthreads();
     // the lanes holding the same digit, from eight ballots (one per digit bit) -- measured faster than __match_any_sync
     // here (index build 1.54 instead of 1.63 ms at 10^7 keys: the match instruction's latency dominated the kernel);
     // all rounds' masks are computed before the first counter update, which is ordered through shared memory
@@ -204,7 +206,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINB) k_sort_scatter(const 
         for (int w = 0; w < SORT_WARPS; w++) wb += w < warp ? wtot[w] : 0u;
         const uint32_t off = wb + inc - acc;
         S.toff[tid] = off;
-        S.gpos[tid] = base[tid] + hist[(size_t)tid * tiles + tile] - off;
+        S.gpos[tid] = gbase - off;
     }
     __syncthreads();
     // order the tile in shared memory
