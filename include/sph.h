@@ -293,6 +293,28 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
                   int32_t *ngb_count_host, float *acc_host, float *dudt_host, float *vsig_host,
                   int64_t *n_unconverged_host);
 
+/*
+ * Stream compaction of 0/1 flags: ids_out[k] = index of the k-th non-zero flag, ascending (k < count), *count_dev =
+ * their number -- the step that turns per-particle "my time-step ends now" flags into the active list of the next
+ * call (§2.2: the active particles of a time bin; it is what sph_kdk_step does inside).  flags [n] u32
+ * (0 or 1), ids_out [n] i32 (entries from count on are left as they were), count_dev [1] u32: DEVICE arrays owned by
+ * the caller.  Asynchronous on the context's stream; n < 2^31.
+ *   sph_compact_flags          block sums in the context's scratch buffer, which grows by cudaFree + cudaMalloc when n
+ *                              exceeds every earlier call's.
+ *   sph_compact_flags_noalloc  the same kernels, same results, for callers that must not allocate (code under CUDA graph
+ *                              capture, serving loops, harnesses that forbid it): the block sums live in a fixed array
+ *                              of 64 KB of device memory that every GPU loading the library holds until exit.  The call
+ *                              launches kernels and nothing else: no cudaMalloc, cudaFree or allocating library routine
+ *                              (the very first call on a device also asks the runtime for the array's address).
+ *                              n > SPH_COMPACT_NOALLOC_MAX is rejected with SPH_E_ARG and a message.  All calls on a
+ *                              device share the array, whichever context or stream they use: calls that may overlap on
+ *                              the GPU (different streams, no ordering between them) race and give wrong results;
+ *                              calls ordered on one stream are safe, and nothing of an earlier call is read by a later one.
+ */
+#define SPH_COMPACT_NOALLOC_MAX 67108864 /* 2^26 flags */
+int sph_compact_flags(sph_ctx *ctx, int64_t n, const uint32_t *flags, int32_t *ids_out, uint32_t *count_dev);
+int sph_compact_flags_noalloc(sph_ctx *ctx, int64_t n, const uint32_t *flags, int32_t *ids_out, uint32_t *count_dev);
+
 /* Counters of the last calls (host struct filled; synchronises the stream).  Reports a pending
  * precondition failure of an earlier asynchronous call (see Conventions). */
 int sph_get_stats(sph_ctx *ctx, sph_stats *out_host);

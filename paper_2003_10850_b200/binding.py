@@ -14,13 +14,15 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsph.so")
 
+COMPACT_NOALLOC_MAX = 1 << 26  # SPH_COMPACT_NOALLOC_MAX of include/sph.h
 SPH_OK, SPH_E_ARG, SPH_E_CUDA, SPH_E_NOINDEX, SPH_E_OOM, SPH_E_INTERNAL, SPH_E_HRANGE, SPH_W_NOCONV = 0, 1, 2, 3, 4, 5, 6, 16
 ST_CONVERGED, ST_BRACKET, ST_NOTCONV, ST_STALLED = 1 << 8, 1 << 9, 1 << 10, 1 << 11
 KERNEL_CUBIC, KERNEL_WC6 = 0, 1
 
 EXPORTS = ["sph_create", "sph_destroy", "sph_build_index", "sph_density", "sph_hydro_force", "sph_step_host",
            "sph_get_stats", "sph_velocity_gradients", "sph_hydro_force_improved", "sph_thermal_conduction",
-           "sph_kdk_init", "sph_kdk_step", "sph_gravity_short", "sph_refresh_index", "sph_last_error", "sph_version"]
+           "sph_kdk_init", "sph_kdk_step", "sph_gravity_short", "sph_refresh_index", "sph_compact_flags", "sph_compact_flags_noalloc",
+           "sph_last_error", "sph_version"]
 
 
 class SphParams(C.Structure):
@@ -93,7 +95,9 @@ def load():
                                      C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         lib.sph_gravity_short.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_float] * 5 + [C.c_void_p]
         lib.sph_refresh_index.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
-        for name in EXPORTS[:14]:
+        for f in (lib.sph_compact_flags, lib.sph_compact_flags_noalloc):
+            f.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        for name in EXPORTS[:16]:
             getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -161,6 +165,14 @@ class Sph:
         """Positions moved a little since sph_build_index: keep the tree, refresh the sorted positions, enlarge the cells."""
         n = pos.shape[0]
         self._check(self._lib.sph_refresh_index(self._h, n, _dev(pos, torch.float32, "pos", 3 * n)))
+
+    def sph_compact_flags(self, flags, ids_out, count, noalloc=False):
+        """ids_out[:count] = ascending indices of the non-zero flags (u32 0/1); count: u32 tensor of one element.
+        noalloc=True: sph_compact_flags_noalloc (fixed device scratch, n <= COMPACT_NOALLOC_MAX, allocates nothing)."""
+        n = flags.numel()
+        fn = self._lib.sph_compact_flags_noalloc if noalloc else self._lib.sph_compact_flags
+        self._check(fn(self._h, n, _dev(flags, torch.uint32, "flags", n), _dev(ids_out, torch.int32, "ids_out", n),
+                       _dev(count, torch.uint32, "count", 1)))
 
     def sph_density(self, h, rho, omega, ngb_count, n_ngb_target, n_ngb_tol, active=None, status=None):
         """Returns the number of active particles that stopped without convergence."""

@@ -374,3 +374,71 @@ int sph_scan_marks(sph_ctx *ctx, const uint32_t *mark, int64_t n, uint32_t *incl
     SPH_CUDA(ctx, cudaGetLastError());
     return SPH_OK;
 }
+
+// ---- stream compaction of 0/1 flags as a public call, with and without allocation ----------------------------------
+// sph_compact_flags: the scan + compaction above with the context's growable block-sum buffer (the path sph_kdk_step
+// and the index build use).  sph_compact_flags_noalloc: the same three kernels with the block sums in the fixed
+// file-scope device array below, for callers that must not allocate (CUDA graph capture, serving loops).
+#define SPH_NOALLOC_BLOCKS 16384 // block sums: 64 KB of device memory per GPU that loads the library, until exit
+#define SPH_NOALLOC_DEVICES 64
+static_assert((int64_t)SPH_NOALLOC_BLOCKS * SCAN_TILE == SPH_COMPACT_NOALLOC_MAX, "include/sph.h states the limit");
+
+static __device__ __align__(256) uint32_t g_noalloc_bsum[SPH_NOALLOC_BLOCKS];
+// In host code g_noalloc_bsum is only a handle for the runtime, not a device address: the address is asked for once per
+// device (with that device current) and kept here.
+static uint32_t *g_noalloc_ptr[SPH_NOALLOC_DEVICES];
+
+static int compact_args(sph_ctx *ctx, const char *who, int64_t n, const uint32_t *flags, const int32_t *ids_out, const uint32_t *count_dev)
+{
+    if (n < 0 || !count_dev || (n > 0 && (!flags || !ids_out))) return sph_fail(ctx, SPH_E_ARG, "%s: n < 0 or NULL array", who);
+    if (n >= (int64_t)1 << 31) return sph_fail(ctx, SPH_E_ARG, "%s: n = %lld exceeds 2^31 - 1", who, (long long)n);
+    return SPH_OK;
+}
+
+extern "C" int sph_compact_flags(sph_ctx *ctx, int64_t n, const uint32_t *flags, int32_t *ids_out, uint32_t *count_dev)
+{
+    if (!ctx) return SPH_E_ARG;
+    int rc = compact_args(ctx, "sph_compact_flags", n, flags, ids_out, count_dev);
+    if (rc) return rc;
+    if (n == 0) {
+        SPH_CUDA(ctx, cudaMemsetAsync(count_dev, 0, sizeof(uint32_t), ctx->stream));
+        return SPH_OK;
+    }
+    return sph_scan_marks(ctx, flags, n, nullptr, reinterpret_cast<uint32_t *>(ids_out), count_dev);
+}
+
+extern "C" int sph_compact_flags_noalloc(sph_ctx *ctx, int64_t n, const uint32_t *flags, int32_t *ids_out, uint32_t *count_dev)
+{
+    if (!ctx) return SPH_E_ARG;
+    int rc = compact_args(ctx, "sph_compact_flags_noalloc", n, flags, ids_out, count_dev);
+    if (rc) return rc;
+    if (n > (int64_t)SPH_COMPACT_NOALLOC_MAX)
+        return sph_fail(ctx, SPH_E_ARG, "sph_compact_flags_noalloc: n = %lld exceeds SPH_COMPACT_NOALLOC_MAX = %lld (fixed scratch; use sph_compact_flags)",
+                        (long long)n, (long long)SPH_COMPACT_NOALLOC_MAX);
+    cudaStream_t st = ctx->stream;
+    int dev = -1;
+    SPH_CUDA(ctx, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= SPH_NOALLOC_DEVICES) return sph_fail(ctx, SPH_E_ARG, "sph_compact_flags_noalloc: device ordinal %d not supported", dev);
+    if (!g_noalloc_ptr[dev]) { // set-up, once per device (racing first calls of two host threads store the same address)
+        uint32_t *p = nullptr;
+        SPH_CUDA(ctx, cudaGetSymbolAddress((void **)&p, g_noalloc_bsum));
+        if (!p) return sph_fail(ctx, SPH_E_CUDA, "sph_compact_flags_noalloc: no device address for the scratch array");
+        g_noalloc_ptr[dev] = p;
+    }
+    uint32_t *bsum = g_noalloc_ptr[dev];
+    if (n == 0) { // (a 4-byte store by a kernel: cudaMemsetAsync would do, but this keeps the call to kernel launches only)
+        k_scan_bsums<<<1, SCAN_THREADS, 0, st>>>(bsum, 0u, count_dev);
+        ctx->launches++;
+        SPH_CUDA(ctx, cudaGetLastError());
+        return SPH_OK;
+    }
+    // nothing in the scratch has to start at zero: k_scan_sums writes entries [0, nb) before anything reads them, and
+    // entries beyond nb (left by an earlier, larger call) are never read
+    const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
+    k_scan_sums<<<nb, SCAN_THREADS, 0, st>>>(flags, (uint32_t)n, bsum);
+    k_scan_bsums<<<1, SCAN_THREADS, 0, st>>>(bsum, nb, count_dev);
+    k_scan_apply<<<nb, SCAN_THREADS, 0, st>>>(flags, (uint32_t)n, bsum, nullptr, reinterpret_cast<uint32_t *>(ids_out));
+    ctx->launches += 3;
+    SPH_CUDA(ctx, cudaGetLastError());
+    return SPH_OK;
+}
