@@ -206,8 +206,8 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
     const float yf = PAIRWRAP ? A.yi : recentre(A.yi, fr.thy, L);
     const float zf = PAIRWRAP ? A.zi : recentre(A.zi, fr.thz, L);
     const float2 nx = make_float2(-xf, -xf), ny = make_float2(-yf, -yf), nz = make_float2(-zf, -zf);
-    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP) {
-        const int nt = min(SPH_QSTEP, steps - t0);
+    for (int t0 = 0; t0 < steps; t0 += SPH_QSTEP_FORCE) {
+        const int nt = min(SPH_QSTEP_FORCE, steps - t0);
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
         if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);

@@ -39,7 +39,11 @@
 #define SPH_QCAP 32         // per-lane hit-queue entries (>= 2 * SPH_QSTEP)
 #endif
 #ifndef SPH_QCAP_FORCE
-#define SPH_QCAP_FORCE 32   // the same for the force kernel (a hit costs ~95 instructions there: fuller drains pay)
+#define SPH_QCAP_FORCE 48   // the same for the force kernel (a hit costs ~95 instructions there: fuller drains pay;
+                            // measured at C4: 32 -> 75.1 ms, 44 -> 73.0, 48 -> 72.8, 52 -> 72.7, 64 (4 CTAs per SM) -> 83.0)
+#endif
+#ifndef SPH_QSTEP_FORCE
+#define SPH_QSTEP_FORCE 15  // the same for the force kernel (12 and 20 measured equal or slower)
 #endif
 #ifndef SPH_QSTEP
 #define SPH_QSTEP 15        // candidate-pair steps (2 tests each) between queue-capacity checks
