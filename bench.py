@@ -340,6 +340,24 @@ def main():
     its = (stt & 0xff) if active is None else (stt.index_select(0, active.long()) & 0xff)
     eval_hist = torch.bincount(its.long(), minlength=2).cpu().tolist()
     launches = per[-1]["launches"] - l0
+    # active-subset workloads: the same step with sph_refresh_index in place of sph_build_index (what sph_kdk_step does on
+    # steps with few active particles), outside the timed region; `value` stays the rebuild step's
+    refresh_step = None
+    if active is not None:
+        k = max(3, min(args.steps, 50))
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for rep in range(2):  # first round warms up
+            r0.record(stream)
+            for _ in range(k):
+                h.index_copy_(0, active.long(), h_guess.index_select(0, active.long()))
+                sph.sph_refresh_index(pos)
+                sph.sph_density(h, rho, om, ngb, ps.n_ngb, ps.n_tol, active=active)
+                sph.sph_hydro_force(vel, u, h, rho, om, acc, du, vs, active=active)
+            r1.record(stream)
+            torch.cuda.synchronize()
+        refresh_step = {"ms_per_step": r0.elapsed_time(r1) / k, "steps": k,
+                        "step": "sph_refresh_index + sph_density(h iteration) + sph_hydro_force",
+                        "updates_per_s": n_active * k / (r0.elapsed_time(r1) * 1e-3)}
     # improved-SPH extension, outside the timed region: cost of the velocity-gradient pass and of the
     # force pass with per-particle alpha, shear limiter and conduction on the same converged state (CUDA events)
     ext_ms = None
@@ -477,7 +495,7 @@ def main():
             "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
             "e2e": e2e, "gpu_launches": int(launches), "roofline": roof,
             "phases_ms": {"index": ti, "density_kernel": tk, "force_prep": tp, "force_kernel": tf},
-            "improved_sph_extension_ms": ext_ms, "kdk_driver": kdk,
+            "improved_sph_extension_ms": ext_ms, "kdk_driver": kdk, "refresh_step": refresh_step,
             "pairs": {"density_evals_per_particle": st["dens_evals"] / n_active,
                       "density_true_pairs": st["dens_pairs"], "density_candidates": st["dens_candidates"],
                       "force_true_pairs": st["force_pairs"], "force_candidates": st["force_candidates"],
