@@ -52,6 +52,29 @@ def test_gravity_against_direct_summation(shape):
     g.close()
 
 
+def test_gravity_with_particle_masses():
+    """Per-particle masses (a factor 30 between the lightest and the heaviest): the node moments weight the centres of mass,
+    the direct sum of the oracle weights every pair term."""
+    ps = I.config3(6000, 3)
+    n = ps.n
+    rng = np.random.default_rng(12)
+    m = (ps.mass * np.exp(rng.uniform(-1.7, 1.7, n))).astype(np.float32)
+    kw = dict(G=1.0, r_s=0.03, r_cut=0.135, eps=0.002)
+    o = O.gravity_short(ps.pos, mass=m, **kw)
+    g = GpuRun(ps.pos, ps.kernel, 1.0, mass=m)
+    amag = np.sqrt((o["acc"] ** 2).sum(1))
+    a0 = _run(g, n, 0.0, **kw)
+    err = np.sqrt(((a0 - o["acc"]) ** 2).sum(1))
+    tol = 1e-4 * np.maximum(amag, 1e-3 * o["asum"])
+    assert np.all(err <= tol), float(np.max(err / tol))
+    mom = (m[:, None].astype(np.float64) * a0).sum(0)  # total momentum change: pair terms m_i m_j antisymmetric
+    assert np.all(np.abs(mom) < 1e-5 * (m[:, None] * np.abs(a0)).sum(0))
+    a5 = _run(g, n, 0.5, **kw)
+    rel = np.sqrt(((a5 - o["acc"]) ** 2).sum(1)) / np.maximum(amag, np.median(amag))
+    assert np.median(rel) < 5e-3 and np.percentile(rel, 99) < 3e-2 and rel.max() < 0.15, (np.median(rel), np.percentile(rel, 99), rel.max())
+    g.close()
+
+
 def test_gravity_argument_checks():
     from paper_2003_10850_b200 import binding as B
 
