@@ -85,6 +85,30 @@ def make_workload(name: str, n: int | None):
     return ps
 
 
+def sfc_order(ps, active_np):
+    """--sfc-order: the same particle set handed over in space-filling-curve order of the positions (the paper keeps its
+    particles in Hilbert order; here a 3 x 16-bit Morton order), instead of the generator's order.  Only the
+    order of the caller's arrays changes: the gathers / scatters between caller order and the library's sorted order
+    become nearly sequential."""
+    def spread(v):
+        v = v.astype(np.uint64)
+        v = (v | (v << 32)) & np.uint64(0x1F00000000FFFF)
+        v = (v | (v << 16)) & np.uint64(0x1F0000FF0000FF)
+        v = (v | (v << 8)) & np.uint64(0x100F00F00F00F00F)
+        v = (v | (v << 4)) & np.uint64(0x10C30C30C30C30C3)
+        v = (v | (v << 2)) & np.uint64(0x1249249249249249)
+        return v
+    c = np.minimum((ps.pos.astype(np.float64) / ps.box * 65536.0).astype(np.int64), 65535)
+    key = spread(c[:, 0]) | (spread(c[:, 1]) << np.uint64(1)) | (spread(c[:, 2]) << np.uint64(2))
+    order = np.argsort(key, kind="stable")
+    ps.pos, ps.vel, ps.u, ps.h_guess = ps.pos[order], ps.vel[order], ps.u[order], ps.h_guess[order]
+    if active_np is not None:
+        inv = np.empty(len(order), np.int64)
+        inv[order] = np.arange(len(order))
+        active_np = np.sort(inv[active_np]).astype(np.int32)
+    return active_np
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
 
@@ -199,7 +223,8 @@ def workload_config(args, ps, active):
     names = {"C1": "configs[0]", "C2": "configs[1]", "C3": "configs[2]", "C4": "configs[3]", "C5": "configs[4]"}
     w = args.workload.upper()
     return {
-        "workload": f"{w} = BASELINE.json {names[w]}" + ("" if args.n is None else f" scaled to n={ps.n}"),
+        "workload": f"{w} = BASELINE.json {names[w]}" + ("" if args.n is None else f" scaled to n={ps.n}")
+                    + (" (caller arrays in Morton order: --sfc-order)" if getattr(args, "sfc_order", False) else ""),
         "n_particles": ps.n, "n_active": ps.n if active is None else int(len(active)),
         "kernel": "wendland_c6" if ps.kernel == 1 else "cubic_spline", "n_ngb": ps.n_ngb, "n_tol": ps.n_tol,
         "step": "sph_build_index + sph_density(h iteration) + sph_hydro_force",
@@ -241,6 +266,8 @@ def main():
     ap.add_argument("--kdk-steps", type=int, default=0,
                     help="after the timed region, run this many steps of the kick-drift-kick driver (SURVEY.md 8(f)-3) on the "
                          "workload and report active counts and times per step")
+    ap.add_argument("--sfc-order", action="store_true",
+                    help="hand the particle set over in Morton order of the positions (variant run; default: generator order)")
     ap.add_argument("--kdk-refresh-max", type=int, default=16,
                     help="sph_kdk_params.refresh_max: steps in a row that refresh the index instead of rebuilding it (0 = never)")
     ap.add_argument("--group-cap", type=int, default=0, help="actives per group (0 = library default)")
@@ -269,6 +296,8 @@ def main():
     n = ps.n
     w = args.workload.upper()
     active_np = I.config5_active(ps) if w == "C5" else None
+    if args.sfc_order:
+        active_np = sfc_order(ps, active_np)
     dev = lambda a, dt=torch.float32: torch.from_numpy(np.ascontiguousarray(a)).to(dt).cuda()
     pos, vel, u, h_guess = dev(ps.pos), dev(ps.vel), dev(ps.u), dev(ps.h_guess)
     active = None if active_np is None else dev(active_np, torch.int32)
