@@ -92,8 +92,7 @@ struct Frame {
 // evaluate the m newest queued hits of every lane (n = warp-wide maximum of m)
 // WRAP: 0 raw coordinate differences, 1 recentred frame, 2 per-pair nearest image
 template <int KERNEL, int WRAP, int MODE>
-__device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
-                                      const Frame &fr)
+__device__ __forceinline__ void drain(const ForceArgs &a, uint32_t q0, ForceLane &A, int n, const Frame &fr)
 {
     const int m = min(n, A.cnt), base = A.cnt - m;
     const float L = a.L, alpha = a.alpha;
@@ -103,10 +102,12 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
     // the hits of one call (at most a queue's worth: 32) are summed in fp32, the calls in fp64: the accumulators of
     // R15 stay out of the inner loop's registers at no measurable cost in accuracy
     float sx = 0.f, sy = 0.f, sz = 0.f, su = 0.f;
+    uint32_t qa = q0 + (uint32_t)base * 128u; // shared-memory address of the next queued hit (q0: the lane's entry 0)
 #pragma unroll 2
     for (int k = 0; k < n; k++) {
         if (k < m) {
-            const uint32_t j = lds_u32(smem_u32(qp + (base + k) * 32)); // (volatile: ordered after the pushes)
+            const uint32_t j = lds_u32(qa); // (volatile: ordered after the pushes)
+            qa += 128u;
             const float4 P0 = __ldg(a.xyzh + j), P1 = __ldg(a.vc + 2 * (size_t)j), P2 = __ldg(a.vc + 2 * (size_t)j + 1);
             float dx, dy, dz;
             if (WRAP == 2) {
@@ -121,7 +122,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
             // dominated by the error of r amplified by w''/w' (~10), and a sum of ~500 such terms is compared
             // with 1e-7 of the sum of their magnitudes (R15)
             const float r2c = fmaxf(r2, 1e-37f);
-            float rinv = rsqrtf(r2c);
+            float rinv = rsqrt_ftz(r2c);
             rinv = rinv * fmaf(-0.5f * r2c, rinv * rinv, 1.5f);
             const float r = r2 * rinv;
             const bool other = j != A.slot; // j == i: no self force, no self signal velocity
@@ -163,7 +164,7 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
                 const float Pj = a.gm1 * P2.x * E.z;
                 cond = a.alpha_cond * sqrtf(fabsf(A.P - Pj) * rbi) * (A.u - E.z) * Fbar * rbi;   // R20
             } else {
-                Pi = -alpha * vs * mu * __fdividef(1.f, A.rho + P2.x);
+                Pi = -alpha * vs * mu * rcp_ftz(A.rho + P2.x);
             }
             const float AiFi = A.A * Fi;
             const float pv = Pi * Fbar;
@@ -183,19 +184,18 @@ __device__ __forceinline__ void drain(const ForceArgs &a, const uint32_t *__rest
 }
 
 template <int KERNEL, int MODE>
-__device__ __forceinline__ void drain_any(const ForceArgs &a, const uint32_t *__restrict__ qp, ForceLane &A, int n,
-                                          const Frame &fr)
+__device__ __forceinline__ void drain_any(const ForceArgs &a, uint32_t q0, ForceLane &A, int n, const Frame &fr)
 {
-    if (fr.pairwrap) drain<KERNEL, 2, MODE>(a, qp, A, n, fr);
-    else if (fr.rec) drain<KERNEL, 1, MODE>(a, qp, A, n, fr);
-    else drain<KERNEL, 0, MODE>(a, qp, A, n, fr);
+    if (fr.pairwrap) drain<KERNEL, 2, MODE>(a, q0, A, n, fr);
+    else if (fr.rec) drain<KERNEL, 1, MODE>(a, q0, A, n, fr);
+    else drain<KERNEL, 0, MODE>(a, q0, A, n, fr);
 }
 
 // Test the candidate pairs of the gathered chunk against this lane's active (symmetric set, R10):
 // hit if r^2 < max(H_i, H_j)^2; a hit pushes the candidate's sorted slot onto the lane's queue.
 template <int KERNEL, bool PAIRWRAP, int MODE>
 __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *__restrict__ slotp,
-                                              const uint32_t *__restrict__ gp, uint32_t *__restrict__ qp, ForceLane &A,
+                                              const uint32_t *__restrict__ gp, uint32_t q0, ForceLane &A,
                                               int s, int f, bool live, const Frame &fr)
 {
     const int steps = (SPH_CH / 2) / f;
@@ -211,9 +211,8 @@ __device__ __forceinline__ void consume_chunk(const ForceArgs &a, const float4 *
         const int mx = __reduce_max_sync(FULLMASK, A.cnt);
         if (mx + 2 * nt > SPH_QCAP_FORCE) {
             const int mn = __reduce_min_sync(FULLMASK, live ? A.cnt : 0x7fffffff);
-            drain_any<KERNEL, MODE>(a, qp, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
+            drain_any<KERNEL, MODE>(a, q0, A, max(mn, mx + 2 * nt - SPH_QCAP_FORCE), fr);
         }
-        const uint32_t q0 = smem_u32(qp);
         uint32_t qw = q0 + (uint32_t)A.cnt * 128u;
 #pragma unroll 2
         for (int t = 0; t < nt; t++) {
@@ -256,7 +255,7 @@ __global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_
     if (a.cnt->err | a.cnt->idx_err) return; // a precondition failed (ids, h, state, positions): compute nothing (uniform over the grid)
     const unsigned int n_groups = *a.n_groups;
     unsigned long long st_cands = 0, st_pairs = 0;
-    uint32_t *qp = W.q + lane;
+    const uint32_t q0 = smem_u32(W.q + lane); // shared-memory address of entry 0 of this lane's hit queue
 
     unsigned int gnext = 0, gend = 0; // this warp's block of consecutive groups
     for (;;) {
@@ -321,7 +320,7 @@ __global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_
                 cands += ctl.total;
                 // queued hits of an earlier batch are evaluated in the frame they were found in
                 if (ctl.pairwrap != fr.pairwrap || ctl.thx != fr.thx || ctl.thy != fr.thy || ctl.thz != fr.thz) {
-                    drain_any<KERNEL, MODE>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+                    drain_any<KERNEL, MODE>(a, q0, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
                     fr.thx = ctl.thx; fr.thy = ctl.thy; fr.thz = ctl.thz; fr.pairwrap = ctl.pairwrap;
                     fr.rec = ctl.thx < 1e30f || ctl.thy < 1e30f || ctl.thz < 1e30f;
                 }
@@ -333,11 +332,11 @@ __global__ void __launch_bounds__(SPH_THREADS, MODE == MODE_IMPROVED ? SPH_CTAS_
                     GatherRegs G;
                     gather_load(W.ws, ctl, gc, c, G, a.xyzh);
                     gather_store<true, true>(ctl, G, W.slot, W.gidx, L);
-                    if (fr.pairwrap) consume_chunk<KERNEL, true, MODE>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
-                    else consume_chunk<KERNEL, false, MODE>(a, W.slot, W.gidx, qp, A, s, f, live, fr);
+                    if (fr.pairwrap) consume_chunk<KERNEL, true, MODE>(a, W.slot, W.gidx, q0, A, s, f, live, fr);
+                    else consume_chunk<KERNEL, false, MODE>(a, W.slot, W.gidx, q0, A, s, f, live, fr);
                 }
             } while (ctl.sp > 0);
-            drain_any<KERNEL, MODE>(a, qp, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
+            drain_any<KERNEL, MODE>(a, q0, A, __reduce_max_sync(FULLMASK, A.cnt), fr);
             // cross-stream totals
             double X = A.px, Y = A.py, Z = A.pz, U = A.pdu;
             float V = A.pvs;

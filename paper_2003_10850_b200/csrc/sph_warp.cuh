@@ -239,6 +239,21 @@ struct GatherCtl { // warp-uniform registers
     int kseg; // first segment that overlaps the next chunk to gather
 };
 
+// MUFU.RSQ / MUFU.RCP without the denormal scaling the C intrinsics wrap around them (arguments here are normal numbers:
+// r^2 clamped to >= 1e-37, a sum of two densities); for normal arguments the results are those of rsqrtf / __fdividef(1, x)
+__device__ __forceinline__ float rsqrt_ftz(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_ftz(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 __device__ __forceinline__ float4 ldg_nc(const float4 *p)
 {
     float4 v;
