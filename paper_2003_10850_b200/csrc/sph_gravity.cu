@@ -41,9 +41,9 @@ struct GravWarp {
 __device__ __forceinline__ float grav_pair(const GravArgs &a, float r2, float m)
 {
     const float s2 = r2 + a.eps2;
-    const float ri = rsqrtf(s2);
-    const float r = r2 * rsqrtf(fmaxf(r2, 1e-37f)), x = r * a.hrs;
-    const float t = __fdividef(1.f, fmaf(0.3275911f, x, 1.f));
+    const float ri = rsqrt_ftz(fmaxf(s2, 1e-37f));
+    const float r = r2 * rsqrt_ftz(fmaxf(r2, 1e-37f)), x = r * a.hrs;
+    const float t = rcp_ftz(fmaf(0.3275911f, x, 1.f));
     const float P = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.061405429f, -1.453152027f), 1.421413741f), -0.284496736f), 0.254829592f);
     const float fac = __expf(-x * x) * fmaf(1.1283791670955126f, x, P);
     return r2 < a.rcut2 ? a.G * m * fac * ri * ri * ri : 0.f;
