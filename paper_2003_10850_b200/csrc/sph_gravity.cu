@@ -8,6 +8,8 @@
 // warp walks for a group of <= 32 neighbouring active particles and collects an interaction list of accepted nodes
 // (monopoles: centre of mass, mass) and of leaf particle runs, which is then evaluated by all lanes -- so the pair
 // arithmetic is separated from the walk branch.
+#include <type_traits>
+
 #include "sph_warp.cuh"
 
 namespace {
@@ -79,6 +81,8 @@ __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
         const float gcx = 0.5f * (x0 + x1), ghx = 0.5f * (x1 - x0) * (1.f + 1e-6f);
         const float gcy = 0.5f * (y0 + y1), ghy = 0.5f * (y1 - y0) * (1.f + 1e-6f);
         const float gcz = 0.5f * (z0 + z1), ghz = 0.5f * (z1 - z0) * (1.f + 1e-6f);
+        const float rcw = a.rcut * (1.f + 1e-5f);
+        const bool plain = x0 - rcw >= 0.f && x1 + rcw < L && y0 - rcw >= 0.f && y1 + rcw < L && z0 - rcw >= 0.f && z1 + rcw < L;
         double ax = 0.0, ay = 0.0, az = 0.0;
         int sp = 0;
         int nseg = 0, nmono = 0;
@@ -127,13 +131,15 @@ __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
                 nseg += __popc(me); nmono += __popc(ma); sp += __popc(mp);
                 __syncwarp();
             }
+            auto evaluate = [&](auto plain_c) {
+                constexpr bool PLAIN = decltype(plain_c)::value;
             // evaluate: lane = (active, stream); the streams split the accepted nodes and the flat sequence of the leaf
             // runs' particles; 16 terms at a time are summed in fp32, those sums in fp64
             if (live) {
                 float bx = 0.f, by = 0.f, bz = 0.f;
                 for (int i = s; i < nmono; i += f) {
                     const float4 q = W.mono[i];
-                    const float ddx = image_diff(pi.x, q.x, L), ddy = image_diff(pi.y, q.y, L), ddz = image_diff(pi.z, q.z, L);
+                    const float ddx = (PLAIN ? pi.x - q.x : image_diff(pi.x, q.x, L)), ddy = (PLAIN ? pi.y - q.y : image_diff(pi.y, q.y, L)), ddz = (PLAIN ? pi.z - q.z : image_diff(pi.z, q.z, L));
                     const float t = grav_pair(a, fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)), q.w);
                     bx = fmaf(-t, ddx, bx); by = fmaf(-t, ddy, by); bz = fmaf(-t, ddz, bz);
                 }
@@ -149,7 +155,7 @@ __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
                         }
                         if (k >= nseg) break;
                         const float4 q = __ldg(a.xyzm + j);
-                        const float ddx = image_diff(pi.x, q.x, L), ddy = image_diff(pi.y, q.y, L), ddz = image_diff(pi.z, q.z, L);
+                        const float ddx = (PLAIN ? pi.x - q.x : image_diff(pi.x, q.x, L)), ddy = (PLAIN ? pi.y - q.y : image_diff(pi.y, q.y, L)), ddz = (PLAIN ? pi.z - q.z : image_diff(pi.z, q.z, L));
                         const float t = j != slot ? grav_pair(a, fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx)), q.w) : 0.f;
                         bx = fmaf(-t, ddx, bx); by = fmaf(-t, ddy, by); bz = fmaf(-t, ddz, bz);
                         j += (uint32_t)f;
@@ -162,6 +168,11 @@ __global__ void __launch_bounds__(SPH_THREADS) k_gravity(GravArgs a)
                 }
                 ax += (double)bx; ay += (double)by; az += (double)bz;
             }
+            };
+            // no wall within r_cut of the group: every pair closer than r_cut has its nearest image at the plain difference,
+            // and a plain difference is never shorter than the nearest-image one (pairs beyond r_cut contribute nothing)
+            if (plain) evaluate(std::true_type());
+            else evaluate(std::false_type());
             nseg = nmono = 0;
             __syncwarp();
         }
