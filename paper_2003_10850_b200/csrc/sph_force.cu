@@ -151,18 +151,18 @@ __device__ __forceinline__ void drain(const ForceArgs &a, uint32_t q0, ForceLane
                 // R21: m_j / (rho_i rho_j) * 4 k_i k_j / (k_i + k_j) * (T_i - T_j) * Fbar / r
                 const float4 E = __ldg(a.ext + j); // kappa_j, T_j
                 const float ks = A.al + E.x;
-                const float kij = ks > 0.f ? 4.f * A.al * E.x / ks : 0.f;
-                const float e = other ? P2.z / (A.rho * P2.x) * kij * (A.u - E.y) * Fbar * rinv : 0.f;
+                const float kij = ks > 0.f ? 4.f * A.al * E.x * rcp_ftz(ks) : 0.f;
+                const float e = other ? P2.z * rcp_ftz(A.rho * P2.x) * kij * (A.u - E.y) * Fbar * rinv : 0.f;
                 su += e;
                 continue;
             }
             float Pi, cond = 0.f;
             if (MODE == MODE_IMPROVED) {
                 const float4 E = __ldg(a.ext + j);                         // alpha_j, f_j, u_j
-                const float rbi = 2.f / (A.rho + P2.x);                    // 1 / rho_bar
+                const float rbi = 2.f * rcp_ftz(A.rho + P2.x);                    // 1 / rho_bar
                 Pi = -0.25f * (A.al + E.x) * vs * mu * rbi * 0.5f * (A.fb + E.y);               // R9 with R18, R19
                 const float Pj = a.gm1 * P2.x * E.z;
-                cond = a.alpha_cond * sqrtf(fabsf(A.P - Pj) * rbi) * (A.u - E.z) * Fbar * rbi;   // R20
+                cond = a.alpha_cond * sqrt_ftz(fabsf(A.P - Pj) * rbi) * (A.u - E.z) * Fbar * rbi;   // R20
             } else {
                 Pi = -alpha * vs * mu * rcp_ftz(A.rho + P2.x);
             }
