@@ -47,7 +47,7 @@ __device__ __forceinline__ float grav_pair(const GravArgs &a, float r2, float m)
     const float r = r2 * rsqrt_ftz(fmaxf(r2, 1e-37f)), x = r * a.hrs;
     const float t = rcp_ftz(fmaf(0.3275911f, x, 1.f));
     const float P = t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, 1.061405429f, -1.453152027f), 1.421413741f), -0.284496736f), 0.254829592f);
-    const float fac = __expf(-x * x) * fmaf(1.1283791670955126f, x, P);
+    const float fac = ex2_ftz(-1.4426950408889634f * x * x) * fmaf(1.1283791670955126f, x, P); // exp(-x^2), x <= r_cut / 2 r_s
     return r2 < a.rcut2 ? a.G * m * fac * ri * ri * ri : 0.f;
 }
 

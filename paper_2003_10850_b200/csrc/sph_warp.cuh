@@ -253,6 +253,12 @@ __device__ __forceinline__ float sqrt_ftz(float x)
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float ex2_ftz(float x) // 2^x, MUFU.EX2 without the range wrapper of __expf (|x| small here)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float rcp_ftz(float x)
 {
     float y;
