@@ -78,3 +78,33 @@ def test_noalloc_compaction_allocates_nothing_and_rejects_oversize():
     torch.cuda.synchronize()
     assert int(cnt.cpu().numpy()[0]) == 0
     sph.close()
+
+
+def test_noalloc_compaction_under_cuda_graph_capture():
+    """The use case: the call is captured into a CUDA graph (stream capture forbids cudaMalloc / cudaFree) and replayed on
+    new flags; the allocating path is not captured.  The first call on the device is made before the capture."""
+    s = torch.cuda.Stream()
+    sph = B.Sph(stream=s)
+    n = 300_000
+    f_np = _flags(n, 0.3, 21)
+    flags = torch.from_numpy(f_np).cuda()
+    ids = torch.full((n,), -1, device="cuda", dtype=torch.int32)
+    cnt = torch.zeros(1, device="cuda", dtype=torch.int32).view(torch.uint32)
+    with torch.cuda.stream(s):
+        sph.sph_compact_flags(flags, ids, cnt, noalloc=True)  # set-up call, not captured
+    s.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        sph.sph_compact_flags(flags, ids, cnt, noalloc=True)
+    for seed in (22, 23):
+        f_np = _flags(n, 0.1 * (seed - 20), seed)
+        flags.copy_(torch.from_numpy(f_np).cuda())
+        ids.fill_(-1)
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        want = np.flatnonzero(f_np).astype(np.int32)
+        c = int(cnt.cpu().numpy()[0])
+        assert c == len(want) and np.array_equal(ids.cpu().numpy()[:c], want)
+    del g
+    sph.close()
