@@ -305,7 +305,10 @@ def main():
     rho, om, du, vs = (torch.zeros(n, device="cuda") for _ in range(4))
     ngb = torch.zeros(n, device="cuda", dtype=torch.int32)
     acc = torch.zeros((n, 3), device="cuda")
-    stream = torch.cuda.current_stream()
+    # a stream of its own (the legacy default stream cannot be captured: sph_build_index replays its launches from a CUDA
+    # graph from the third identical call on); every torch operation of the bench runs on it as well
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
     sph = B.Sph(kernel=ps.kernel, stream=stream, group_cap=args.group_cap, group_node=args.group_node)
     n_active = n if active is None else int(active.numel())
     flush = None if n * 76 > 126e6 else torch.empty(64 << 20, device="cuda", dtype=torch.float32)

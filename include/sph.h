@@ -114,6 +114,9 @@ int sph_destroy(sph_ctx *ctx);
  * n = 0 is valid (later calls do nothing).  Asynchronous.  If the octree node pool runs out (more than
  * about two nodes per particle: extremely clumped input) the remaining cells stay oversize leaves: results
  * are unaffected, the gather slows down, and sph_stats.node_pool_overflow reports it.
+ * Small sets are bound by the ~45 dependent kernel launches of the build: from the second call in a row with the same
+ * (n, pos, mass, mass_scalar) on, the launch sequence is captured into a CUDA graph and replayed (same kernels, same
+ * arguments, current contents of the arrays; not on the legacy default stream, which cannot be captured).
  */
 int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass, float mass_scalar);
 

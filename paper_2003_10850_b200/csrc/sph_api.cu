@@ -119,6 +119,7 @@ int sph_destroy(sph_ctx *ctx)
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
     dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
     for (int i = 0; i < 8; i++) cudaEventDestroy(ctx->ev[i]);
+    if (ctx->idx_graph) cudaGraphExecDestroy(ctx->idx_graph);
     if (ctx->copy_stream) {
         cudaStreamSynchronize(ctx->copy_stream);
         for (int i = 0; i < 4; i++) cudaEventDestroy(ctx->cev[i]);
@@ -141,9 +142,60 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
     ctx->has_mass = mass != nullptr;
     ctx->mass_scalar = mass ? 1.f : mass_scalar;
     ctx->err[0] = 0;
-    cudaEventRecord(ctx->ev[0], ctx->stream);
-    rc = sph_index_build(ctx, pos, mass);
-    cudaEventRecord(ctx->ev[1], ctx->stream);
+    cudaStream_t st = ctx->stream;
+    cudaEventRecord(ctx->ev[0], st);
+    const float ms = ctx->mass_scalar;
+    if (ctx->idx_graph && n == ctx->gk_n && pos == ctx->gk_pos && mass == ctx->gk_mass && ms == ctx->gk_ms) {
+        // replay: the same kernels with the same arguments, reading the arrays' current contents
+        SPH_CUDA(ctx, cudaGraphLaunch(ctx->idx_graph, st));
+        ctx->launches += ctx->idx_graph_launches;
+        ctx->have_index = true;
+        rc = SPH_OK;
+    } else {
+        const bool same = n > 0 && n == ctx->lk_n && pos == ctx->lk_pos && mass == ctx->lk_mass && ms == ctx->lk_ms;
+        bool capturable = st != nullptr && st != cudaStreamLegacy && !ctx->idx_graph_off;
+        if (capturable && same) { // (a caller that is capturing the stream itself gets plain launches into its own graph)
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+            if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+                cudaGetLastError();
+                capturable = false;
+            }
+        }
+        bool done = false;
+        if (same && capturable) { // (same n as the last build: every buffer is already large enough, nothing allocates)
+            if (ctx->idx_graph) { cudaGraphExecDestroy(ctx->idx_graph); ctx->idx_graph = nullptr; }
+            cudaGraph_t graph = nullptr;
+            const int64_t l0 = ctx->launches;
+            if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                const int rcb = sph_index_build(ctx, pos, mass);
+                const cudaError_t e = cudaStreamEndCapture(st, &graph);
+                if (rcb == SPH_OK && e == cudaSuccess && graph &&
+                    cudaGraphInstantiate(&ctx->idx_graph, graph, 0) == cudaSuccess &&
+                    cudaGraphLaunch(ctx->idx_graph, st) == cudaSuccess) {
+                    ctx->gk_n = n; ctx->gk_pos = pos; ctx->gk_mass = mass; ctx->gk_ms = ms;
+                    ctx->idx_graph_launches = ctx->launches - l0;
+                    done = true;
+                    rc = SPH_OK;
+                } else {
+                    if (ctx->idx_graph) { cudaGraphExecDestroy(ctx->idx_graph); ctx->idx_graph = nullptr; }
+                    ctx->idx_graph_off = true;
+                    ctx->launches = l0;
+                    ctx->have_index = false;
+                    ctx->err[0] = 0;
+                    cudaGetLastError();
+                }
+                if (graph) cudaGraphDestroy(graph);
+            } else {
+                cudaGetLastError();
+                ctx->idx_graph_off = true;
+            }
+        }
+        if (!done) {
+            rc = sph_index_build(ctx, pos, mass);
+            ctx->lk_n = n; ctx->lk_pos = pos; ctx->lk_mass = mass; ctx->lk_ms = ms;
+        }
+    }
+    cudaEventRecord(ctx->ev[1], st);
     ctx->ev_set[0] = true;
     return rc;
 }

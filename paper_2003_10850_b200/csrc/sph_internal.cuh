@@ -137,6 +137,16 @@ struct sph_ctx {
 
     // phase timing: events recorded on the stream around the phases named in sph_stats
     cudaEvent_t ev[8]; // 0,1 index  2,3 density kernel  4,5 force prep  6,7 force kernel
+    // sph_build_index, launch-bound for small sets (~45 dependent launches): the second call in a row with the same
+    // (n, pos, mass, mass_scalar) captures the launch sequence into a CUDA graph, later ones replay it (not on the legacy
+    // default stream, which cannot be captured)
+    cudaGraphExec_t idx_graph;
+    const float *gk_pos, *gk_mass; // key of the graph (idx_graph != NULL) ...
+    const float *lk_pos, *lk_mass; // ... and of the last direct build
+    int64_t gk_n, lk_n;
+    float gk_ms, lk_ms;
+    int64_t idx_graph_launches;
+    bool idx_graph_off;            // capture failed once: stay with direct launches
     cudaStream_t copy_stream; // sph_step_host: host copies that overlap the kernels (created at first use)
     cudaEvent_t cev[4];       // sph_step_host: positions up / velocities, energies up / density results final / h up
     bool ev_set[4];
