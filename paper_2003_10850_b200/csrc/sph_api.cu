@@ -192,7 +192,8 @@ int sph_build_index(sph_ctx *ctx, int64_t n, const float *pos, const float *mass
         }
         if (!done) {
             rc = sph_index_build(ctx, pos, mass);
-            ctx->lk_n = n; ctx->lk_pos = pos; ctx->lk_mass = mass; ctx->lk_ms = ms;
+            ctx->lk_n = rc == SPH_OK ? n : -1; // (a failed build is never the template of a capture)
+            ctx->lk_pos = pos; ctx->lk_mass = mass; ctx->lk_ms = ms;
         }
     }
     cudaEventRecord(ctx->ev[1], st);
