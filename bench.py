@@ -469,7 +469,7 @@ def main():
         t_e2e = sum(tt[1:])  # first call (allocations) is warm-up
         t_e2e = max_over_ranks(t_e2e, world, "cuda")
         h2d = n * 32 + (0 if hact is None else 4 * len(active_np) + 8 * n)
-        d2h = n * 44
+        d2h = n * 44 if hact is None else 36 * len(active_np)  # an active list: only the actives' results travel back
         e2e = {"value": world * n_active * args.steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * t_e2e / args.steps}
         sph2.close()

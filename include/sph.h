@@ -282,9 +282,9 @@ int sph_kdk_step(sph_ctx *ctx, int64_t n, float mass_scalar, const sph_kdk_param
 /*
  * One whole pass of the hot path with HOST buffers (used for the end-to-end measurement): copies
  * pos, vel, u, h (guess) [and active ids] to the device, runs sph_build_index, sph_density and
- * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back (whole arrays; entries
- * of inactive particles of the outputs rho..vsig_max are unspecified unless the caller pre-filled the
- * device state through an earlier call), and synchronises.  All pointers are HOST pointers;
+ * sph_hydro_force, copies h, rho, omega, ngb_count, acc, dudt, vsig_max back -- the whole arrays when all
+ * particles are active; with an active list only the active particles' entries travel (packed on the device,
+ * 36 bytes each) and the other entries of the caller's arrays are left as they are --, and synchronises.  All pointers are HOST pointers;
  * `active_host` may be NULL (all active).  With PINNED host memory the copies overlap the kernels on a
  * second stream of the context: h, vel and u go up while the index is built and the density runs, h, rho,
  * omega and ngb_count come down while the force pass runs; only pos (up) and acc, dudt, vsig_max (down)

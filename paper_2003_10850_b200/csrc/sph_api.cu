@@ -51,6 +51,26 @@ int report(sph_ctx *ctx, const char *where, unsigned int err, unsigned int idx_e
                     (idx_err & SPH_ERR_POS) ? " position outside [0, box) in sph_build_index (rebuild the index);" : "");
 }
 
+// sph_step_host with an active list: the results of the active particles only, packed array after array
+// (h, rho, omega, ngb, acc[3], dudt, vsig: 9 words per active particle)
+__global__ void k_pack_active(int64_t na, const int32_t *__restrict__ active, const float *__restrict__ h, const float *__restrict__ rho,
+                              const float *__restrict__ omega, const int32_t *__restrict__ ngb, const float *__restrict__ acc,
+                              const float *__restrict__ dudt, const float *__restrict__ vsig, uint32_t *__restrict__ pack)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= na) return;
+    const int64_t i = active[k];
+    pack[k] = __float_as_uint(h[i]);
+    pack[na + k] = __float_as_uint(rho[i]);
+    pack[2 * na + k] = __float_as_uint(omega[i]);
+    pack[3 * na + k] = (uint32_t)ngb[i];
+    pack[4 * na + 3 * k] = __float_as_uint(acc[3 * i]);
+    pack[4 * na + 3 * k + 1] = __float_as_uint(acc[3 * i + 1]);
+    pack[4 * na + 3 * k + 2] = __float_as_uint(acc[3 * i + 2]);
+    pack[7 * na + k] = __float_as_uint(dudt[i]);
+    pack[8 * na + k] = __float_as_uint(vsig[i]);
+}
+
 int check_sticky(sph_ctx *ctx)
 {
     cudaError_t e = cudaPeekAtLastError();
@@ -117,7 +137,8 @@ int sph_destroy(sph_ctx *ctx)
     dfree(ctx->node_hmax); dfree(ctx->node_slack); dfree(ctx->kdk_grav); dfree(ctx->node_mom); dfree(ctx->act_slot); dfree(ctx->act_slot_alt); dfree(ctx->act_flag);
     dfree(ctx->agrp_start);
     dfree(ctx->d_pos); dfree(ctx->d_vel); dfree(ctx->d_u); dfree(ctx->d_h); dfree(ctx->d_rho); dfree(ctx->d_omega);
-    dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active);
+    dfree(ctx->d_acc); dfree(ctx->d_dudt); dfree(ctx->d_vsig); dfree(ctx->d_ngb); dfree(ctx->d_active); dfree(ctx->d_pack);
+    if (ctx->h_pack) cudaFreeHost(ctx->h_pack);
     for (int i = 0; i < 8; i++) cudaEventDestroy(ctx->ev[i]);
     if (ctx->idx_graph) cudaGraphExecDestroy(ctx->idx_graph);
     if (ctx->copy_stream) {
@@ -409,6 +430,42 @@ int sph_step_host(sph_ctx *ctx, int64_t n, const float *pos_host, const float *v
                          ctx->d_dudt, ctx->d_vsig);
     ctx->act_keep = false;
     if (rc) { cudaStreamSynchronize(cs); return rc; }
+    if (act && n_active > 0) {
+        // an active list: only the active particles' results travel (9 words each instead of 11 per particle of the set);
+        // the entries of the other particles in the caller's arrays stay as they are
+        const int64_t na = n_active;
+        if (na > ctx->cap_pack) {
+            ctx->cap_pack = 0;
+            dfree(ctx->d_pack);
+            if (ctx->h_pack) { cudaFreeHost(ctx->h_pack); ctx->h_pack = nullptr; }
+            const int64_t cap = na + na / 8 + 1024;
+            SPH_CUDA(ctx, cudaMalloc((void **)&ctx->d_pack, 9 * (size_t)cap * sizeof(uint32_t)));
+            SPH_CUDA(ctx, cudaMallocHost((void **)&ctx->h_pack, 9 * (size_t)cap * sizeof(uint32_t)));
+            ctx->cap_pack = cap;
+        }
+        k_pack_active<<<(int)((na + 255) / 256), 256, 0, st>>>(na, act, ctx->d_h, ctx->d_rho, ctx->d_omega, ctx->d_ngb, ctx->d_acc,
+                                                               ctx->d_dudt, ctx->d_vsig, ctx->d_pack);
+        ctx->launches++;
+        SPH_CUDA(ctx, cudaMemcpyAsync(ctx->h_pack, ctx->d_pack, 9 * (size_t)na * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        SPH_CUDA(ctx, cudaStreamSynchronize(st));
+        SPH_CUDA(ctx, cudaStreamSynchronize(cs));
+        SPH_CUDA(ctx, cudaGetLastError());
+        const float *pf = reinterpret_cast<const float *>(ctx->h_pack);
+        const int32_t *pi = reinterpret_cast<const int32_t *>(ctx->h_pack);
+        for (int64_t k = 0; k < na; k++) { // (the ids were checked on the device: a bad list returned above)
+            const int64_t i = active_host[k];
+            h_host[i] = pf[k];
+            rho_host[i] = pf[na + k];
+            omega_host[i] = pf[2 * na + k];
+            ngb_count_host[i] = pi[3 * na + k];
+            acc_host[3 * i] = pf[4 * na + 3 * k];
+            acc_host[3 * i + 1] = pf[4 * na + 3 * k + 1];
+            acc_host[3 * i + 2] = pf[4 * na + 3 * k + 2];
+            dudt_host[i] = pf[7 * na + k];
+            vsig_host[i] = pf[8 * na + k];
+        }
+        return rcd;
+    }
     // the density results go down on the copy stream while the force pass runs (enqueued AFTER the force kernels:
     // enqueued before them, the copies held the kernels back by their whole duration -- measured, 4.2 ms at 10^7)
     SPH_CUDA(ctx, cudaStreamWaitEvent(cs, ctx->cev[2], 0));

@@ -131,6 +131,8 @@ struct sph_ctx {
     int64_t cap_host;
     float *d_pos, *d_vel, *d_u, *d_h, *d_rho, *d_omega, *d_acc, *d_dudt, *d_vsig;
     int32_t *d_ngb, *d_active;
+    uint32_t *d_pack, *h_pack;   // sph_step_host with an active list: the actives' results packed (device / pinned host), 9 words each
+    int64_t cap_pack;
 
     int64_t launches;
     int64_t kdk_tick;  // sph_kdk_*: current tick of the integer timeline

@@ -330,6 +330,41 @@ def test_step_host_matches_device_calls():
     g.close()
 
 
+def test_step_host_with_an_active_list():
+    """Host-buffer pass with an active list: the active entries equal those of the device calls, the others are untouched
+    (only the actives' results travel back)."""
+    ps = I.config3(12000, 3)
+    n = ps.n
+    o_all = GpuRun(ps.pos, 0, ps.mass)
+    full = o_all.density(ps.h_guess, 64, 2)
+    act = np.sort(np.random.default_rng(8).choice(n, 900, replace=False)).astype(np.int32)
+    hg = I.perturb_h(full["H"], act, 77)
+    gd = o_all.density(hg, 64, 2, active=act)
+    H = hg.copy(); H[act] = gd["H"][act]
+    rho = full["rho"].copy(); rho[act] = gd["rho"][act]
+    om = full["omega"].copy(); om[act] = gd["omega"][act]
+    gf = o_all.force(ps.vel, ps.u, H, rho, om, active=act)
+    o_all.close()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h, r_, o_ = pin(hg.copy()), pin(full["rho"].copy()), pin(full["omega"].copy())
+    ngb = torch.full((n,), -5, dtype=torch.int32).pin_memory()
+    acc = torch.full((n, 3), 7.0).pin_memory()
+    du, vs = torch.full((n,), 7.0).pin_memory(), torch.full((n,), 7.0).pin_memory()
+    sph = B.Sph(kernel=0)
+    for _ in range(2):  # (the second call reuses the packed buffers)
+        h.copy_(torch.from_numpy(hg))
+        unconv = sph.sph_step_host(pin(ps.pos), pin(ps.vel), pin(ps.u), ps.mass, h, r_, o_, ngb, acc, du, vs, 64, 2, active=pin(act))
+        assert unconv == 0
+        assert np.array_equal(h.numpy()[act], gd["H"][act]) and np.array_equal(ngb.numpy()[act], gd["Nint"][act])
+        assert np.allclose(r_.numpy()[act], gd["rho"][act], rtol=1e-6)
+        assert np.allclose(acc.numpy()[act], gf["acc"][act], rtol=1e-4, atol=1e-6 * np.abs(gf["acc"][act]).max())
+        assert np.allclose(vs.numpy()[act], gf["vsig"][act], rtol=1e-6)
+        inact = np.ones(n, bool); inact[act] = False
+        assert np.all(acc.numpy()[inact] == 7.0) and np.all(ngb.numpy()[inact] == -5) and np.all(du.numpy()[inact] == 7.0)
+        assert np.array_equal(h.numpy()[inact], hg[inact]) and np.array_equal(r_.numpy()[inact], full["rho"][inact])
+    sph.close()
+
+
 def test_errors_are_return_codes():
     sph = B.Sph(kernel=0)
     z = torch.zeros(4, device="cuda")
