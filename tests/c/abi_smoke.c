@@ -90,6 +90,30 @@ int main(void)
     CHECK(cudaMemcpy(ngb2, d_ngb, sizeof ngb2, cudaMemcpyDeviceToHost) == cudaSuccess);
     for (int i = 0; i < N; i++) CHECK(ngb2[i] == ngb[i]);
 
+    /* flags -> ascending id list, with the context's scratch and with the fixed device scratch */
+    {
+        static uint32_t fl[N];
+        static int32_t idl[2][N];
+        uint32_t cnt[2] = {77u, 77u};
+        int want = 0;
+        for (int i = 0; i < N; i++) { fl[i] = (i % 3 == 1) || (i > N - 5); want += (int)fl[i]; }
+        uint32_t *d_fl = dev(fl, sizeof fl), *d_cnt = dev(NULL, sizeof cnt);
+        int32_t *d_id0 = dev(NULL, sizeof idl[0]), *d_id1 = dev(NULL, sizeof idl[1]);
+        CHECK(d_fl && d_cnt && d_id0 && d_id1);
+        CHECK(sph_compact_flags(ctx, N, d_fl, d_id0, d_cnt) == SPH_OK);
+        CHECK(sph_compact_flags_noalloc(ctx, N, d_fl, d_id1, d_cnt + 1) == SPH_OK);
+        CHECK(sph_compact_flags_noalloc(ctx, (int64_t)SPH_COMPACT_NOALLOC_MAX + 1, d_fl, d_id1, d_cnt + 1) == SPH_E_ARG);
+        CHECK(cudaDeviceSynchronize() == cudaSuccess);
+        CHECK(cudaMemcpy(cnt, d_cnt, sizeof cnt, cudaMemcpyDeviceToHost) == cudaSuccess);
+        CHECK(cudaMemcpy(idl[0], d_id0, sizeof idl[0], cudaMemcpyDeviceToHost) == cudaSuccess);
+        CHECK(cudaMemcpy(idl[1], d_id1, sizeof idl[1], cudaMemcpyDeviceToHost) == cudaSuccess);
+        CHECK((int)cnt[0] == want && (int)cnt[1] == want);
+        for (int k = 0, i = 0; k < want; k++, i++) {
+            while (!fl[i]) i++;
+            CHECK(idl[0][k] == i && idl[1][k] == i);
+        }
+    }
+
     /* a support radius >= box / 2 among the guesses: nothing is computed, SPH_E_HRANGE */
     h[7] = 0.75f;
     CHECK(cudaMemcpy(d_h, h, sizeof h, cudaMemcpyHostToDevice) == cudaSuccess);
